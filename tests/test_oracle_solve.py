@@ -164,7 +164,7 @@ def test_P9_krylov_invariants(oracle_mod):
         y, res, *_ = np.linalg.lstsq(Hj, e1, rcond=None)
         xj = Z[:j].T @ y
         true = np.linalg.norm(b - A @ xj) / bn
-        assert hist[j - 1] == pytest.approx(true, rel=(1e-8 if j <= 5 else 1e-2), abs=1e-14)
+        assert hist[j - 1] == pytest.approx(true, rel=(1e-8 if j <= 5 else (1e-4 if true > 1e-6 else 5e-2)), abs=1e-14)
 
 
 def test_P9_preconditioner_special_cases(oracle_mod):
