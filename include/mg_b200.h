@@ -1,0 +1,147 @@
+/* mg_b200.h — C ABI of the B200-native fGMRES + geometric-multigrid elliptic solver.
+ *
+ * Solves  lambda*u - div(c grad u) = f  (Eq. 3 with paper-xi = 1, Eq. 6) on a
+ * locally Cartesian, logically unstructured 2D mesh (Eq. 9) with Dirichlet and Neumann
+ * guard points (Eq. 11-16), by flexible GMRES preconditioned with one
+ * geometric-multigrid V-cycle using red-black-boundary Gauss-Seidel.
+ * The three-call shape create / update / solve is PAPER.md:133-139.  DESIGN.md section 3 lists the
+ * readings taken where the paper is silent (rule numbers M*, D*, T*, GS, C, V, K* are quoted below).
+ *
+ * Conventions
+ *  - "HOST" / "DEVICE" says where a pointer must live.  Device pointers are plain CUDA device memory of
+ *    the current device; `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - User vectors have length n (all mesh points, inner + guard) in the CALLER'S point order, fp64.
+ *    f[l] = rho_l on inner rows, phi_D,l on Dirichlet rows, Gamma_l on Neumann rows.
+ *  - "Level vectors" (test entry points) have length mg_level_n(level) in the level's canonical order:
+ *    ascending (J, I) of the level's own lattice indices (rule M7).  Levels are 0-based (0 = finest).
+ *  - Ownership: the handle owns all device memory it allocates (through the allocator installed with
+ *    mg_set_allocator, default cudaMalloc/cudaFree); callers own every array they pass in; host mesh
+ *    arrays may be freed after mg_setup returns.  One handle = one mesh = one stream at a time.
+ *  - Errors: every call returns 0 on success, a negative MG_E* code on failure (never throws, never
+ *    aborts); mg_solve may also return the positive MG_NOT_CONVERGED / MG_BREAKDOWN.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns MG_ECUDA.
+ */
+#ifndef MG_B200_H
+#define MG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_handle_s* mg_handle;
+#define MG_SETUP_HOST_ONLY 1
+
+enum {
+    MG_OK = 0,
+    MG_NOT_CONVERGED = 1, /* max_iters reached; x holds the last iterate                                  */
+    MG_BREAKDOWN = 2,     /* h_{j+1,j} = 0 with the residual still above rtol (rule K3)                  */
+    MG_EINVAL = -1,       /* null pointer, n <= 0, h <= 0, bad option, bad level                         */
+    MG_EMESH = -2,        /* duplicate (i,j); inner point lacking a neighbour; guard without an inner
+                             4-neighbour (rule M2); coarsest level too large for the dense solve */
+    MG_ECOEFF = -3,       /* reserved (coefficient check)                                   */
+    MG_ENOTREADY = -4,    /* solve / cycle before the first mg_update_coeffs                             */
+    MG_ECUDA = -5,        /* CUDA runtime error or no device                                             */
+    MG_ENOMEM = -6
+};
+
+/* Mesh: HOST pointers, length n, borrowed for the duration of mg_setup (Eq. 9). */
+typedef struct {
+    int64_t n;        /* number of mesh points, inner + guard                     */
+    const int32_t* i; /* lattice column index i_l (any int32, negative allowed)   */
+    const int32_t* j; /* lattice row index j_l                                    */
+    double h;         /* finest grid spacing                                      */
+} mg_mesh;
+
+/* Boundary classification: HOST pointer, length n. 0 = inner, 1 = Dirichlet guard (Eq. 11),
+ * 2 = Neumann guard (Eq. 16). */
+typedef struct {
+    const uint8_t* kind;
+} mg_bc;
+
+/* Solver parameters ("create ... based on the specified algorithm and solver parameters").
+ * Zero-initialise and override; 0 means "default" for every field. */
+typedef struct {
+    int levels;    /* N_sigma; 0 = auto: coarsen while the bounding lattice > 9x9 and |Inner| >= 16 (M8) */
+    int nu_pre;    /* nsmooth_pre, default 2; must be >= 1 (rule T2)                     */
+    int nu_post;   /* nsmooth_post, default 2                                             */
+    int restart_m; /* fGMRES restart length m, default 30, max 64                                        */
+    int max_iters; /* cap on preconditioner applications, default 200                                    */
+    int flags;     /* bit 0 (MG_SETUP_HOST_ONLY): build the host hierarchy only, touch no device; only the
+                      inspection calls mg_num_levels / mg_level_n / mg_level_info / mg_transfer_info work,
+                      every compute call returns MG_ECUDA.  Other bits must be 0.                        */
+} mg_options;
+
+/* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).
+ * alloc returns a device pointer or NULL; both may be NULL to restore cudaMalloc/cudaFree. */
+typedef void* (*mg_alloc_fn)(uint64_t bytes, void* stream);
+typedef void (*mg_free_fn)(void* ptr);
+int mg_set_allocator(mg_alloc_fn alloc_fn, mg_free_fn free_fn);
+
+/* create: builds the level hierarchy on the host (rules M1-M8: coarse point lists,
+ * guard classification, Neumann stencils, tile layout, transfer tables), uploads it and allocates all
+ * work space.  Synchronous.  Errors: MG_EINVAL, MG_EMESH, MG_ECUDA, MG_ENOMEM. */
+int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* stream, mg_handle* out);
+
+/* update: new coefficients lambda, c (= BASELINE "xi") on ALL n points, DEVICE
+ * pointers, user order.  Restricts them to all coarser levels (rule T4) and factorises the coarsest
+ * operator (rule C) on the device.  Asynchronous on `stream`. */
+int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream);
+
+/* solve: fGMRES(m) with one V-cycle as right preconditioner (rules K1-K5), stopping
+ * on ||A x - f|| / ||f|| < rtol (Eq. 23).  d_f, d_x0, d_x: DEVICE, length n, user order;
+ * d_x may alias d_x0.  iters (HOST, may be NULL) receives the number of preconditioner applications,
+ * final_relres (HOST, may be NULL) the recomputed true relative residual.  Returns after the stream
+ * has finished the solve.  Returns MG_OK, MG_NOT_CONVERGED, MG_BREAKDOWN or an error. */
+int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, double rtol, int* iters,
+             double* final_relres, void* stream);
+
+/* Same two calls with HOST buffers (pageable or pinned): the library stages them through device
+ * buffers it owns; copies run on `stream` (PAPER.md:217 describes exactly this transfer pattern). */
+int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c, void* stream);
+int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_x, double rtol, int* iters,
+                  double* final_relres, void* stream);
+
+int mg_destroy(mg_handle h);
+
+/* ---- inspection (HOST outputs; any output pointer may be NULL) -------------------------------- */
+int mg_num_levels(mg_handle h);
+int64_t mg_level_n(mg_handle h, int level);
+/* Per-level arrays in canonical order: lattice indices I, J; kind (0/1/2); colour (0 red, 1 black,
+ * 2 guard; rule M6); nbr [4n] = canonical indices of W, E, S, N (-1 absent, rule M5); for Neumann
+ * guards ns_tn [2n] = (2 n^R, 2 n^Z) of Eq. 13 and ns_fallback [n] (rule D3); slot [n] = position of
+ * the point in the device tile layout.  user2canon [n_0] (level 0 only) = canonical index of each
+ * user point. */
+int mg_level_info(mg_handle h, int level, int32_t* I, int32_t* J, uint8_t* kind, uint8_t* colour, int32_t* nbr,
+                  int8_t* ns_tn, uint8_t* ns_fallback, int32_t* slot, int64_t* user2canon);
+/* Transfer tables between `level` (fine) and level+1: fine9 [9*n_{level+1}] = canonical fine indices
+ * of the 3x3 neighbourhood of each coarse point (row-major dy, dx; -1 absent); parent [4*n_level] =
+ * canonical coarse indices of the bilinear parents (-1 absent / unused), ptype [n_level] = 0 coincident,
+ * 1 R-edge, 2 Z-edge, 3 centre (Fig. 3). */
+int mg_transfer_info(mg_handle h, int level, int32_t* fine9, int32_t* parent, uint8_t* ptype);
+/* Current coefficients of a level (DEVICE -> HOST copy, canonical order). */
+int mg_level_coeffs(mg_handle h, int level, double* h_lambda, double* h_c, void* stream);
+
+/* ---- single steps, for parity tests.  DEVICE level vectors in canonical order ------------------ */
+int mg_apply(mg_handle h, int level, const double* d_x, double* d_y, void* stream);            /* y = A x (D1-D3) */
+int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, void* stream); /* GS rbb        */
+int mg_restrict(mg_handle h, int level, const double* d_fine, double* d_coarse, void* stream);  /* rule T2        */
+int mg_prolong_correct(mg_handle h, int level, const double* d_coarse_e, double* d_x_fine, void* stream); /* T3   */
+int mg_coarse_solve(mg_handle h, const double* d_b, double* d_x, void* stream);                 /* rule C         */
+int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stream);
+
+/* Counters: kernels launched by this handle since creation (graph-launched kernels included). */
+int64_t mg_kernel_launches(mg_handle h);
+/* Wall-clock-free timing of the last mg_solve / mg_update_coeffs on the device (CUDA events on the
+ * launching stream), in milliseconds; negative if not available. */
+double mg_last_solve_ms(mg_handle h);
+double mg_last_update_ms(mg_handle h);
+
+const char* mg_strerror(int code);
+const char* mg_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG_B200_H */

@@ -1,0 +1,557 @@
+// C-ABI layer of libmg_b200 (include/mg_b200.h): handle, device hierarchy upload, V-cycle and fGMRES
+// orchestration (CUDA graph per Arnoldi iteration), inspection and single-step test entry points.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/mg_b200.h"
+#include "mg_device.h"
+
+using namespace mgb;
+
+namespace {
+
+thread_local std::string g_last_error;
+mg_alloc_fn g_alloc = nullptr;
+mg_free_fn g_free = nullptr;
+
+#define CU(call)                                                                             \
+    do {                                                                                     \
+        cudaError_t e__ = (call);                                                            \
+        if (e__ != cudaSuccess) {                                                            \
+            g_last_error = std::string(#call) + ": " + cudaGetErrorString(e__);              \
+            return MG_ECUDA;                                                                 \
+        }                                                                                    \
+    } while (0)
+
+struct LevelBuf {           // device arrays owned per level
+    uint16_t* code = nullptr;
+    int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
+    double *lam = nullptr, *c = nullptr, *x = nullptr, *b = nullptr, *d = nullptr;
+};
+
+}  // namespace
+
+struct mg_handle_s {
+    HostHierarchy hh;
+    int L = 0;
+    int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
+    int64_t n = 0;
+    std::vector<LevelDev> lev;
+    std::vector<LevelBuf> buf;
+    std::vector<void*> allocs;
+    int32_t* user2slot = nullptr;
+    // Krylov space (level-0 tile layout, stride = nslots of level 0)
+    double *V = nullptr, *Z = nullptr, *w = nullptr, *r = nullptr, *xs = nullptr, *bs = nullptr;
+    GmresState* st = nullptr;
+    double* partial = nullptr;
+    int* h_hdr = nullptr;                 // pinned copy of the first 8 ints of the state
+    GmresState* h_state = nullptr;        // pinned full copy (read at the end of a solve)
+    // coarsest level
+    int nL = 0;
+    int32_t *cslot = nullptr, *slot2row = nullptr;
+    double *cwork = nullptr, *Ainv = nullptr;
+    // host-buffer staging
+    double* stage[3] = {nullptr, nullptr, nullptr};
+    bool have_coeffs = false;
+    bool host_only = false;
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t iter_graph = nullptr;
+    int64_t iter_graph_kernels = 0;
+    int64_t launches = 0;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool solve_timed = false, update_timed = false;
+};
+
+namespace {
+
+int dev_alloc(mg_handle h, void** p, size_t bytes, cudaStream_t s) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 8;
+    if (g_alloc) {
+        *p = g_alloc((uint64_t)bytes, (void*)s);
+        if (!*p) { g_last_error = "allocator returned NULL"; return MG_ENOMEM; }
+    } else {
+        cudaError_t e = cudaMalloc(p, bytes);
+        if (e != cudaSuccess) { g_last_error = std::string("cudaMalloc: ") + cudaGetErrorString(e); cudaGetLastError(); return MG_ENOMEM; }
+    }
+    h->allocs.push_back(*p);
+    CU(cudaMemsetAsync(*p, 0, bytes, s));
+    return MG_OK;
+}
+
+template <class T>
+int upload(mg_handle h, T** dst, const std::vector<T>& src, cudaStream_t s) {
+    int rc = dev_alloc(h, (void**)dst, src.size() * sizeof(T), s);
+    if (rc) return rc;
+    if (!src.empty()) CU(cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s));
+    return MG_OK;
+}
+
+Launch LZ(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }
+
+// mg_cycle of PAPER.md:171-195 with gamma = 1, enqueued on L.stream.
+void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b) {
+    const LevelDev& lv = h->lev[s];
+    if (s == h->L - 1) {                                              // P:173-177 direct solve
+        launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, b, x);
+        return;
+    }
+    for (int k = 0; k < h->nu_pre; k++) launch_gs_sweep(L, lv, x, b);
+    launch_apply(L, lv, x, b, vec(h->buf[s].d), 2);                             // P:183  d = A x - b
+    launch_restrict(L, lv, h->lev[s + 1], h->buf[s].d, h->buf[s + 1].b);
+    if (s + 1 < h->L - 1) launch_zero(L, vec(h->buf[s + 1].x), h->lev[s + 1].nslots);   // P:186  e = 0
+    enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b));
+    launch_prolong_correct(L, lv, h->lev[s + 1], h->buf[s + 1].x, h->buf[s].d, x);
+    for (int k = 0; k < h->nu_post; k++) launch_gs_sweep(L, lv, x, b);
+}
+
+// One Arnoldi step (rule K2): z_j = MG(v_j), w = A z_j, CGS2, Givens + stop test, v_{j+1}.
+void enqueue_iteration(mg_handle h, const Launch& L) {
+    const int64_t ns = h->lev[0].nslots;
+    VecRef zj{h->Z, ns, &h->st->j, 0}, vj{h->V, ns, &h->st->j, 0};
+    launch_zero(L, zj, ns);
+    enqueue_cycle(h, L, 0, zj, vj);
+    launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
+    launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
+    launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 0);
+    launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
+    launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 1);
+    launch_givens(L, h->st);
+    launch_next_v(L, h->w, h->V, ns, ns, h->st);
+}
+
+int build_iter_graph(mg_handle h) {
+    if (h->iter_graph) return MG_OK;
+    cudaGraph_t g = nullptr;
+    const int64_t before = h->launches;
+    CU(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    enqueue_iteration(h, LZ(h, h->cap_stream));
+    CU(cudaStreamEndCapture(h->cap_stream, &g));
+    h->iter_graph_kernels = h->launches - before;
+    h->launches = before;
+    CU(cudaGraphInstantiate(&h->iter_graph, g, 0));
+    CU(cudaGraphDestroy(g));
+    return MG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mg_last_error(void) { return g_last_error.c_str(); }
+
+const char* mg_strerror(int code) {
+    switch (code) {
+        case MG_OK: return "ok";
+        case MG_NOT_CONVERGED: return "not converged (max_iters reached)";
+        case MG_BREAKDOWN: return "breakdown (h_{j+1,j} = 0)";
+        case MG_EINVAL: return "invalid argument";
+        case MG_EMESH: return "invalid mesh";
+        case MG_ECOEFF: return "invalid coefficients";
+        case MG_ENOTREADY: return "mg_update_coeffs has not been called";
+        case MG_ECUDA: return "CUDA error";
+        case MG_ENOMEM: return "out of device memory";
+        default: return "unknown error";
+    }
+}
+
+int mg_set_allocator(mg_alloc_fn a, mg_free_fn f) {
+    if ((a == nullptr) != (f == nullptr)) return MG_EINVAL;
+    g_alloc = a; g_free = f;
+    return MG_OK;
+}
+
+int mg_destroy(mg_handle h) {
+    if (!h) return MG_EINVAL;
+    if (h->host_only) { delete h; return MG_OK; }
+    cudaDeviceSynchronize();
+    if (h->iter_graph) cudaGraphExecDestroy(h->iter_graph);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+    if (h->h_hdr) cudaFreeHost(h->h_hdr);
+    if (h->h_state) cudaFreeHost(h->h_state);
+    for (void* p : h->allocs) { if (g_free) g_free(p); else cudaFree(p); }
+    delete h;
+    return MG_OK;
+}
+
+int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* stream, mg_handle* out) {
+    if (!out) return MG_EINVAL;
+    *out = nullptr;
+    if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
+    mg_options o{};
+    if (opt) o = *opt;
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || (o.flags & ~1) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    const bool host_only = (o.flags & 1) != 0;
+    int ndev = 0;
+    if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
+    mg_handle h = new (std::nothrow) mg_handle_s();
+    if (!h) return MG_ENOMEM;
+    h->nu_pre = o.nu_pre ? o.nu_pre : 2;
+    h->nu_post = o.nu_post ? o.nu_post : 2;
+    h->m = o.restart_m ? o.restart_m : 30;
+    h->max_iters = o.max_iters ? o.max_iters : 200;
+    h->n = mesh->n;
+    int rc = build_hierarchy(mesh->n, mesh->i, mesh->j, bc->kind, mesh->h, o.levels, h->hh);
+    if (rc) { g_last_error = h->hh.err; delete h; return rc; }
+    h->L = (int)h->hh.lev.size();
+    h->nL = (int)h->hh.lev.back().n;
+    if (h->nL > 1024) { g_last_error = "coarsest level has more than 1024 points; use more levels"; delete h; return MG_EMESH; }
+    if (host_only) { h->host_only = true; *out = h; return MG_OK; }
+    cudaStream_t s = (cudaStream_t)stream;
+    auto fail = [&](int code) { mg_destroy(h); return code; };
+#define TRY(x) do { int rc__ = (x); if (rc__) return fail(rc__); } while (0)
+#define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_error = std::string(#call) + ": " + cudaGetErrorString(e__); return fail(MG_ECUDA); } } while (0)
+    CUF(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+    for (auto& e : h->ev) CUF(cudaEventCreate(&e));
+    CUF(cudaMallocHost((void**)&h->h_hdr, 64));
+    CUF(cudaMallocHost((void**)&h->h_state, sizeof(GmresState)));
+    h->lev.resize(h->L); h->buf.resize(h->L);
+    for (int l = 0; l < h->L; l++) {
+        HostLevel& hl = h->hh.lev[l];
+        LevelBuf& b = h->buf[l];
+        TRY(upload(h, &b.code, hl.code, s));
+        TRY(upload(h, &b.tnb, hl.tnb, s));
+        TRY(upload(h, &b.ctab, hl.ctab, s));
+        TRY(upload(h, &b.ptab, hl.ptab, s));
+        std::vector<int32_t> tij(2 * (size_t)hl.ntiles);
+        for (int t = 0; t < hl.ntiles; t++) { tij[2 * t] = hl.tI[t]; tij[2 * t + 1] = hl.tJ[t]; }
+        TRY(upload(h, &b.tij, tij, s));
+        TRY(upload(h, &b.canon2slot, hl.canon2slot, s));
+        const size_t vb = (size_t)hl.nslots() * sizeof(double);
+        TRY(dev_alloc(h, (void**)&b.lam, vb, s));
+        TRY(dev_alloc(h, (void**)&b.c, vb, s));
+        TRY(dev_alloc(h, (void**)&b.x, vb, s));
+        TRY(dev_alloc(h, (void**)&b.b, vb, s));
+        TRY(dev_alloc(h, (void**)&b.d, vb, s));
+        LevelDev& d = h->lev[l];
+        d.ntiles = hl.ntiles;
+        d.ntiles_fine = l > 0 ? h->hh.lev[l - 1].ntiles : 0;
+        d.ntiles_coarse = l + 1 < h->L ? h->hh.lev[l + 1].ntiles : 0;
+        d.nslots = hl.nslots();
+        d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
+        d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c;
+    }
+    TRY(upload(h, &h->user2slot, h->hh.user2slot, s));
+    const size_t v0 = (size_t)h->lev[0].nslots * sizeof(double);
+    TRY(dev_alloc(h, (void**)&h->V, v0 * (h->m + 1), s));
+    TRY(dev_alloc(h, (void**)&h->Z, v0 * (h->m + 1), s));
+    TRY(dev_alloc(h, (void**)&h->w, v0, s));
+    TRY(dev_alloc(h, (void**)&h->r, v0, s));
+    TRY(dev_alloc(h, (void**)&h->xs, v0, s));
+    TRY(dev_alloc(h, (void**)&h->bs, v0, s));
+    TRY(dev_alloc(h, (void**)&h->st, sizeof(GmresState), s));
+    TRY(dev_alloc(h, (void**)&h->partial, sizeof(double) * RED_BLOCKS * (MAX_M + 2), s));
+    {   // coarsest level: canonical row -> slot and its inverse
+        HostLevel& cl = h->hh.lev.back();
+        std::vector<int32_t> s2r((size_t)cl.nslots(), 0);
+        for (int r = 0; r < h->nL; r++) s2r[cl.canon2slot[r]] = r;
+        h->cslot = h->buf[h->L - 1].canon2slot;
+        TRY(upload(h, &h->slot2row, s2r, s));
+        TRY(dev_alloc(h, (void**)&h->cwork, sizeof(double) * 2 * (size_t)h->nL * h->nL, s));
+        TRY(dev_alloc(h, (void**)&h->Ainv, sizeof(double) * (size_t)h->nL * h->nL, s));
+    }
+    CUF(cudaStreamSynchronize(s));
+#undef TRY
+#undef CUF
+    *out = h;
+    return MG_OK;
+}
+
+}  // extern "C"
+
+// ============================================================================ update / solve
+extern "C" {
+
+int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream) {
+    if (!h || !d_lambda || !d_c) return MG_EINVAL;
+    if (h->host_only) return MG_ECUDA;
+    cudaStream_t s = (cudaStream_t)stream;
+    Launch L = LZ(h, s);
+    CU(cudaEventRecord(h->ev[2], s));
+    launch_gather(L, d_lambda, h->user2slot, h->buf[0].lam, h->n);
+    launch_gather(L, d_c, h->user2slot, h->buf[0].c, h->n);
+    for (int l = 0; l + 1 < h->L; l++) launch_restrict_coeff(L, h->lev[l], h->lev[l + 1]);     // rule T4
+    launch_coarse_factor(L, h->lev[h->L - 1], h->cslot, h->slot2row, h->nL, h->cwork, h->Ainv);   // rule C
+    CU(cudaEventRecord(h->ev[3], s));
+    CU(cudaGetLastError());
+    h->have_coeffs = true;
+    h->update_timed = true;
+    return MG_OK;
+}
+
+int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, double rtol, int* iters,
+             double* final_relres, void* stream) {
+    if (!h || !d_f || !d_x0 || !d_x || !(rtol > 0.0)) return MG_EINVAL;
+    if (!h->have_coeffs) return MG_ENOTREADY;
+    cudaStream_t s = (cudaStream_t)stream;
+    Launch L = LZ(h, s);
+    int rc = build_iter_graph(h);
+    if (rc) return rc;
+    const int64_t ns = h->lev[0].nslots;
+    CU(cudaEventRecord(h->ev[0], s));
+    launch_init_state(L, h->st, h->m, h->max_iters, rtol);
+    launch_gather(L, d_f, h->user2slot, h->bs, h->n);                 // B1: user order -> tile layout
+    launch_gather(L, d_x0, h->user2slot, h->xs, h->n);
+    launch_norm2(L, h->bs, ns, h->st, h->partial, 0);                 // K1: bn = ||b||
+    int status = 0;
+    for (int cycle = 0; cycle < 1000000; cycle++) {
+        launch_apply(L, h->lev[0], vec(h->xs), vec(h->bs), vec(h->r), 1);      // r = b - A x (rule D4)
+        launch_norm2(L, h->r, ns, h->st, h->partial, 1);
+        launch_start_cycle(L, h->st, h->r, h->V, ns);
+        CU(cudaMemcpyAsync(h->h_hdr, h->st, 32, cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        status = h->h_hdr[2];
+        if (h->h_hdr[3]) break;                                       // cycle_end set by start: finished
+        for (int it = 0; it < h->m; it++) {
+            CU(cudaGraphLaunch(h->iter_graph, s));
+            h->launches += h->iter_graph_kernels;
+            CU(cudaMemcpyAsync(h->h_hdr, h->st, 32, cudaMemcpyDeviceToHost, s));
+            CU(cudaStreamSynchronize(s));
+            if (h->h_hdr[3]) break;
+        }
+        launch_update_x(L, h->xs, h->Z, ns, ns, h->st);               // K4
+    }
+    if (status == 4) launch_zero(L, vec(h->xs), ns);                  // K1: zero right-hand side
+    launch_scatter(L, h->xs, h->user2slot, d_x, h->n);                // B1: tile layout -> user order
+    CU(cudaEventRecord(h->ev[1], s));
+    CU(cudaMemcpyAsync(h->h_state, h->st, sizeof(GmresState), cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    CU(cudaGetLastError());
+    h->solve_timed = true;
+    if (iters) *iters = h->h_state->iters;
+    if (final_relres) *final_relres = h->h_state->relres;
+    if (status == 1 || status == 4) return MG_OK;
+    if (status == 3) return MG_BREAKDOWN;
+    return MG_NOT_CONVERGED;
+}
+
+static int ensure_stage(mg_handle h, cudaStream_t s) {
+    for (int k = 0; k < 3; k++)
+        if (!h->stage[k]) { int rc = dev_alloc(h, (void**)&h->stage[k], sizeof(double) * (size_t)h->n, s); if (rc) return rc; }
+    return MG_OK;
+}
+
+int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c, void* stream) {
+    if (!h || !h_lambda || !h_c) return MG_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_stage(h, s);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    return mg_update_coeffs(h, h->stage[0], h->stage[1], stream);
+}
+
+int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_x, double rtol, int* iters,
+                  double* final_relres, void* stream) {
+    if (!h || !h_f || !h_x0 || !h_x) return MG_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_stage(h, s);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h->stage[0], h_f, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[1], h_x0, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    rc = mg_solve(h, h->stage[0], h->stage[1], h->stage[2], rtol, iters, final_relres, stream);
+    if (rc < 0) return rc;
+    CU(cudaMemcpyAsync(h_x, h->stage[2], sizeof(double) * h->n, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return rc;
+}
+
+int64_t mg_kernel_launches(mg_handle h) { return h ? h->launches : 0; }
+
+double mg_last_solve_ms(mg_handle h) {
+    float ms = -1.f;
+    if (!h || !h->solve_timed || cudaEventElapsedTime(&ms, h->ev[0], h->ev[1]) != cudaSuccess) { cudaGetLastError(); return -1.0; }
+    return ms;
+}
+double mg_last_update_ms(mg_handle h) {
+    float ms = -1.f;
+    if (!h || !h->update_timed || cudaEventSynchronize(h->ev[3]) != cudaSuccess || cudaEventElapsedTime(&ms, h->ev[2], h->ev[3]) != cudaSuccess) { cudaGetLastError(); return -1.0; }
+    return ms;
+}
+
+}  // extern "C"
+
+// ============================================================================ inspection
+extern "C" {
+
+int mg_num_levels(mg_handle h) { return h ? h->L : MG_EINVAL; }
+int64_t mg_level_n(mg_handle h, int level) { return (h && level >= 0 && level < h->L) ? h->hh.lev[level].n : (int64_t)MG_EINVAL; }
+
+int mg_level_info(mg_handle h, int level, int32_t* I, int32_t* J, uint8_t* kind, uint8_t* colour, int32_t* nbr,
+                  int8_t* ns_tn, uint8_t* ns_fallback, int32_t* slot, int64_t* user2canon) {
+    if (!h || level < 0 || level >= h->L) return MG_EINVAL;
+    const HostLevel& lv = h->hh.lev[level];
+    std::vector<int32_t> s2c;
+    if (nbr || user2canon) {
+        s2c.assign((size_t)lv.nslots(), -1);
+        for (int64_t k = 0; k < lv.n; k++) s2c[lv.canon2slot[k]] = (int32_t)k;
+    }
+    const int dI[4] = {-1, 1, 0, 0}, dJ[4] = {0, 0, -1, 1};
+    for (int64_t k = 0; k < lv.n; k++) {
+        const int64_t s = lv.canon2slot[k];
+        const int t = (int)(s / TS), ly = (int)(s % TS) / TX, lx = (int)(s % TS) % TX;
+        const int64_t pi = (int64_t)lv.tI[t] * TX + lx, pj = (int64_t)lv.tJ[t] * TY + ly;
+        const uint16_t c = lv.code[s];
+        const int kd = code_kind(c);
+        if (I) I[k] = (int32_t)pi;
+        if (J) J[k] = (int32_t)pj;
+        if (kind) kind[k] = (uint8_t)(kd - 1);
+        if (colour) colour[k] = (uint8_t)(kd == C_INNER ? ((pi + pj) & 1) : 2);          // rule M6
+        if (nbr)
+            for (int d = 0; d < 4; d++) {
+                const int64_t q = lv.slot_of(pi + dI[d], pj + dJ[d]);
+                nbr[4 * k + d] = q < 0 ? -1 : s2c[q];
+            }
+        if (ns_tn) {
+            ns_tn[2 * k] = (int8_t)(kd == C_NEU ? ((c >> 2) & 7) - 2 : 0);
+            ns_tn[2 * k + 1] = (int8_t)(kd == C_NEU ? ((c >> 5) & 7) - 2 : 0);
+        }
+        if (ns_fallback) ns_fallback[k] = (uint8_t)(kd == C_NEU ? (c >> 8) & 1 : 0);
+        if (slot) slot[k] = (int32_t)s;
+    }
+    if (user2canon) {
+        if (level != 0) return MG_EINVAL;
+        for (int64_t p = 0; p < h->n; p++) user2canon[p] = s2c[h->hh.user2slot[p]];
+    }
+    return MG_OK;
+}
+
+int mg_transfer_info(mg_handle h, int level, int32_t* fine9, int32_t* parent, uint8_t* ptype) {
+    if (!h || level < 0 || level + 1 >= h->L) return MG_EINVAL;
+    const HostLevel &f = h->hh.lev[level], &c = h->hh.lev[level + 1];
+    auto s2c_of = [](const HostLevel& lv) {
+        std::vector<int32_t> m((size_t)lv.nslots(), -1);
+        for (int64_t k = 0; k < lv.n; k++) m[lv.canon2slot[k]] = (int32_t)k;
+        return m;
+    };
+    auto coords = [](const HostLevel& lv, int64_t s, int64_t& pi, int64_t& pj) {
+        const int t = (int)(s / TS);
+        pi = (int64_t)lv.tI[t] * TX + (s % TS) % TX; pj = (int64_t)lv.tJ[t] * TY + (s % TS) / TX;
+    };
+    if (fine9) {
+        const std::vector<int32_t> fm = s2c_of(f);
+        for (int64_t q = 0; q < c.n; q++) {
+            int64_t ci, cj; coords(c, c.canon2slot[q], ci, cj);
+            for (int dy = -1; dy <= 1; dy++)
+                for (int dx = -1; dx <= 1; dx++) {
+                    const int64_t s = f.slot_of(2 * ci + dx, 2 * cj + dy);
+                    fine9[9 * q + 3 * (dy + 1) + dx + 1] = s < 0 ? -1 : fm[s];
+                }
+        }
+    }
+    if (parent || ptype) {
+        const std::vector<int32_t> cm = s2c_of(c);
+        for (int64_t l = 0; l < f.n; l++) {
+            int64_t fi, fj; coords(f, f.canon2slot[l], fi, fj);
+            const int ox = (int)(fi & 1), oy = (int)(fj & 1);
+            const int64_t ci = floordiv(fi, 2), cj = floordiv(fj, 2);
+            if (ptype) ptype[l] = (uint8_t)(ox + 2 * oy);
+            if (parent) {
+                int cnt = 0;
+                for (int b = 0; b <= oy; b++)
+                    for (int a = 0; a <= ox; a++) {
+                        const int64_t s = c.slot_of(ci + a, cj + b);
+                        parent[4 * l + cnt++] = s < 0 ? -1 : cm[s];
+                    }
+                for (; cnt < 4; cnt++) parent[4 * l + cnt] = -1;
+            }
+        }
+    }
+    return MG_OK;
+}
+
+int mg_level_coeffs(mg_handle h, int level, double* h_lambda, double* h_c, void* stream) {
+    if (!h || level < 0 || level >= h->L) return MG_EINVAL;
+    if (!h->have_coeffs) return MG_ENOTREADY;
+    cudaStream_t s = (cudaStream_t)stream;
+    const HostLevel& lv = h->hh.lev[level];
+    std::vector<double> tmp((size_t)lv.nslots());
+    for (int k = 0; k < 2; k++) {
+        double* out = k ? h_c : h_lambda;
+        if (!out) continue;
+        CU(cudaMemcpyAsync(tmp.data(), k ? h->buf[level].c : h->buf[level].lam, tmp.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        for (int64_t q = 0; q < lv.n; q++) out[q] = tmp[lv.canon2slot[q]];
+    }
+    return MG_OK;
+}
+
+// ============================================================================ single steps (parity tests)
+#define CHECK_LEVEL(cond) do { if (!h || !(cond)) return MG_EINVAL; if (h->host_only) return MG_ECUDA; if (!h->have_coeffs) return MG_ENOTREADY; } while (0)
+
+int mg_apply(mg_handle h, int level, const double* d_x, double* d_y, void* stream) {
+    CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_y);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    const int64_t n = h->hh.lev[level].n;
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
+    launch_apply(L, h->lev[level], vec(h->buf[level].x), vec(nullptr), vec(h->buf[level].d), 0);
+    launch_scatter(L, h->buf[level].d, h->buf[level].canon2slot, d_y, n);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, void* stream) {
+    CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_b && sweeps >= 0);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    const int64_t n = h->hh.lev[level].n;
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
+    for (int k = 0; k < sweeps; k++) launch_gs_sweep(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].b));
+    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int mg_restrict(mg_handle h, int level, const double* d_fine, double* d_coarse, void* stream) {
+    CHECK_LEVEL(level >= 0 && level + 1 < h->L && d_fine && d_coarse);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    launch_gather(L, d_fine, h->buf[level].canon2slot, h->buf[level].d, h->hh.lev[level].n);
+    launch_restrict(L, h->lev[level], h->lev[level + 1], h->buf[level].d, h->buf[level + 1].b);
+    launch_scatter(L, h->buf[level + 1].b, h->buf[level + 1].canon2slot, d_coarse, h->hh.lev[level + 1].n);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int mg_prolong_correct(mg_handle h, int level, const double* d_coarse_e, double* d_x_fine, void* stream) {
+    CHECK_LEVEL(level >= 0 && level + 1 < h->L && d_coarse_e && d_x_fine);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    launch_gather(L, d_coarse_e, h->buf[level + 1].canon2slot, h->buf[level + 1].x, h->hh.lev[level + 1].n);
+    launch_gather(L, d_x_fine, h->buf[level].canon2slot, h->buf[level].x, h->hh.lev[level].n);
+    launch_prolong_correct(L, h->lev[level], h->lev[level + 1], h->buf[level + 1].x, h->buf[level].d, vec(h->buf[level].x));
+    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x_fine, h->hh.lev[level].n);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int mg_coarse_solve(mg_handle h, const double* d_b, double* d_x, void* stream) {
+    CHECK_LEVEL(d_b && d_x);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    const int l = h->L - 1;
+    launch_gather(L, d_b, h->buf[l].canon2slot, h->buf[l].b, h->nL);
+    launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, vec(h->buf[l].b), vec(h->buf[l].x));
+    launch_scatter(L, h->buf[l].x, h->buf[l].canon2slot, d_x, h->nL);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stream) {
+    CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_b);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    const int64_t n = h->hh.lev[level].n;
+    // level buffers x/b of `level` are free here: the recursion only uses those of the coarser levels
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
+    enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].b));
+    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,97 @@
+// Device-side structures and kernel launch wrappers of libmg_b200 (internal).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "mg_common.h"
+
+namespace mgb {
+
+constexpr int MAX_M = 64;          // largest fGMRES restart length
+constexpr int RED_BLOCKS = 592;    // 4 x 148 SMs: blocks of the grid-wide reductions
+constexpr int RED_THREADS = 256;
+
+// One multigrid level on the device (all pointers device memory; vectors have nslots entries).
+struct LevelDev {
+    int32_t ntiles;
+    int32_t ntiles_fine;     // null-tile id of the next finer level (for ctab), 0 on level 0
+    int32_t ntiles_coarse;   // null-tile id of the next coarser level (for ptab)
+    int64_t nslots;
+    double h, kappa;         // kappa = 1 / (2 h^2), rule D1
+    const uint16_t* code;
+    const int32_t* tnb;      // 9 per tile
+    const int32_t* ctab;     // 9 per tile (this level as the coarse side)
+    const int32_t* ptab;     // 4 per tile (this level as the fine side)
+    const int32_t* tij;      // 2 per tile: tile coordinates (TI, TJ)
+    double* lam;
+    double* c;
+};
+
+// A vector that may be one column of a Krylov basis selected on the device:
+// address = base + (idx ? *idx + off : 0) * stride.
+struct VecRef {
+    double* base;
+    int64_t stride;
+    const int* idx;
+    int off;
+};
+__host__ __device__ inline VecRef vec(double* p) { return VecRef{p, 0, nullptr, 0}; }
+#ifdef __CUDACC__
+__device__ __forceinline__ double* resolve(const VecRef& v) {
+    return v.base + (v.idx ? (int64_t)(*v.idx + v.off) * v.stride : 0);
+}
+#endif
+
+// fGMRES state, resident on the device (rules K1-K5).  Givens rotations, the least-squares
+// right-hand side and the stop test live here so that no iteration needs the host.
+struct GmresState {
+    int j;            // current column (0-based) of the running restart cycle
+    int iters;        // preconditioner applications so far
+    int status;       // 0 running, 1 converged, 2 max_iters, 3 breakdown
+    int cycle_end;    // 1: the running cycle ended (converged, j == m, max_iters or breakdown)
+    int m, max_iters;
+    int ticket;       // last-block-done counter of the grid reductions
+    int pad;
+    double rtol, bn, beta, relres, hn, inv_hn;
+    double red[MAX_M + 2];          // results of the last multi-reduction
+    double hcol[MAX_M + 2];         // Hessenberg column being built (h_0j .. h_j+1,j)
+    double H[(MAX_M + 1) * MAX_M];  // rotated Hessenberg (upper triangular R), row-major, ld = MAX_M
+    double g[MAX_M + 1], cs[MAX_M], sn[MAX_M], y[MAX_M];
+    double hist[512];               // |g_{k+1}| / bn per iteration
+};
+
+struct Launch {
+    cudaStream_t stream;
+    int64_t* counter;   // host counter of kernel launches (may be null)
+};
+
+// ---- tile kernels (mg_kernels.cu) ----
+// mode 0: y = A x      1: y = b - A x      2: y = A x - b
+void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRef y, int mode);
+void launch_gs_sweep(const Launch& L, const LevelDev& lv, VecRef x, VecRef b);
+void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse);
+void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
+                            double* e_fine_tmp, VecRef x_fine);
+void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse);
+void launch_zero(const Launch& L, VecRef x, int64_t n);
+void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n);   // dst[slot[k]] = src[k]
+void launch_scatter(const Launch& L, const double* src_tiled, const int32_t* slot, double* dst, int64_t n);  // dst[k] = src[slot[k]]
+
+// ---- coarsest level (mg_coarse.cu) ----
+void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
+                          double* work /* n x 2n */, double* Ainv /* n x n */);
+void launch_coarse_solve(const Launch& L, const double* Ainv, const int32_t* cslot, int n, VecRef b_tiled, VecRef x_tiled);
+
+// ---- fGMRES vector kernels (mg_krylov.cu) ----
+void launch_norm2(const Launch& L, const double* v, int64_t n, GmresState* st, double* partial, int which);  // which: 0 -> bn, 1 -> beta
+void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double* V0, int64_t n);
+void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial);
+void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass);
+void launch_givens(const Launch& L, GmresState* st);
+void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
+void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st);
+void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol);
+void launch_final_check(const Launch& L, GmresState* st);
+
+}  // namespace mgb

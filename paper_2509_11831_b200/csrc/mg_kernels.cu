@@ -1,0 +1,310 @@
+// Tile kernels of the multigrid hierarchy (sm_100a): operator apply / residual (S1), red-black-boundary
+// Gauss-Seidel (S2), full-weighting restriction (S3), bilinear prolongation + set_bnds_hom + correction
+// (S4), coefficient restriction (U1).  One CTA per active tile; halo values come from the neighbour
+// tiles through the per-tile 3x3 table (missing tiles map to the all-absent null tile).
+#include "mg_device.h"
+
+#include <algorithm>
+
+namespace mgb {
+
+namespace {
+
+constexpr int NT = 256;                 // threads per CTA: 32 x 8, two rows per thread
+constexpr int ROWS_PER_PASS = NT / TX;  // 8
+
+// slot of the point at local offset (lx, ly) in [-TX, 2TX) x [-TY, 2TY) relative to tile whose 3x3
+// neighbour table is tn[9]
+__device__ __forceinline__ int64_t nslot(const int* tn, int lx, int ly) {
+    const int ox = (lx < 0) ? -1 : (lx >= TX ? 1 : 0);
+    const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
+    return (int64_t)tn[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + (lx - ox * TX);
+}
+
+// Rule D3 / Eq. 14-16: upstream value of a Neumann guard. Returns sum over non-self nodes of w*x,
+// the weight on the point itself and the distance delta = h |n| (h for the fallback).
+__device__ __forceinline__ void neumann_row(uint16_t code, const int* tn, int lx, int ly, const double* __restrict__ x,
+                                            double h, double& sum, double& wself, double& delta) {
+    const int tnR = ((code >> 2) & 7) - 2, tnZ = ((code >> 5) & 7) - 2;
+    sum = 0.0; wself = 0.0;
+    if (code & (1 << 8)) {                                  // fallback: mean of the inner 4-neighbours
+        const int mask = (code >> 9) & 15;
+        if (mask & 1) sum += x[nslot(tn, lx - 1, ly)];
+        if (mask & 2) sum += x[nslot(tn, lx + 1, ly)];
+        if (mask & 4) sum += x[nslot(tn, lx, ly - 1)];
+        if (mask & 8) sum += x[nslot(tn, lx, ly + 1)];
+        sum = sum / (double)__popc(mask);
+        delta = h;
+        return;
+    }
+    int ox[2], oy[2], nx, ny; double wx, wy;
+    if (tnR & 1) { nx = 2; ox[0] = 0; ox[1] = tnR; wx = 0.5; } else { nx = 1; ox[0] = tnR / 2; ox[1] = 0; wx = 1.0; }
+    if (tnZ & 1) { ny = 2; oy[0] = 0; oy[1] = tnZ; wy = 0.5; } else { ny = 1; oy[0] = tnZ / 2; oy[1] = 0; wy = 1.0; }
+    const double w = wx * wy;
+    for (int b = 0; b < ny; b++)
+        for (int a = 0; a < nx; a++) {
+            if (ox[a] == 0 && oy[b] == 0) { wself += w; continue; }
+            sum += w * x[nslot(tn, lx + ox[a], ly + oy[b])];
+        }
+    delta = h * sqrt(0.25 * (double)(tnR * tnR + tnZ * tnZ));
+}
+
+// ---------------------------------------------------------------------------------- S1 apply / residual
+template <int MODE>
+__global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr) {
+    __shared__ int tn[9];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
+    __syncthreads();
+    const double* __restrict__ x = resolve(xr);
+    const double* __restrict__ b = (MODE != 0) ? resolve(br) : nullptr;
+    double* __restrict__ y = resolve(yr);
+    const int lx = threadIdx.x % TX;
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        const uint16_t code = lv.code[s];
+        const int kind = code & 3;
+        double ax = 0.0;
+        if (kind == C_INNER) {                                          // Eq. 10 with 1/h^2 (rule D1)
+            const int64_t sW = nslot(tn, lx - 1, ly), sE = nslot(tn, lx + 1, ly), sS = nslot(tn, lx, ly - 1), sN = nslot(tn, lx, ly + 1);
+            const double cl = lv.c[s];
+            const double aW = lv.kappa * (cl + lv.c[sW]), aE = lv.kappa * (cl + lv.c[sE]);
+            const double aS = lv.kappa * (cl + lv.c[sS]), aN = lv.kappa * (cl + lv.c[sN]);
+            const double all = lv.lam[s] + aW + aE + aS + aN;
+            ax = all * x[s] - aW * x[sW] - aE * x[sE] - aS * x[sS] - aN * x[sN];
+        } else if (kind == C_DIR) {                                     // Eq. 11
+            ax = x[s];
+        } else if (kind == C_NEU) {                                     // Eq. 16
+            double sum, wself, delta;
+            neumann_row(code, tn, lx, ly, x, lv.h, sum, wself, delta);
+            const double xl = x[s];
+            ax = (sum + wself * xl - xl) / delta;
+        }
+        if (kind == C_ABSENT) y[s] = 0.0;
+        else if (MODE == 0) y[s] = ax;
+        else if (MODE == 1) y[s] = b[s] - ax;
+        else y[s] = ax - b[s];
+    }
+}
+
+// ---------------------------------------------------------------------------------- S2 smoother
+// One group of gauss_seidel_rbb: GROUP 0 red inner ((I+J) even), 1 black inner, 2 guards.
+template <int GROUP>
+__global__ void __launch_bounds__(NT) k_gs_group(LevelDev lv, VecRef xr, VecRef br) {
+    __shared__ int tn[9];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
+    __syncthreads();
+    double* __restrict__ x = resolve(xr);
+    const double* __restrict__ b = resolve(br);
+    const int lx = threadIdx.x % TX;
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        const uint16_t code = lv.code[s];
+        const int kind = code & 3;
+        if (GROUP < 2) {
+            if (kind != C_INNER || ((lx + ly) & 1) != GROUP) continue;
+            const int64_t sW = nslot(tn, lx - 1, ly), sE = nslot(tn, lx + 1, ly), sS = nslot(tn, lx, ly - 1), sN = nslot(tn, lx, ly + 1);
+            const double cl = lv.c[s];
+            const double aW = lv.kappa * (cl + lv.c[sW]), aE = lv.kappa * (cl + lv.c[sE]);
+            const double aS = lv.kappa * (cl + lv.c[sS]), aN = lv.kappa * (cl + lv.c[sN]);
+            const double all = lv.lam[s] + aW + aE + aS + aN;
+            x[s] = (b[s] + aW * x[sW] + aE * x[sE] + aS * x[sS] + aN * x[sN]) / all;
+        } else {
+            if (kind == C_DIR) x[s] = b[s];
+            else if (kind == C_NEU) {
+                double sum, wself, delta;
+                neumann_row(code, tn, lx, ly, x, lv.h, sum, wself, delta);
+                x[s] = (sum - delta * b[s]) / (1.0 - wself);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------- S3 restriction (rule T2)
+// One CTA per COARSE tile. Fine point (2 lxc + dx, 2 lyc + dy) lives in one of the 3x3 fine tiles of ctab.
+__device__ __forceinline__ int64_t fine_slot(const int* ct, int fx, int fy) {   // fx in [-1, 2TX), fy in [-1, 2TY)
+    const int cx = (fx < 0) ? 0 : (fx < TX ? 1 : 2);
+    const int cy = (fy < 0) ? 0 : (fy < TY ? 1 : 2);
+    return (int64_t)ct[cy * 3 + cx] * TS + (fy - (cy - 1) * TY) * TX + (fx - (cx - 1) * TX);
+}
+
+__global__ void __launch_bounds__(NT) k_restrict(LevelDev fine, LevelDev coarse, const double* __restrict__ df, double* __restrict__ dc) {
+    __shared__ int ct[9];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 9) ct[threadIdx.x] = coarse.ctab[9 * t + threadIdx.x];
+    __syncthreads();
+    const int lx = threadIdx.x % TX;
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        const int kind = coarse.code[s] & 3;
+        double acc = 0.0;
+        if (kind == C_INNER) {
+#pragma unroll
+            for (int dy = -1; dy <= 1; dy++)
+#pragma unroll
+                for (int dx = -1; dx <= 1; dx++) {
+                    const int64_t fs = fine_slot(ct, 2 * lx + dx, 2 * ly + dy);
+                    const double w = (dx == 0 ? 2.0 : 1.0) * (dy == 0 ? 2.0 : 1.0) * 0.0625;
+                    if ((fine.code[fs] & 3) == C_INNER) acc += w * df[fs];
+                }
+        }
+        dc[s] = acc;        // coarse guard rows and absent slots: 0
+    }
+}
+
+// ---------------------------------------------------------------------------------- U1 coefficient restriction (rule T4)
+__global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev coarse) {
+    __shared__ int ct[9];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 9) ct[threadIdx.x] = coarse.ctab[9 * t + threadIdx.x];
+    __syncthreads();
+    const int lx = threadIdx.x % TX;
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        double sl = 0.0, sc = 0.0, sw = 0.0;
+        if ((coarse.code[s] & 3) != C_ABSENT) {
+#pragma unroll
+            for (int dy = -1; dy <= 1; dy++)
+#pragma unroll
+                for (int dx = -1; dx <= 1; dx++) {
+                    const int64_t fs = fine_slot(ct, 2 * lx + dx, 2 * ly + dy);
+                    const double w = (dx == 0 ? 2.0 : 1.0) * (dy == 0 ? 2.0 : 1.0) * 0.0625;
+                    if ((fine.code[fs] & 3) != C_ABSENT) { sl += w * fine.lam[fs]; sc += w * fine.c[fs]; sw += w; }
+                }
+            sl /= sw; sc /= sw;
+        }
+        coarse.lam[s] = sl;
+        coarse.c[s] = sc;
+    }
+}
+
+
+// ---------------------------------------------------------------------------------- S4 prolongation (rule T3)
+__device__ __forceinline__ int64_t parent_slot(const int* pt, int cx, int cy) {   // cx in [0, TX], cy in [0, TY]
+    const int ox = cx >= TX, oy = cy >= TY;
+    return (int64_t)pt[oy * 2 + ox] * TS + (cy - oy * TY) * TX + (cx - ox * TX);
+}
+
+// Phase A: e = P e_c on fine inner points (bilinear; absent parents hold 0), 0 elsewhere.
+__global__ void __launch_bounds__(NT) k_prolong(LevelDev fine, const double* __restrict__ ec, double* __restrict__ ef) {
+    __shared__ int pt[4];
+    __shared__ int odd[2];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 4) pt[threadIdx.x] = fine.ptab[4 * t + threadIdx.x];
+    if (threadIdx.x < 2) odd[threadIdx.x] = fine.tij[2 * t + threadIdx.x] & 1;
+    __syncthreads();
+    const int lx = threadIdx.x % TX;
+    const int cx = odd[0] * (TX / 2) + (lx >> 1);
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        double e = 0.0;
+        if ((fine.code[s] & 3) == C_INNER) {
+            const int cy = odd[1] * (TY / 2) + (ly >> 1);
+            const int ax = lx & 1, ay = ly & 1;
+            if (!ax && !ay) e = ec[parent_slot(pt, cx, cy)];
+            else if (ax && !ay) e = 0.5 * ec[parent_slot(pt, cx, cy)] + 0.5 * ec[parent_slot(pt, cx + 1, cy)];
+            else if (!ax && ay) e = 0.5 * ec[parent_slot(pt, cx, cy)] + 0.5 * ec[parent_slot(pt, cx, cy + 1)];
+            else e = 0.25 * ec[parent_slot(pt, cx, cy)] + 0.25 * ec[parent_slot(pt, cx + 1, cy)] +
+                     0.25 * ec[parent_slot(pt, cx, cy + 1)] + 0.25 * ec[parent_slot(pt, cx + 1, cy + 1)];
+        }
+        ef[s] = e;
+    }
+}
+
+// Phase B: set_bnds_hom on the guards of e (homogeneous Eq. 11 / Eq. 16), then x <- x - e.
+__global__ void __launch_bounds__(NT) k_correct(LevelDev fine, const double* __restrict__ ef, VecRef xr) {
+    __shared__ int tn[9];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 9) tn[threadIdx.x] = fine.tnb[9 * t + threadIdx.x];
+    __syncthreads();
+    double* __restrict__ x = resolve(xr);
+    const int lx = threadIdx.x % TX;
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        const uint16_t code = fine.code[s];
+        const int kind = code & 3;
+        if (kind == C_INNER) x[s] -= ef[s];
+        else if (kind == C_NEU) {
+            double sum, wself, delta;
+            neumann_row(code, tn, lx, ly, ef, fine.h, sum, wself, delta);
+            x[s] -= sum / (1.0 - wself);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------- small helpers
+__global__ void k_zero(VecRef xr, int64_t n) {
+    double* x = resolve(xr);
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) x[k] = 0.0;
+}
+__global__ void k_gather(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n) {
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[slot[k]] = src[k];
+}
+__global__ void k_scatter(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n) {
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[k] = src[slot[k]];
+}
+
+inline int grid1d(int64_t n) { return (int)std::min<int64_t>((n + 255) / 256, 148 * 8); }
+inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; }
+
+}  // namespace
+
+void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRef y, int mode) {
+    if (mode == 0) k_apply<0><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
+    else if (mode == 1) k_apply<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
+    else k_apply<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
+    count(L);
+}
+
+void launch_gs_sweep(const Launch& L, const LevelDev& lv, VecRef x, VecRef b) {
+    k_gs_group<0><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b);
+    k_gs_group<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b);
+    k_gs_group<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b);
+    count(L, 3);
+}
+
+void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse) {
+    k_restrict<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse, d_fine, d_coarse);
+    count(L);
+}
+
+void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
+                            double* e_fine_tmp, VecRef x_fine) {
+    (void)coarse;
+    k_prolong<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_coarse, e_fine_tmp);
+    k_correct<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_fine_tmp, x_fine);
+    count(L, 2);
+}
+
+void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse) {
+    k_restrict_coeff<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse);
+    count(L);
+}
+
+void launch_zero(const Launch& L, VecRef x, int64_t n) {
+    k_zero<<<grid1d(n), 256, 0, L.stream>>>(x, n);
+    count(L);
+}
+void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n) {
+    k_gather<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n);
+    count(L);
+}
+void launch_scatter(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n) {
+    k_scatter<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n);
+    count(L);
+}
+
+}  // namespace mgb

@@ -1,0 +1,250 @@
+// fGMRES(m) vector kernels (rules K1-K5; Saad's flexible GMRES).  The paper drives
+// GMRES from the host through a reverse-communication interface; here the Hessenberg
+// column, Givens rotations, least-squares right-hand side and the stop test (Eq. 23) stay
+// on the device in GmresState; every kernel reads the running column index j from it, so one captured
+// graph serves all iterations.
+//
+// Orthogonalisation: classical Gram-Schmidt applied twice (CGS2): fused multi-dot (one pass over w and
+// v_0..v_j), fused update + norm; twice.  Same Krylov iterates as the oracle's modified Gram-Schmidt up
+// to rounding.  Grid reductions: per-block partials + last-block-done ticket, summed in a fixed order
+// (deterministic run to run).
+#include "mg_device.h"
+
+namespace mgb {
+
+namespace {
+
+constexpr int CH = 8;   // basis vectors per register chunk in the multi-dot
+
+__device__ __forceinline__ double warp_sum(double v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Block-level sum; result valid in thread 0.
+__device__ __forceinline__ double block_sum(double v, double* sm) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (threadIdx.x < 32) {
+        r = (threadIdx.x < (blockDim.x >> 5)) ? sm[threadIdx.x] : 0.0;
+        r = warp_sum(r);
+    }
+    return r;
+}
+
+// true in every thread of the block that arrived last
+__device__ __forceinline__ bool last_block(GmresState* st) {
+    __shared__ int is_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int t = atomicAdd(&st->ticket, 1);
+        is_last = (t == (int)gridDim.x - 1);
+        if (is_last) st->ticket = 0;
+    }
+    __syncthreads();
+    if (is_last) __threadfence();
+    return is_last;
+}
+
+__global__ void __launch_bounds__(RED_THREADS) k_norm2(const double* __restrict__ v, int64_t n, GmresState* st,
+                                                      double* __restrict__ partial, int which) {
+    __shared__ double sm[32];
+    double acc = 0.0;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        const double a = v[k];
+        acc += a * a;
+    }
+    acc = block_sum(acc, sm);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+    if (last_block(st)) {
+        double s = 0.0;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) s += ((volatile double*)partial)[b];
+        s = block_sum(s, sm);
+        if (threadIdx.x == 0) {
+            if (which == 0) st->bn = sqrt(s); else st->beta = sqrt(s);
+        }
+    }
+}
+
+// K1/K2/K5: relres = beta / bn decides converged / restart; v_0 = r / beta; g = (beta, 0, ...).
+__global__ void k_start_cycle(GmresState* st, const double* __restrict__ r, double* __restrict__ V0, int64_t n) {
+    const double beta = st->beta, bn = st->bn;
+    const double relres = (bn > 0.0) ? beta / bn : 0.0;
+    const bool conv = (bn == 0.0) || (relres < st->rtol);
+    const bool capped = st->iters >= st->max_iters;
+    const bool broke = st->status == 3;
+    __syncthreads();
+    if (!conv && !capped && !broke) {
+        const double inv = 1.0 / beta;
+        for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) V0[k] = r[k] * inv;
+    }
+    // the header is rewritten by one thread after every block has read it
+    __shared__ int dummy;
+    (void)dummy;
+    if (last_block(st) && threadIdx.x == 0) {
+        st->relres = relres;
+        if (bn == 0.0) { st->status = 4; st->cycle_end = 1; }           // zero right-hand side: x = 0 (K1)
+        else if (conv) { st->status = 1; st->cycle_end = 1; }
+        else if (broke) { st->cycle_end = 1; }
+        else if (capped) { st->status = 2; st->cycle_end = 1; }
+        else { st->status = 0; st->cycle_end = 0; st->j = 0; st->g[0] = beta; }
+    }
+}
+
+// red[i] = (w, v_i), i = 0..j.  One pass over w per chunk of CH basis vectors.
+__global__ void __launch_bounds__(RED_THREADS) k_multidot(const double* __restrict__ w, const double* __restrict__ V, int64_t stride,
+                                                         int64_t n, GmresState* st, double* __restrict__ partial) {
+    __shared__ double sm[32];
+    if (st->cycle_end) return;
+    const int nv = st->j + 1;
+    for (int i0 = 0; i0 < nv; i0 += CH) {
+        double acc[CH];
+#pragma unroll
+        for (int c = 0; c < CH; c++) acc[c] = 0.0;
+        const int nc = min(CH, nv - i0);
+        for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+            const double wk = w[k];
+#pragma unroll
+            for (int c = 0; c < CH; c++)
+                if (c < nc) acc[c] += wk * V[(int64_t)(i0 + c) * stride + k];
+        }
+#pragma unroll
+        for (int c = 0; c < CH; c++) {
+            const double s = block_sum(acc[c], sm);
+            if (threadIdx.x == 0 && c < nc) partial[(size_t)blockIdx.x * (MAX_M + 2) + i0 + c] = s;
+        }
+    }
+    if (last_block(st)) {
+        for (int i = threadIdx.x; i < nv; i += blockDim.x) {
+            double s = 0.0;
+            for (int b = 0; b < (int)gridDim.x; b++) s += ((volatile double*)partial)[(size_t)b * (MAX_M + 2) + i];
+            st->red[i] = s;
+        }
+    }
+}
+
+// w -= sum_i red[i] v_i ; hcol (+)= red ; hcol[j+1] = ||w||.
+__global__ void __launch_bounds__(RED_THREADS) k_update_w(double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
+                                                         GmresState* st, double* __restrict__ partial, int pass) {
+    __shared__ double sm[32];
+    __shared__ double hh[MAX_M + 1];
+    if (st->cycle_end) return;
+    const int nv = st->j + 1;
+    for (int i = threadIdx.x; i < nv; i += blockDim.x) hh[i] = st->red[i];
+    __syncthreads();
+    double acc = 0.0;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        double s = w[k];
+#pragma unroll 4
+        for (int i = 0; i < nv; i++) s -= hh[i] * V[(int64_t)i * stride + k];
+        w[k] = s;
+        acc += s * s;
+    }
+    acc = block_sum(acc, sm);
+    if (threadIdx.x == 0) partial[(size_t)blockIdx.x * (MAX_M + 2) + MAX_M + 1] = acc;
+    if (last_block(st)) {
+        double s = 0.0;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) s += ((volatile double*)partial)[(size_t)b * (MAX_M + 2) + MAX_M + 1];
+        s = block_sum(s, sm);
+        for (int i = threadIdx.x; i < nv; i += blockDim.x) st->hcol[i] = (pass == 0) ? hh[i] : st->hcol[i] + hh[i];
+        if (threadIdx.x == 0) st->hcol[nv] = sqrt(s);
+    }
+}
+
+// K2/K3: rotate the new Hessenberg column, update g, count the iteration, evaluate the stop test.
+__global__ void k_givens(GmresState* st) {
+    if (threadIdx.x != 0 || st->cycle_end) return;
+    const int j = st->j, m = st->m;
+    double* H = st->H;
+    for (int i = 0; i <= j + 1; i++) H[i * MAX_M + j] = st->hcol[i];
+    const double hn = st->hcol[j + 1];
+    for (int i = 0; i < j; i++) {
+        const double a = H[i * MAX_M + j], b = H[(i + 1) * MAX_M + j];
+        H[i * MAX_M + j] = st->cs[i] * a + st->sn[i] * b;
+        H[(i + 1) * MAX_M + j] = -st->sn[i] * a + st->cs[i] * b;
+    }
+    const double rho = hypot(H[j * MAX_M + j], hn);
+    st->cs[j] = H[j * MAX_M + j] / rho;
+    st->sn[j] = hn / rho;
+    H[j * MAX_M + j] = rho;
+    H[(j + 1) * MAX_M + j] = 0.0;
+    st->g[j + 1] = -st->sn[j] * st->g[j];
+    st->g[j] = st->cs[j] * st->g[j];
+    st->iters += 1;
+    const double rel = fabs(st->g[j + 1]) / st->bn;
+    if (st->iters <= 512) st->hist[st->iters - 1] = rel;
+    st->hn = hn;
+    st->inv_hn = hn > 0.0 ? 1.0 / hn : 0.0;
+    st->j = j + 1;
+    if (rel < st->rtol) st->cycle_end = 1;                              // K3 (confirmed by the true residual, K5)
+    else if (hn == 0.0) { st->status = 3; st->cycle_end = 1; }          // breakdown
+    else if (j + 1 >= m || st->iters >= st->max_iters) st->cycle_end = 1;
+}
+
+// v_{j+1} = w / h_{j+1,j}
+__global__ void k_next_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n, GmresState* st) {
+    if (st->cycle_end) return;
+    double* v = V + (int64_t)st->j * stride;
+    const double inv = st->inv_hn;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) v[k] = w[k] * inv;
+}
+
+// K4: back-substitute R y = g (tiny; redone by every block), x += sum_i y_i z_i.
+__global__ void __launch_bounds__(256) k_update_x(double* __restrict__ x, const double* __restrict__ Z, int64_t stride, int64_t n, GmresState* st) {
+    __shared__ double y[MAX_M];
+    const int nv = st->j;
+    if (threadIdx.x == 0) {
+        for (int i = nv - 1; i >= 0; i--) {
+            double s = st->g[i];
+            for (int k = i + 1; k < nv; k++) s -= st->H[i * MAX_M + k] * y[k];
+            y[i] = s / st->H[i * MAX_M + i];
+        }
+    }
+    __syncthreads();
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        double s = x[k];
+#pragma unroll 4
+        for (int i = 0; i < nv; i++) s += y[i] * Z[(int64_t)i * stride + k];
+        x[k] = s;
+    }
+}
+
+__global__ void k_init_state(GmresState* st, int m, int max_iters, double rtol) {
+    if (threadIdx.x != 0) return;
+    st->j = 0; st->iters = 0; st->status = 0; st->cycle_end = 0; st->m = m; st->max_iters = max_iters;
+    st->ticket = 0; st->rtol = rtol; st->bn = 0.0; st->beta = 0.0; st->relres = 0.0; st->hn = 0.0; st->inv_hn = 0.0;
+}
+
+inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; }
+
+}  // namespace
+
+void launch_norm2(const Launch& L, const double* v, int64_t n, GmresState* st, double* partial, int which) {
+    k_norm2<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(v, n, st, partial, which); count(L);
+}
+void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double* V0, int64_t n) {
+    k_start_cycle<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
+}
+void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial) {
+    k_multidot<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial); count(L);
+}
+void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass) {
+    k_update_w<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
+}
+void launch_givens(const Launch& L, GmresState* st) { k_givens<<<1, 32, 0, L.stream>>>(st); count(L); }
+void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
+    k_next_v<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+}
+void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st) {
+    k_update_x<<<RED_BLOCKS, 256, 0, L.stream>>>(x, Z, stride, n, st); count(L);
+}
+void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol) {
+    k_init_state<<<1, 32, 0, L.stream>>>(st, m, max_iters, rtol); count(L);
+}
+void launch_final_check(const Launch&, GmresState*) {}
+
+}  // namespace mgb

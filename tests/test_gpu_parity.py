@@ -1,0 +1,136 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI, against the CPU oracle on the
+same seeded inputs.  Tolerances (north_star): single operator / smoother / transfer applications
+1e-13 relative L2 in fp64; solves to rtol 1e-10 agree within 1e-8 relative L2 with iteration counts
+equal +-1; index construction bit-exact (tests/test_host_setup.py covers the latter on the CPU and is
+repeated here on the handle the kernels really use)."""
+import numpy as np
+import pytest
+
+from paper_2509_11831_b200 import workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-13
+TOL_SOLVE = 1e-8
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2509_11831_b200 import binding as B
+    B.lib()
+    B.use_torch_allocator()
+    return B
+
+
+def rel(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def host(t):
+    return t.cpu().numpy()
+
+
+CASES = {
+    "cfg1_square65": lambda: W.make_plane(1),
+    "cfg2_annulus129_shuffled": lambda: W.make_plane(2, 129, order="shuffle"),
+    "cfg2_annulus513": lambda: W.make_plane(2),
+    "cfg3_dshape257": lambda: W.make_plane(3, 257),
+    "cfg4_dshape257": lambda: W.make_plane(4, 257),
+    "annulus65_negative_origin": lambda: H.small_annulus(65, 4, i0=-37, j0=-22),
+}
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def pair(request, gpu, oracle_mod):
+    import torch
+    pl = CASES[request.param]()
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    torch.cuda.synchronize()
+    yield pl, o, s
+    s.close()
+
+
+def test_levels_and_coefficients(pair):
+    pl, o, s = pair
+    assert s.levels == o.levels
+    for lv in range(o.levels):
+        a, g = o.level_arrays(lv), s.level_info(lv)
+        for k in ("I", "J", "kind", "colour", "nbr", "ns_fallback"):
+            assert np.array_equal(a[k], g[k])
+        lo, co = o.level_coeffs(lv)
+        lg, cg = s.level_coeffs(lv)
+        assert rel(lg, lo) <= TOL_STEP and rel(cg, co) <= TOL_STEP       # U1, rule T4
+        assert (cg > 0).all()
+
+
+def test_apply(pair):
+    pl, o, s = pair
+    rng = np.random.default_rng(1)
+    for lv in range(o.levels):
+        x = rng.standard_normal(o.level_n(lv))
+        assert rel(host(s.apply(lv, dev(x))), o.apply(lv, x)) <= TOL_STEP
+
+
+def test_smoother(pair):
+    pl, o, s = pair
+    rng = np.random.default_rng(2)
+    for lv in range(o.levels):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        for sweeps in (1, 3):
+            assert rel(host(s.smooth(lv, dev(x), dev(b), sweeps)), o.smooth(lv, x, b, sweeps)) <= TOL_STEP
+
+
+def test_transfers(pair):
+    pl, o, s = pair
+    rng = np.random.default_rng(3)
+    for lv in range(o.levels - 1):
+        d = rng.standard_normal(o.level_n(lv))
+        assert rel(host(s.restrict(lv, dev(d))), o.restrict(lv, d)) <= TOL_STEP
+        ec, x = rng.standard_normal(o.level_n(lv + 1)), rng.standard_normal(o.level_n(lv))
+        assert rel(host(s.prolong_correct(lv, dev(ec), dev(x))), o.prolong_correct(lv, ec, x)) <= TOL_STEP
+
+
+def test_coarse_solve(pair):
+    pl, o, s = pair
+    b = np.random.default_rng(4).standard_normal(o.level_n(o.levels - 1))
+    # both sides are direct solves of the same dense system: forward error <= cond * eps
+    assert rel(host(s.coarse_solve(dev(b))), o.coarse_solve(b)) <= 1e-11
+
+
+def test_vcycle(pair):
+    pl, o, s = pair
+    rng = np.random.default_rng(5)
+    for lv in (0, max(0, o.levels - 2)):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        assert rel(host(s.vcycle(lv, dev(x), dev(b))), o.cycle(lv, x, b)) <= 1e-12
+
+
+def test_solve(pair):
+    pl, o, s = pair
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    x, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert rc == 0 and ro["status"] == 0
+    assert abs(iters - ro["iters"]) <= 1
+    assert rel(host(x), ro["x"]) <= TOL_SOLVE
+    assert relres < 1e-10
+    # the reported residual is the true one, recomputed by the oracle's operator (Eq. 23)
+    xc = H.canon(o, host(x)); fc = H.canon(o, pl.f)
+    true = np.linalg.norm(fc - o.apply(0, xc)) / np.linalg.norm(fc)
+    assert true < 1.05e-10 and relres == pytest.approx(true, rel=1e-3)
+    # host-buffer entry points give the same answer
+    s.update_coeffs_host(pl.lam, pl.c)
+    xh, it2, rr2, rc2 = s.solve_host(pl.f, pl.x0, 1e-10)
+    assert rc2 == 0 and it2 == iters and rel(xh, host(x)) <= 1e-12
