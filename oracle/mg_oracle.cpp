@@ -256,8 +256,11 @@ static inline double row_apply(const Level& lv, int64_t l, const double* x) {
         const double aE = kappa * (cl + lv.c[nb[1]]);
         const double aS = kappa * (cl + lv.c[nb[2]]);
         const double aN = kappa * (cl + lv.c[nb[3]]);
-        const double all = lv.lam[l] + aW + aE + aS + aN;
-        return all * x[l] - aW * x[nb[0]] - aE * x[nb[1]] - aS * x[nb[2]] - aN * x[nb[3]];
+        // same row as Eq. 10, evaluated in difference form (rule D1): lam x_l + sum a_nb (x_l - x_nb).
+        // Algebraically identical to a_ll x_l - sum a_nb x_nb, but free of the O(eps |a_ll x_l|)
+        // cancellation error that otherwise puts the attainable residual above 1e-10 at h ~ 5e-4.
+        const double xl = x[l];
+        return lv.lam[l] * xl + aW * (xl - x[nb[0]]) + aE * (xl - x[nb[1]]) + aS * (xl - x[nb[2]]) + aN * (xl - x[nb[3]]);
     }
     if (lv.kind[l] == DIRICHLET) return x[l];
     double phiN = lv.ns_wself[l] * x[l];
@@ -623,11 +626,15 @@ int orc_solve_ex(void* h, const double* f_user, const double* x0_user, double* x
             else if (precond == 1) Z[j] = V[j];
             else lu_solve(o->lu0, o->piv0, n, V[j].data(), Z[j].data());
             apply(lv, Z[j].data(), w.data());
-            for (int i = 0; i <= j; i++) {                                         // modified Gram-Schmidt
-                const double hij = dot(w.data(), V[i].data(), n);
-                H[(size_t)i * m + j] = hij;
-                for (int64_t k = 0; k < n; k++) w[k] -= hij * V[i][k];
-            }
+            // modified Gram-Schmidt, applied twice (reorthogonalisation, rule K2): the second pass keeps
+            // V orthogonal to working precision, so the iteration count does not depend on how the
+            // orthogonalisation rounds (identical counts across backends)
+            for (int pass = 0; pass < 2; pass++)
+                for (int i = 0; i <= j; i++) {
+                    const double hij = dot(w.data(), V[i].data(), n);
+                    H[(size_t)i * m + j] += hij;
+                    for (int64_t k = 0; k < n; k++) w[k] -= hij * V[i][k];
+                }
             const double hn = std::sqrt(dot(w.data(), w.data(), n));
             H[(size_t)(j + 1) * m + j] = hn;
             if (first_cycle) for (int i = 0; i <= j + 1; i++) Hraw[(size_t)i * m + j] = H[(size_t)i * m + j];

@@ -72,8 +72,8 @@ __global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br,
             const double cl = lv.c[s];
             const double aW = lv.kappa * (cl + lv.c[sW]), aE = lv.kappa * (cl + lv.c[sE]);
             const double aS = lv.kappa * (cl + lv.c[sS]), aN = lv.kappa * (cl + lv.c[sN]);
-            const double all = lv.lam[s] + aW + aE + aS + aN;
-            ax = all * x[s] - aW * x[sW] - aE * x[sE] - aS * x[sS] - aN * x[sN];
+            const double xl = x[s];                                     // difference form (rule D1)
+            ax = lv.lam[s] * xl + aW * (xl - x[sW]) + aE * (xl - x[sE]) + aS * (xl - x[sS]) + aN * (xl - x[sN]);
         } else if (kind == C_DIR) {                                     // Eq. 11
             ax = x[s];
         } else if (kind == C_NEU) {                                     // Eq. 16
