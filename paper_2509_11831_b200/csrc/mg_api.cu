@@ -32,7 +32,7 @@ mg_free_fn g_free = nullptr;
 struct LevelBuf {           // device arrays owned per level
     uint16_t* code = nullptr;
     int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
-    double *lam = nullptr, *c = nullptr, *x = nullptr, *b = nullptr, *d = nullptr;
+    double *lam = nullptr, *c = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
 };
 
 }  // namespace
@@ -95,28 +95,44 @@ int upload(mg_handle h, T** dst, const std::vector<T>& src, cudaStream_t s) {
 
 Launch LZ(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }
 
-// mg_cycle of PAPER.md:171-195 with gamma = 1, enqueued on L.stream.
-void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b) {
+// nu Gauss-Seidel sweeps, two per launch where possible, ping-ponging between `cur` and `other`.
+// Returns the buffer that holds the result.
+VecRef enqueue_smooth(const Launch& L, const LevelDev& lv, VecRef cur, VecRef other, VecRef b, int nu, bool cur_is_zero) {
+    while (nu > 0) {
+        const int k = nu >= 2 ? 2 : 1;
+        launch_gs_fused(L, lv, cur, other, b, k, cur_is_zero);
+        std::swap(cur, other);
+        cur_is_zero = false;
+        nu -= k;
+    }
+    return cur;
+}
+
+// mg_cycle of PAPER.md:171-195 with gamma = 1, enqueued on L.stream.  x_is_zero: the initial guess is
+// the zero vector and x need not be read (nor zeroed beforehand).
+void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero) {
     const LevelDev& lv = h->lev[s];
     if (s == h->L - 1) {                                              // P:173-177 direct solve
         launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, b, x);
         return;
     }
-    for (int k = 0; k < h->nu_pre; k++) launch_gs_sweep(L, lv, x, b);
-    launch_apply(L, lv, x, b, vec(h->buf[s].d), 2);                             // P:183  d = A x - b
-    launch_restrict(L, lv, h->lev[s + 1], h->buf[s].d, h->buf[s + 1].b);        // P:184
-    if (s + 1 < h->L - 1) launch_zero(L, vec(h->buf[s + 1].x), h->lev[s + 1].nslots);   // P:186  e = 0
-    enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b));
-    launch_prolong_correct(L, lv, h->lev[s + 1], h->buf[s + 1].x, h->buf[s].d, x);
-    for (int k = 0; k < h->nu_post; k++) launch_gs_sweep(L, lv, x, b);
+    VecRef tmp = vec(h->buf[s].x2);
+    if (x_is_zero && h->nu_pre == 0) { launch_zero(L, x, lv.nslots); x_is_zero = false; }
+    VecRef cur = enqueue_smooth(L, lv, x, tmp, b, h->nu_pre, x_is_zero);
+    VecRef other = (cur.base == x.base) ? tmp : x;
+    launch_apply(L, lv, cur, b, vec(h->buf[s].d), 2);                                     // P:183  d = A x - b
+    launch_restrict(L, lv, h->lev[s + 1], h->buf[s].d, h->buf[s + 1].b);                  // P:184
+    enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), true);         // P:186-189, e0 = 0
+    launch_prolong_correct(L, lv, h->lev[s + 1], h->buf[s + 1].x, h->buf[s].d, cur);
+    VecRef fin = enqueue_smooth(L, lv, cur, other, b, h->nu_post, false);
+    if (fin.base != x.base) launch_copy(L, fin, x, lv.nslots);
 }
 
 // One Arnoldi step (rule K2): z_j = MG(v_j), w = A z_j, CGS2, Givens + stop test, v_{j+1}.
 void enqueue_iteration(mg_handle h, const Launch& L) {
     const int64_t ns = h->lev[0].nslots;
     VecRef zj{h->Z, ns, &h->st->j, 0}, vj{h->V, ns, &h->st->j, 0};
-    launch_zero(L, zj, ns);
-    enqueue_cycle(h, L, 0, zj, vj);
+    enqueue_cycle(h, L, 0, zj, vj, true);
     launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
     launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
     launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 0);
@@ -228,6 +244,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         TRY(dev_alloc(h, (void**)&b.lam, vb, s));
         TRY(dev_alloc(h, (void**)&b.c, vb, s));
         TRY(dev_alloc(h, (void**)&b.x, vb, s));
+        TRY(dev_alloc(h, (void**)&b.x2, vb, s));
         TRY(dev_alloc(h, (void**)&b.b, vb, s));
         TRY(dev_alloc(h, (void**)&b.d, vb, s));
         LevelDev& d = h->lev[l];
@@ -503,8 +520,8 @@ int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps
     const int64_t n = h->hh.lev[level].n;
     launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
     launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
-    for (int k = 0; k < sweeps; k++) launch_gs_sweep(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].b));
-    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
+    VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].b), sweeps, false);
+    launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n);
     CU(cudaGetLastError());
     return MG_OK;
 }
@@ -548,7 +565,7 @@ int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stre
     // level buffers x/b of `level` are free here: the recursion only uses those of the coarser levels
     launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
     launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
-    enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].b));
+    enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].b), false);
     launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
     CU(cudaGetLastError());
     return MG_OK;

@@ -14,8 +14,8 @@ namespace mgb {
 // (id = ntiles) is the all-absent "null tile" every missing neighbour points to, so that halo
 // addressing needs no branch.  TX and TY are even, hence colour(I + J) == colour(lx + ly) and a
 // coarse tile covers exactly 2 x 2 fine tiles.
-constexpr int TX = 32;
-constexpr int TY = 16;
+constexpr int TX = 64;
+constexpr int TY = 32;
 constexpr int TS = TX * TY;
 
 // Per-slot 16-bit code.

@@ -69,7 +69,11 @@ struct Launch {
 // ---- tile kernels (mg_kernels.cu) ----
 // mode 0: y = A x      1: y = b - A x      2: y = A x - b
 void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRef y, int mode);
-void launch_gs_sweep(const Launch& L, const LevelDev& lv, VecRef x, VecRef b);
+// `sweeps` (1 or 2) full red-black-boundary Gauss-Seidel sweeps in ONE pass over memory: x_out = S^sweeps x_in.
+// x_in and x_out must be different buffers (halo cells are recomputed by neighbouring CTAs);
+// x_in_zero: treat x_in as the zero vector without reading it.
+void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero);
+void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n);
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse);
 void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
                             double* e_fine_tmp, VecRef x_fine);

@@ -10,7 +10,7 @@ namespace mgb {
 
 namespace {
 
-constexpr int NT = 256;                 // threads per CTA: 32 x 8, two rows per thread
+constexpr int NT = 512;                 // threads per CTA: 64 x 8, four rows per thread
 constexpr int ROWS_PER_PASS = NT / TX;  // 8
 
 // slot of the point at local offset (lx, ly) in [-TX, 2TX) x [-TY, 2TY) relative to tile whose 3x3
@@ -89,41 +89,7 @@ __global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br,
     }
 }
 
-// ---------------------------------------------------------------------------------- S2 smoother
-// One group of gauss_seidel_rbb: GROUP 0 red inner ((I+J) even), 1 black inner, 2 guards.
-template <int GROUP>
-__global__ void __launch_bounds__(NT) k_gs_group(LevelDev lv, VecRef xr, VecRef br) {
-    __shared__ int tn[9];
-    const int t = blockIdx.x;
-    if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
-    __syncthreads();
-    double* __restrict__ x = resolve(xr);
-    const double* __restrict__ b = resolve(br);
-    const int lx = threadIdx.x % TX;
-#pragma unroll
-    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
-        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
-        const int64_t s = (int64_t)t * TS + ly * TX + lx;
-        const uint16_t code = lv.code[s];
-        const int kind = code & 3;
-        if (GROUP < 2) {
-            if (kind != C_INNER || ((lx + ly) & 1) != GROUP) continue;
-            const int64_t sW = nslot(tn, lx - 1, ly), sE = nslot(tn, lx + 1, ly), sS = nslot(tn, lx, ly - 1), sN = nslot(tn, lx, ly + 1);
-            const double cl = lv.c[s];
-            const double aW = lv.kappa * (cl + lv.c[sW]), aE = lv.kappa * (cl + lv.c[sE]);
-            const double aS = lv.kappa * (cl + lv.c[sS]), aN = lv.kappa * (cl + lv.c[sN]);
-            const double all = lv.lam[s] + aW + aE + aS + aN;
-            x[s] = (b[s] + aW * x[sW] + aE * x[sE] + aS * x[sS] + aN * x[sN]) / all;
-        } else {
-            if (kind == C_DIR) x[s] = b[s];
-            else if (kind == C_NEU) {
-                double sum, wself, delta;
-                neumann_row(code, tn, lx, ly, x, lv.h, sum, wself, delta);
-                x[s] = (sum - delta * b[s]) / (1.0 - wself);
-            }
-        }
-    }
-}
+// (S2, the smoother, lives in mg_smoother.cu)
 
 // ---------------------------------------------------------------------------------- S3 restriction (rule T2)
 // One CTA per COARSE tile. Fine point (2 lxc + dx, 2 lyc + dy) lives in one of the 3x3 fine tiles of ctab.
@@ -267,13 +233,6 @@ void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRe
     else if (mode == 1) k_apply<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
     else k_apply<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
     count(L);
-}
-
-void launch_gs_sweep(const Launch& L, const LevelDev& lv, VecRef x, VecRef b) {
-    k_gs_group<0><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b);
-    k_gs_group<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b);
-    k_gs_group<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b);
-    count(L, 3);
 }
 
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse) {
