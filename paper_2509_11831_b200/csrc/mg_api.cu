@@ -135,6 +135,11 @@ void enqueue_iteration(mg_handle h, const Launch& L) {
     enqueue_cycle(h, L, 0, zj, vj, true);
     launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
     launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
+    if (h->m <= MAX_M_FUSED) {                                     // three passes over the basis
+        launch_update_dot(L, h->w, h->V, ns, ns, h->st, h->partial);
+        launch_final_v(L, h->w, h->V, ns, ns, h->st);
+        return;
+    }
     launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 0);
     launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
     launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 1);

@@ -93,6 +93,10 @@ void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double
 void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial);
 void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass);
 void launch_givens(const Launch& L, GmresState* st);
+// fused CGS2 for restart lengths m <= MAX_M_FUSED (three passes over the basis, Givens inside the second)
+constexpr int MAX_M_FUSED = 32;
+void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial);
+void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st);
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol);

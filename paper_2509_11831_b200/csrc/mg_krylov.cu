@@ -155,9 +155,9 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_w(double* __restrict__ w
     }
 }
 
-// K2/K3: rotate the new Hessenberg column, update g, count the iteration, evaluate the stop test.
-__global__ void k_givens(GmresState* st) {
-    if (threadIdx.x != 0 || st->cycle_end) return;
+// K2/K3: rotate the new Hessenberg column (st->hcol[0..j+1]), update g, count the iteration, evaluate the
+// stop test.  Serial, one thread.
+__device__ void givens_step(GmresState* st) {
     const int j = st->j, m = st->m;
     double* H = st->H;
     for (int i = 0; i <= j + 1; i++) H[i * MAX_M + j] = st->hcol[i];
@@ -183,6 +183,143 @@ __global__ void k_givens(GmresState* st) {
     if (rel < st->rtol) st->cycle_end = 1;                              // K3 (confirmed by the true residual, K5)
     else if (hn == 0.0) { st->status = 3; st->cycle_end = 1; }          // breakdown
     else if (j + 1 >= m || st->iters >= st->max_iters) st->cycle_end = 1;
+}
+
+__global__ void k_givens(GmresState* st) {
+    if (threadIdx.x != 0 || st->cycle_end) return;
+    givens_step(st);
+}
+
+// ---------------------------------------------------------------------------- fused CGS2 (m <= FUSED_NV)
+// Three passes over the basis per Arnoldi step instead of four:
+//   pass 1  k_multidot      h1 = V^T w
+//   pass 2  k_update_dot    w' = w - V h1 (written), h2 = V^T w', ||w'||^2 — V is read ONCE: the values used
+//                           for the update stay in registers for the second set of dot products; the last
+//                           block then forms h = h1 + h2, h_{j+1,j} = sqrt(||w'||^2 - sum h2^2) (exact for
+//                           orthonormal V; h2 = O(eps) after the first projection so nothing cancels) and runs
+//                           the Givens step, so no separate norm pass and no separate Givens launch
+//   pass 3  k_final_v       v_{j+1} = (w' - V h2) / h_{j+1,j}, written straight into the basis
+// Traffic at column j: 8(j+2) + (16 + 8(j+1)) + (16 + 8(j+1)) = 24 j + 64 B/pt against 32 j + 96.
+constexpr int FUSED_NV = 32;
+constexpr int UD_THREADS = 128;
+constexpr int UD_BLOCKS = 148 * 2;   // 254 registers x 128 threads: two blocks per SM, one wave
+
+// One grid-stride sweep with NV basis values x EPT elements held in registers per thread.
+template <int NV, int EPT>
+__device__ __forceinline__ void update_dot_body(double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
+                                                int nv, const double* hh, double (&acc)[FUSED_NV], double& accn) {
+    const int64_t G = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k0 < n; k0 += G * EPT) {
+        double v[EPT][NV], s[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+            const int64_t k = k0 + e * G;
+            const bool ok = k < n;
+            s[e] = ok ? w[k] : 0.0;
+#pragma unroll
+            for (int c = 0; c < NV; c++) v[e][c] = (ok && c < nv) ? V[(int64_t)c * stride + k] : 0.0;
+        }
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+            const int64_t k = k0 + e * G;
+#pragma unroll
+            for (int c = 0; c < NV; c++) s[e] -= hh[c] * v[e][c];
+            if (k < n) w[k] = s[e];
+            accn += s[e] * s[e];
+#pragma unroll
+            for (int c = 0; c < NV; c++) acc[c] += s[e] * v[e][c];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
+                                                            int64_t n, GmresState* st, double* __restrict__ partial) {
+    __shared__ double hh[FUSED_NV];
+    __shared__ double red[UD_THREADS / 32][FUSED_NV + 1];
+    __shared__ double tot[FUSED_NV + 1];
+    if (st->cycle_end) return;
+    const int nv = st->j + 1;
+    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
+    __syncthreads();
+    double acc[FUSED_NV], accn = 0.0;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) acc[c] = 0.0;
+    if (nv <= 8) update_dot_body<8, 4>(w, V, stride, n, nv, hh, acc, accn);
+    else if (nv <= 16) update_dot_body<16, 2>(w, V, stride, n, nv, hh, acc, accn);
+    else update_dot_body<32, 1>(w, V, stride, n, nv, hh, acc, accn);
+    // block reduction: warp shuffles, then one thread per value over the warps
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) {
+        const double r = warp_sum(acc[c]);
+        if (lane == 0) red[warp][c] = r;
+    }
+    accn = warp_sum(accn);
+    if (lane == 0) red[warp][FUSED_NV] = accn;
+    __syncthreads();
+    if (threadIdx.x <= FUSED_NV) {
+        double r = 0.0;
+        for (int q = 0; q < UD_THREADS / 32; q++) r += red[q][threadIdx.x];
+        partial[(size_t)blockIdx.x * (MAX_M + 2) + threadIdx.x] = r;
+    }
+    if (last_block(st)) {
+        if (threadIdx.x <= FUSED_NV) {
+            double r = 0.0;
+            for (int b = 0; b < (int)gridDim.x; b++) r += ((volatile double*)partial)[(size_t)b * (MAX_M + 2) + threadIdx.x];
+            tot[threadIdx.x] = r;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s2 = 0.0;
+            for (int i = 0; i < nv; i++) {
+                st->hcol[i] = hh[i] + tot[i];     // h_ij = first + second projection
+                st->red[i] = tot[i];              // h2, consumed by k_final_v
+                s2 += tot[i] * tot[i];
+            }
+            const double hn2 = tot[FUSED_NV] - s2;
+            st->hcol[nv] = hn2 > 0.0 ? sqrt(hn2) : 0.0;
+            givens_step(st);
+        }
+    }
+}
+
+template <int NV, int EPT>
+__device__ __forceinline__ void final_v_body(const double* __restrict__ w, const double* __restrict__ V, double* __restrict__ out,
+                                             int64_t stride, int64_t n, int nv, const double* hh, double inv) {
+    const int64_t G = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k0 < n; k0 += G * EPT) {
+        double v[EPT][NV], s[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+            const int64_t k = k0 + e * G;
+            const bool ok = k < n;
+            s[e] = ok ? w[k] : 0.0;
+#pragma unroll
+            for (int c = 0; c < NV; c++) v[e][c] = (ok && c < nv) ? V[(int64_t)c * stride + k] : 0.0;
+        }
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+            const int64_t k = k0 + e * G;
+#pragma unroll
+            for (int c = 0; c < NV; c++) s[e] -= hh[c] * v[e][c];
+            if (k < n) out[k] = s[e] * inv;
+        }
+    }
+}
+
+// v_{j+1} = (w' - V h2) / h_{j+1,j}; st->j has already been advanced by the Givens step.
+__global__ void __launch_bounds__(RED_THREADS) k_final_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n,
+                                                        GmresState* st) {
+    __shared__ double hh[FUSED_NV];
+    if (st->cycle_end) return;
+    const int nv = st->j;
+    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
+    __syncthreads();
+    double* out = V + (int64_t)nv * stride;
+    const double inv = st->inv_hn;
+    if (nv <= 8) final_v_body<8, 4>(w, V, out, stride, n, nv, hh, inv);
+    else if (nv <= 16) final_v_body<16, 2>(w, V, out, stride, n, nv, hh, inv);
+    else final_v_body<32, 1>(w, V, out, stride, n, nv, hh, inv);
 }
 
 // v_{j+1} = w / h_{j+1,j}
@@ -234,6 +371,12 @@ void launch_multidot(const Launch& L, const double* w, const double* V, int64_t 
 }
 void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass) {
     k_update_w<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
+}
+void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial) {
+    k_update_dot<<<UD_BLOCKS, UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial); count(L);
+}
+void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
+    k_final_v<<<148 * 2, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
 }
 void launch_givens(const Launch& L, GmresState* st) { k_givens<<<1, 32, 0, L.stream>>>(st); count(L); }
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {

@@ -134,3 +134,22 @@ def test_solve(pair):
     s.update_coeffs_host(pl.lam, pl.c)
     xh, it2, rr2, rc2 = s.solve_host(pl.f, pl.x0, 1e-10)
     assert rc2 == 0 and it2 == iters and rel(xh, host(x)) <= 1e-12
+
+
+@pytest.mark.parametrize("m,max_iters", [(4, 200), (40, 200), (30, 7)])
+def test_solve_restart_lengths(gpu, oracle_mod, m, max_iters):
+    """Restarts (K5), the unfused Gram-Schmidt path used for m > 32, and the iteration cap."""
+    pl = W.make_plane(3, 129)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, m=m, max_iters=max_iters)
+    o.update(pl.lam, pl.c)
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, restart_m=m, max_iters=max_iters)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    x, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    s.close()
+    assert rc == ro["status"]
+    assert abs(iters - ro["iters"]) <= 1
+    if rc == 0:
+        assert rel(host(x), ro["x"]) <= TOL_SOLVE and relres < 1e-10
+    else:                                   # capped: both stopped at max_iters with the same iterate
+        assert iters == max_iters and rel(host(x), ro["x"]) <= 1e-6
