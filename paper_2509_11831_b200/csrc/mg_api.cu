@@ -65,6 +65,7 @@ struct mg_handle_s {
     int64_t iter_graph_kernels = 0;
     int64_t launches = 0;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t hev[2] = {nullptr, nullptr};   // header copies of the two Arnoldi steps in flight
     bool solve_timed = false, update_timed = false;
 };
 
@@ -123,8 +124,15 @@ void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
     launch_apply(L, lv, cur, b, vec(h->buf[s].d), 2);                                     // P:183  d = A x - b
     launch_restrict(L, lv, h->lev[s + 1], h->buf[s].d, h->buf[s + 1].b);
     enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), true);         // P:186-189, e0 = 0
-    launch_prolong_correct(L, lv, h->lev[s + 1], h->buf[s + 1].x, h->buf[s].d, cur);
-    VecRef fin = enqueue_smooth(L, lv, cur, other, b, h->nu_post, false);
+    VecRef fin;
+    if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass
+        const int k = h->nu_post >= 2 ? 2 : 1;
+        launch_gs_correct(L, lv, h->buf[s + 1].x, cur, other, b, k);
+        fin = enqueue_smooth(L, lv, other, cur, b, h->nu_post - k, false);
+    } else {
+        launch_prolong_correct(L, lv, h->lev[s + 1], h->buf[s + 1].x, h->buf[s].d, cur);
+        fin = cur;
+    }
     if (fin.base != x.base) launch_copy(L, fin, x, lv.nslots);
 }
 
@@ -152,7 +160,9 @@ int build_iter_graph(mg_handle h) {
     cudaGraph_t g = nullptr;
     const int64_t before = h->launches;
     CU(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    enqueue_iteration(h, LZ(h, h->cap_stream));
+    Launch L = LZ(h, h->cap_stream);
+    L.stop = &h->st->cycle_end;          // iterations are enqueued one ahead of the convergence test
+    enqueue_iteration(h, L);
     CU(cudaStreamEndCapture(h->cap_stream, &g));
     h->iter_graph_kernels = h->launches - before;
     h->launches = before;
@@ -195,6 +205,7 @@ int mg_destroy(mg_handle h) {
     if (h->iter_graph) cudaGraphExecDestroy(h->iter_graph);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+    for (auto& e : h->hev) if (e) cudaEventDestroy(e);
     if (h->h_hdr) cudaFreeHost(h->h_hdr);
     if (h->h_state) cudaFreeHost(h->h_state);
     for (void* p : h->allocs) { if (g_free) g_free(p); else cudaFree(p); }
@@ -231,6 +242,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
 #define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_error = std::string(#call) + ": " + cudaGetErrorString(e__); return fail(MG_ECUDA); } } while (0)
     CUF(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     for (auto& e : h->ev) CUF(cudaEventCreate(&e));
+    for (auto& e : h->hev) CUF(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     CUF(cudaMallocHost((void**)&h->h_hdr, 64));
     CUF(cudaMallocHost((void**)&h->h_state, sizeof(GmresState)));
     h->lev.resize(h->L); h->buf.resize(h->L);
@@ -331,12 +343,18 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
         CU(cudaStreamSynchronize(s));
         status = h->h_hdr[2];
         if (h->h_hdr[3]) break;                                       // cycle_end set by start: finished
+        // One graph launch per Arnoldi step.  The host stays one step ahead: step `it` is enqueued before
+        // the header of step it-1 is inspected, so the GPU never idles on the round trip; a step enqueued
+        // after the cycle has ended finds cycle_end set and every kernel in it returns at once.
         for (int it = 0; it < h->m; it++) {
             CU(cudaGraphLaunch(h->iter_graph, s));
             h->launches += h->iter_graph_kernels;
-            CU(cudaMemcpyAsync(h->h_hdr, h->st, 32, cudaMemcpyDeviceToHost, s));
-            CU(cudaStreamSynchronize(s));
-            if (h->h_hdr[3]) break;
+            CU(cudaMemcpyAsync(h->h_hdr + 8 * (it & 1), h->st, 32, cudaMemcpyDeviceToHost, s));
+            CU(cudaEventRecord(h->hev[it & 1], s));
+            if (it >= 1) {
+                CU(cudaEventSynchronize(h->hev[(it - 1) & 1]));
+                if (h->h_hdr[8 * ((it - 1) & 1) + 3]) break;
+            }
         }
         launch_update_x(L, h->xs, h->Z, ns, ns, h->st);               // K4
     }

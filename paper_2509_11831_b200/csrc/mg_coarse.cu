@@ -118,8 +118,9 @@ __global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict_
 
 // x = A^-1 b on the coarsest level; vectors in the tile layout, rows addressed through cslot.
 __global__ void __launch_bounds__(CT) k_coarse_solve(const double* __restrict__ Ainv, const int32_t* __restrict__ cslot, int n,
-                                                     VecRef br, VecRef xr) {
+                                                     VecRef br, VecRef xr, const int* __restrict__ stop) {
     __shared__ double sb[1024];
+    if (stop != nullptr && *stop) return;
     const double* __restrict__ b = resolve(br);
     double* __restrict__ x = resolve(xr);
     for (int r = threadIdx.x; r < n; r += CT) sb[r] = b[cslot[r]];
@@ -143,7 +144,7 @@ void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cs
 }
 
 void launch_coarse_solve(const Launch& L, const double* Ainv, const int32_t* cslot, int n, VecRef b_tiled, VecRef x_tiled) {
-    k_coarse_solve<<<1, CT, 0, L.stream>>>(Ainv, cslot, n, b_tiled, x_tiled);
+    k_coarse_solve<<<1, CT, 0, L.stream>>>(Ainv, cslot, n, b_tiled, x_tiled, L.stop);
     if (L.counter) *L.counter += 1;
 }
 

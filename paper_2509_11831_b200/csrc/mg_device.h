@@ -22,7 +22,7 @@ struct LevelDev {
     const uint16_t* code;
     const int32_t* tnb;      // 9 per tile
     const int32_t* ctab;     // 9 per tile (this level as the coarse side)
-    const int32_t* ptab;     // 4 per tile (this level as the fine side)
+    const int32_t* ptab;     // 9 per tile (this level as the fine side): coarse tiles around the parent tile
     const int32_t* tij;      // 2 per tile: tile coordinates (TI, TJ)
     double* lam;
     double* c;
@@ -64,6 +64,8 @@ struct GmresState {
 struct Launch {
     cudaStream_t stream;
     int64_t* counter;   // host counter of kernel launches (may be null)
+    const int* stop = nullptr;   // device flag: V-cycle kernels return at once when *stop != 0 (iterations
+                                 // enqueued ahead of the convergence test), null = always run
 };
 
 // ---- tile kernels (mg_kernels.cu) ----
@@ -73,6 +75,8 @@ void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRe
 // x_in and x_out must be different buffers (halo cells are recomputed by neighbouring CTAs);
 // x_in_zero: treat x_in as the zero vector without reading it.
 void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero);
+// Same, preceded in the same pass by the coarse-grid correction x_in - P e_c with set_bnds_hom (rule T3).
+void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps);
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n);
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse);
 void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,

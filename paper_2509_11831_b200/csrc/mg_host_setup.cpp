@@ -134,13 +134,13 @@ void build_transfer_tables(HostLevel& f, HostLevel& c) {
                 const int32_t q = f.find_tile(2 * (int64_t)c.tI[t] - 1 + b, 2 * (int64_t)c.tJ[t] - 1 + a);
                 c.ctab[(size_t)9 * t + a * 3 + b] = q < 0 ? f.ntiles : q;
             }
-    f.ptab.assign((size_t)4 * f.ntiles, c.ntiles);
+    f.ptab.assign((size_t)9 * f.ntiles, c.ntiles);
     for (int32_t t = 0; t < f.ntiles; t++) {
-        const int64_t pI = floordiv(f.tI[t], 2), pJ = floordiv(f.tJ[t], 2);
-        for (int a = 0; a < 2; a++)
-            for (int b = 0; b < 2; b++) {
+        const int64_t pI = floordiv(f.tI[t], 2), pJ = floordiv(f.tJ[t], 2);   // parent tile
+        for (int a = -1; a <= 1; a++)
+            for (int b = -1; b <= 1; b++) {
                 const int32_t q = c.find_tile(pI + b, pJ + a);
-                f.ptab[(size_t)4 * t + a * 2 + b] = q < 0 ? c.ntiles : q;
+                f.ptab[(size_t)9 * t + (a + 1) * 3 + (b + 1)] = q < 0 ? c.ntiles : q;
             }
     }
 }

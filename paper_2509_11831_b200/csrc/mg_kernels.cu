@@ -51,8 +51,9 @@ __device__ __forceinline__ void neumann_row(uint16_t code, const int* tn, int lx
 
 // ---------------------------------------------------------------------------------- S1 apply / residual
 template <int MODE>
-__global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr) {
+__global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr, const int* __restrict__ stop) {
     __shared__ int tn[9];
+    if (stop != nullptr && *stop) return;
     const int t = blockIdx.x;
     if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
     __syncthreads();
@@ -99,8 +100,9 @@ __device__ __forceinline__ int64_t fine_slot(const int* ct, int fx, int fy) {   
     return (int64_t)ct[cy * 3 + cx] * TS + (fy - (cy - 1) * TY) * TX + (fx - (cx - 1) * TX);
 }
 
-__global__ void __launch_bounds__(NT) k_restrict(LevelDev fine, LevelDev coarse, const double* __restrict__ df, double* __restrict__ dc) {
+__global__ void __launch_bounds__(NT) k_restrict(LevelDev fine, LevelDev coarse, const double* __restrict__ df, double* __restrict__ dc, const int* __restrict__ stop) {
     __shared__ int ct[9];
+    if (stop != nullptr && *stop) return;
     const int t = blockIdx.x;
     if (threadIdx.x < 9) ct[threadIdx.x] = coarse.ctab[9 * t + threadIdx.x];
     __syncthreads();
@@ -155,17 +157,19 @@ __global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev c
 
 
 // ---------------------------------------------------------------------------------- S4 prolongation (rule T3)
-__device__ __forceinline__ int64_t parent_slot(const int* pt, int cx, int cy) {   // cx in [0, TX], cy in [0, TY]
-    const int ox = cx >= TX, oy = cy >= TY;
-    return (int64_t)pt[oy * 2 + ox] * TS + (cy - oy * TY) * TX + (cx - ox * TX);
+__device__ __forceinline__ int64_t parent_slot(const int* pt, int cx, int cy) {   // cx in [-TX, 2TX), cy in [-TY, 2TY)
+    const int ox = (cx < 0) ? -1 : (cx >= TX ? 1 : 0);
+    const int oy = (cy < 0) ? -1 : (cy >= TY ? 1 : 0);
+    return (int64_t)pt[(oy + 1) * 3 + ox + 1] * TS + (cy - oy * TY) * TX + (cx - ox * TX);
 }
 
 // Phase A: e = P e_c on fine inner points (bilinear; absent parents hold 0), 0 elsewhere.
-__global__ void __launch_bounds__(NT) k_prolong(LevelDev fine, const double* __restrict__ ec, double* __restrict__ ef) {
-    __shared__ int pt[4];
+__global__ void __launch_bounds__(NT) k_prolong(LevelDev fine, const double* __restrict__ ec, double* __restrict__ ef, const int* __restrict__ stop) {
+    __shared__ int pt[9];
+    if (stop != nullptr && *stop) return;
     __shared__ int odd[2];
     const int t = blockIdx.x;
-    if (threadIdx.x < 4) pt[threadIdx.x] = fine.ptab[4 * t + threadIdx.x];
+    if (threadIdx.x < 9) pt[threadIdx.x] = fine.ptab[9 * t + threadIdx.x];
     if (threadIdx.x < 2) odd[threadIdx.x] = fine.tij[2 * t + threadIdx.x] & 1;
     __syncthreads();
     const int lx = threadIdx.x % TX;
@@ -189,8 +193,9 @@ __global__ void __launch_bounds__(NT) k_prolong(LevelDev fine, const double* __r
 }
 
 // Phase B: set_bnds_hom on the guards of e (homogeneous Eq. 11 / Eq. 16), then x <- x - e.
-__global__ void __launch_bounds__(NT) k_correct(LevelDev fine, const double* __restrict__ ef, VecRef xr) {
+__global__ void __launch_bounds__(NT) k_correct(LevelDev fine, const double* __restrict__ ef, VecRef xr, const int* __restrict__ stop) {
     __shared__ int tn[9];
+    if (stop != nullptr && *stop) return;
     const int t = blockIdx.x;
     if (threadIdx.x < 9) tn[threadIdx.x] = fine.tnb[9 * t + threadIdx.x];
     __syncthreads();
@@ -229,22 +234,22 @@ inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; 
 }  // namespace
 
 void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRef y, int mode) {
-    if (mode == 0) k_apply<0><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
-    else if (mode == 1) k_apply<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
-    else k_apply<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y);
+    if (mode == 0) k_apply<0><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
+    else if (mode == 1) k_apply<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
+    else k_apply<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
     count(L);
 }
 
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse) {
-    k_restrict<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse, d_fine, d_coarse);
+    k_restrict<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse, d_fine, d_coarse, L.stop);
     count(L);
 }
 
 void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
                             double* e_fine_tmp, VecRef x_fine) {
     (void)coarse;
-    k_prolong<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_coarse, e_fine_tmp);
-    k_correct<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_fine_tmp, x_fine);
+    k_prolong<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_coarse, e_fine_tmp, L.stop);
+    k_correct<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_fine_tmp, x_fine, L.stop);
     count(L, 2);
 }
 

@@ -1,25 +1,43 @@
-// S2: red-black-boundary Gauss-Seidel (gauss_seidel_rbb), NS full sweeps fused into ONE
-// pass over memory.  One CTA per tile loads the tile plus a halo of H = 3*NS cells of x, c and the point
-// codes into shared memory, then runs red / black / boundary phases entirely on-chip, shrinking the valid
-// region by one cell per phase (temporal blocking); halo cells are recomputed redundantly with exactly
-// the arithmetic the owning CTA uses, so the result equals NS sequential sweeps bit for bit.
-// x is double-buffered (x_in -> x_out): a neighbouring CTA may still be reading the old values.
-// HBM traffic per point: x in 8 (0 when x_in is known to be zero) + c 8 + b 8 + lambda 8 + x out 8 + code 2,
-// against 64 B per sweep of the three-loop formulation.
+// S2 (+S4): red-black-boundary Gauss-Seidel (gauss_seidel_rbb), NS full sweeps fused into
+// ONE pass over memory, optionally preceded in the same pass by the coarse-grid correction
+// x <- x - P e_c with set_bnds_hom (rule T3).
+//
+// One CTA per tile loads the tile plus a halo of H cells of x, c and the point codes into shared memory,
+// then runs red / black / boundary phases entirely on-chip; the region in which values are valid shrinks by
+// one cell per phase (temporal blocking), halo cells are recomputed redundantly with exactly the
+// arithmetic the owning CTA uses, so the result does not depend on the tiling.  x is double-buffered
+// (x_in -> x_out): a neighbouring CTA may still be reading the old values.
+//
+// Shared-memory layout is COLOUR-SPLIT: cell (rx, ry) of the region lives at
+// colour * NC + ry * RWC + (rx >> 1), colour = (rx + ry) & 1, so that a warp updating 32 consecutive red
+// cells reads its W/E/S/N black neighbours at unit stride (no bank conflicts, no stride-2 access).
+// Every thread owns a FIXED set of cells (ROUNDS per colour) for the whole kernel: b and 1/a_ll of its
+// inner cells stay in registers across all sweeps, the phase geometry is compile-time, and guard cells
+// are collected once into a compact list, so the colour phases contain no global loads, no integer
+// divisions and no fp64 divisions.
+//
+// HBM traffic per point and launch: x in 8 (0 when x_in is known to be zero) + c 8 + b 8 + lambda 8 +
+// x out 8 + code 2 (+ e_c 2 with the fused correction), against 64 B per sweep of the three-loop
+// formulation.
 #include "mg_device.h"
 
 namespace mgb {
 
 namespace {
 
-constexpr int GT = 512;   // threads per CTA
+constexpr int GT = 512;     // threads per CTA
+constexpr int GCAP = 1024;  // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
-template <int NS>
+template <int NS, bool PC>
 struct Geo {
-    static constexpr int H = 3 * NS;
+    static constexpr int H = 3 * NS + (PC ? 1 : 0);
     static constexpr int RW = TX + 2 * H;
     static constexpr int RH = TY + 2 * H;
-    static constexpr int RN = RW * RH;
+    static constexpr int RWC = RW / 2;              // cells per colour and row
+    static constexpr int NC = RH * RWC;             // cells per colour
+    static constexpr int RN = 2 * NC;
+    static constexpr int ROUNDS = (NC + GT - 1) / GT;
+    static constexpr size_t SMEM = (size_t)RN * (2 * sizeof(double) + sizeof(uint16_t)) + (size_t)GCAP * (sizeof(double) + sizeof(uint16_t));
 };
 
 // global slot of region cell (rx, ry); region origin is (-H, -H) relative to the tile
@@ -31,103 +49,243 @@ __device__ __forceinline__ int64_t region_slot(const int* tn, int rx, int ry) {
     return (int64_t)tn[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + (lx - ox * TX);
 }
 
-template <int NS>
-__global__ void __launch_bounds__(GT) k_gs_fused(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, int xin_zero) {
-    using G = Geo<NS>;
-    constexpr int H = G::H, RW = G::RW, RH = G::RH, RN = G::RN;
+template <class G>
+__device__ __forceinline__ int cidx(int rx, int ry) {
+    return ((rx + ry) & 1) * G::NC + ry * G::RWC + (rx >> 1);
+}
+
+// Rule D3 on the shared-memory region: sum over the non-self stencil nodes of w * v, weight on the point
+// itself, distance delta (h |n|, or h for the fallback).
+template <class G>
+__device__ __forceinline__ void neumann_smem(uint16_t code, int rx, int ry, const double* v, double h, double& sum, double& wself,
+                                             double& delta) {
+    const int tnR = ((code >> 2) & 7) - 2, tnZ = ((code >> 5) & 7) - 2;
+    sum = 0.0; wself = 0.0;
+    if (code & (1 << 8)) {
+        const int mask = (code >> 9) & 15;
+        if (mask & 1) sum += v[cidx<G>(rx - 1, ry)];
+        if (mask & 2) sum += v[cidx<G>(rx + 1, ry)];
+        if (mask & 4) sum += v[cidx<G>(rx, ry - 1)];
+        if (mask & 8) sum += v[cidx<G>(rx, ry + 1)];
+        sum = sum / (double)__popc(mask);
+        delta = h;
+        return;
+    }
+    int ox[2], oy[2], nx, ny; double wx, wy;
+    if (tnR & 1) { nx = 2; ox[0] = 0; ox[1] = tnR; wx = 0.5; } else { nx = 1; ox[0] = tnR / 2; ox[1] = 0; wx = 1.0; }
+    if (tnZ & 1) { ny = 2; oy[0] = 0; oy[1] = tnZ; wy = 0.5; } else { ny = 1; oy[0] = tnZ / 2; oy[1] = 0; wy = 1.0; }
+    const double wgt = wx * wy;
+    for (int bb = 0; bb < ny; bb++)
+        for (int aa = 0; aa < nx; aa++) {
+            if (ox[aa] == 0 && oy[bb] == 0) { wself += wgt; continue; }
+            sum += wgt * v[cidx<G>(rx + ox[aa], ry + oy[bb])];
+        }
+    delta = h * sqrt(0.25 * (double)(tnR * tnR + tnZ * tnZ));
+}
+
+__device__ __forceinline__ int64_t parent_slot9(const int* pt, int cx, int cy) {
+    const int ox = (cx < 0) ? -1 : (cx >= TX ? 1 : 0);
+    const int oy = (cy < 0) ? -1 : (cy >= TY ? 1 : 0);
+    return (int64_t)pt[(oy + 1) * 3 + ox + 1] * TS + (cy - oy * TY) * TX + (cx - ox * TX);
+}
+
+// x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
+template <int NS, bool PC>
+__global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
+                                              int xin_zero, const int* __restrict__ stop) {
+    using G = Geo<NS, PC>;
+    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
+    static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* sx = reinterpret_cast<double*>(smem_raw);
     double* sc = sx + RN;
-    uint16_t* scode = reinterpret_cast<uint16_t*>(sc + RN);
+    double* gb = sc + RN;
+    uint16_t* scode = reinterpret_cast<uint16_t*>(gb + GCAP);
+    uint16_t* glist = scode + RN;
     __shared__ int tn[9];
-    const int t = blockIdx.x;
-    if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
+    __shared__ int pt[9];
+    __shared__ int odd[2];
+    __shared__ int gcount;
+    if (stop != nullptr && *stop) return;
+    const int t = blockIdx.x, tid = threadIdx.x;
+    if (tid < 9) {
+        tn[tid] = lv.tnb[9 * t + tid];
+        if (PC) pt[tid] = lv.ptab[9 * t + tid];
+    }
+    if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
+    if (tid == 0) gcount = 0;
     __syncthreads();
     const double* __restrict__ xin = resolve(xin_r);
     double* __restrict__ xout = resolve(xout_r);
     const double* __restrict__ b = resolve(b_r);
 
-    // ---- stage the region
-    for (int idx = threadIdx.x; idx < RN; idx += GT) {
-        const int ry = idx / RW, rx = idx - ry * RW;
-        const int64_t s = region_slot<H>(tn, rx, ry);
-        sc[idx] = lv.c[s];
-        scode[idx] = lv.code[s];
-        sx[idx] = xin_zero ? 0.0 : xin[s];
-    }
-    __syncthreads();
-
-    const double kappa = lv.kappa;
-#pragma unroll 1
-    for (int sweep = 0; sweep < NS; sweep++) {
-        const int m0 = 3 * sweep;
-        // ---- red (colour 0), then black (colour 1): inner points at distance >= m0 + 1 + colour from the edge
-#pragma unroll 1
-        for (int colour = 0; colour < 2; colour++) {
-            const int m = m0 + 1 + colour;
-            const int w = RW - 2 * m, hgt = RH - 2 * m;
-            const int half = (w + 1) >> 1;
-            for (int idx = threadIdx.x; idx < half * hgt; idx += GT) {
-                const int row = idx / half, k = idx - row * half;
-                const int ry = m + row;
-                const int rx = m + 2 * k + ((m + ry + colour) & 1);     // (rx + ry) parity == colour
-                if (rx >= RW - m) continue;
-                const int p = ry * RW + rx;
-                if ((scode[p] & 3) != C_INNER) continue;
+    if (PC) {
+        // ---- coarse-grid correction on the whole region: e = P e_c on inner cells (bilinear, absent parents
+        // hold 0), homogeneous Eq. 11 / Eq. 16 on guards (set_bnds_hom), x <- x - e.  e is staged in sc.
+#pragma unroll
+        for (int col = 0; col < 2; col++)
+#pragma unroll
+            for (int r = 0; r < ROUNDS; r++) {
+                const int q = tid + r * GT;
+                if (q >= NC) continue;
+                const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
                 const int64_t s = region_slot<H>(tn, rx, ry);
-                const double cl = sc[p];
-                const double aW = kappa * (cl + sc[p - 1]), aE = kappa * (cl + sc[p + 1]);
-                const double aS = kappa * (cl + sc[p - RW]), aN = kappa * (cl + sc[p + RW]);
-                const double all = lv.lam[s] + aW + aE + aS + aN;
-                sx[p] = (b[s] + aW * sx[p - 1] + aE * sx[p + 1] + aS * sx[p - RW] + aN * sx[p + RW]) / all;
+                const uint16_t code = lv.code[s];
+                const int idx = col * NC + q;
+                scode[idx] = code;
+                sx[idx] = xin[s];
+                double e = 0.0;
+                if ((code & 3) == C_INNER) {
+                    const int lx = rx - H, ly = ry - H;
+                    const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
+                    const int ax = lx & 1, ay = ly & 1;
+                    if (!ax && !ay) e = ec[parent_slot9(pt, cx, cy)];
+                    else if (ax && !ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx + 1, cy)];
+                    else if (!ax && ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx, cy + 1)];
+                    else e = 0.25 * ec[parent_slot9(pt, cx, cy)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy)] +
+                             0.25 * ec[parent_slot9(pt, cx, cy + 1)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy + 1)];
+                }
+                sc[idx] = e;
+            }
+        __syncthreads();
+#pragma unroll
+        for (int col = 0; col < 2; col++)
+#pragma unroll
+            for (int r = 0; r < ROUNDS; r++) {
+                const int q = tid + r * GT;
+                if (q >= NC) continue;
+                const int idx = col * NC + q;
+                const uint16_t code = scode[idx];
+                const int kind = code & 3;
+                if (kind == C_INNER) sx[idx] -= sc[idx];
+                else if (kind == C_NEU) {
+                    const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
+                    if (rx >= 1 && rx < RW - 1 && ry >= 1 && ry < RH - 1) {      // edge guards are outside the valid region anyway
+                        double sum, wself, delta;
+                        neumann_smem<G>(code, rx, ry, sc, lv.h, sum, wself, delta);
+                        sx[idx] -= sum / (1.0 - wself);
+                    }
+                }
+            }
+        __syncthreads();
+    }
+
+    // ---- stage c (and x, codes if not done above); b and lambda of the owned inner cells go to registers
+    double breg[2][ROUNDS], rd[2][ROUNDS];
+    unsigned act = 0;      // per (colour, round) nibble: bits 0-1 number of sweeps the cell takes part in, bit 2 row parity term
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            breg[col][r] = 0.0; rd[col][r] = 0.0;
+            const int q = tid + r * GT;
+            if (q >= NC) continue;
+            const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
+            const int64_t s = region_slot<H>(tn, rx, ry);
+            const int idx = col * NC + q;
+            uint16_t code;
+            if (PC) code = scode[idx];
+            else {
+                code = lv.code[s];
+                scode[idx] = code;
+                sx[idx] = xin_zero ? 0.0 : xin[s];
+            }
+            sc[idx] = lv.c[s];
+            const int kind = code & 3;
+            if (kind == C_INNER) {
+                const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
+                const int base = 1 + col + (PC ? 1 : 0);
+                const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
+                if (nsw > 0) { breg[col][r] = b[s]; rd[col][r] = lv.lam[s]; }
+                act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
+            } else if (kind != C_ABSENT) {
+                const int pos = atomicAdd(&gcount, 1);
+                if (pos < GCAP) { glist[pos] = (uint16_t)(ry * RW + rx); gb[pos] = b[s]; }
+            }
+        }
+    __syncthreads();
+    const double kappa = lv.kappa;
+    // 1 / a_ll of the owned inner cells (rule D1: a_ll = lambda + a_W + a_E + a_S + a_N, a_X = kappa (c_l + c_X))
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            const unsigned nib = (act >> (4 * (col * ROUNDS + r))) & 15u;
+            if ((nib & 3u) == 0) continue;
+            const int q = tid + r * GT, tpar = (nib >> 2) & 1;
+            const int own = col * NC + q, ob = (1 - col) * NC + q;
+            const double cl = sc[own];
+            const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
+            const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
+            rd[col][r] = 1.0 / (rd[col][r] + aW + aE + aS + aN);
+        }
+    const int ng = gcount;
+
+#pragma unroll
+    for (int sweep = 0; sweep < NS; sweep++) {
+        // ---- red (colour 0), then black (colour 1)
+#pragma unroll
+        for (int col = 0; col < 2; col++) {
+#pragma unroll
+            for (int r = 0; r < ROUNDS; r++) {
+                const unsigned nib = (act >> (4 * (col * ROUNDS + r))) & 15u;
+                if (sweep < (int)(nib & 3u)) {
+                    const int q = tid + r * GT, tpar = (nib >> 2) & 1;
+                    const int own = col * NC + q, ob = (1 - col) * NC + q;
+                    const double cl = sc[own];
+                    double acc = (cl + sc[ob + tpar - 1]) * sx[ob + tpar - 1];
+                    acc = fma(cl + sc[ob + tpar], sx[ob + tpar], acc);
+                    acc = fma(cl + sc[ob - RWC], sx[ob - RWC], acc);
+                    acc = fma(cl + sc[ob + RWC], sx[ob + RWC], acc);
+                    sx[own] = fma(kappa, acc, breg[col][r]) * rd[col][r];
+                }
             }
             __syncthreads();
         }
-        // ---- boundary points at distance >= m0 + 3 (Eq. 11, Eq. 16 solved for the point)
-        {
-            const int m = m0 + 3;
-            const int w = RW - 2 * m, hgt = RH - 2 * m;
-            for (int idx = threadIdx.x; idx < w * hgt; idx += GT) {
-                const int row = idx / w;
-                const int ry = m + row, rx = m + (idx - row * w);
-                const int p = ry * RW + rx;
-                const uint16_t code = scode[p];
-                const int kind = code & 3;
-                if (kind == C_DIR) {
-                    sx[p] = b[region_slot<H>(tn, rx, ry)];
-                } else if (kind == C_NEU) {
-                    const int tnR = ((code >> 2) & 7) - 2, tnZ = ((code >> 5) & 7) - 2;
-                    double sum = 0.0, wself = 0.0, delta;
-                    if (code & (1 << 8)) {
-                        const int mask = (code >> 9) & 15;
-                        if (mask & 1) sum += sx[p - 1];
-                        if (mask & 2) sum += sx[p + 1];
-                        if (mask & 4) sum += sx[p - RW];
-                        if (mask & 8) sum += sx[p + RW];
-                        sum = sum / (double)__popc(mask);
-                        delta = lv.h;
-                    } else {
-                        int ox[2], oy[2], nx, ny; double wx, wy;
-                        if (tnR & 1) { nx = 2; ox[0] = 0; ox[1] = tnR; wx = 0.5; } else { nx = 1; ox[0] = tnR / 2; ox[1] = 0; wx = 1.0; }
-                        if (tnZ & 1) { ny = 2; oy[0] = 0; oy[1] = tnZ; wy = 0.5; } else { ny = 1; oy[0] = tnZ / 2; oy[1] = 0; wy = 1.0; }
-                        const double wgt = wx * wy;
-                        for (int bb = 0; bb < ny; bb++)
-                            for (int aa = 0; aa < nx; aa++) {
-                                if (ox[aa] == 0 && oy[bb] == 0) { wself += wgt; continue; }
-                                sum += wgt * sx[p + oy[bb] * RW + ox[aa]];
-                            }
-                        delta = lv.h * sqrt(0.25 * (double)(tnR * tnR + tnZ * tnZ));
+        // ---- boundary points (Eq. 11, Eq. 16 solved for the point)
+        if (ng > 0) {
+            const int m = 3 * sweep + 3 + (PC ? 1 : 0);
+            if (ng <= GCAP) {
+                for (int g = tid; g < ng; g += GT) {
+                    const int cell = glist[g];
+                    const int ry = cell / RW, rx = cell - ry * RW;
+                    if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) < m) continue;
+                    const int idx = cidx<G>(rx, ry);
+                    const uint16_t code = scode[idx];
+                    if ((code & 3) == C_DIR) sx[idx] = gb[g];
+                    else {
+                        double sum, wself, delta;
+                        neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
+                        sx[idx] = (sum - delta * gb[g]) / (1.0 - wself);
                     }
-                    sx[p] = (sum - delta * b[region_slot<H>(tn, rx, ry)]) / (1.0 - wself);
                 }
+            } else {                                   // list overflow: every thread scans its own cells
+                for (int col = 0; col < 2; col++)
+                    for (int r = 0; r < ROUNDS; r++) {
+                        const int q = tid + r * GT;
+                        if (q >= NC) continue;
+                        const int idx = col * NC + q;
+                        const uint16_t code = scode[idx];
+                        const int kind = code & 3;
+                        if (kind != C_DIR && kind != C_NEU) continue;
+                        const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
+                        if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) < m) continue;
+                        const double bv = b[region_slot<H>(tn, rx, ry)];
+                        if (kind == C_DIR) sx[idx] = bv;
+                        else {
+                            double sum, wself, delta;
+                            neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
+                            sx[idx] = (sum - delta * bv) / (1.0 - wself);
+                        }
+                    }
             }
             __syncthreads();
         }
     }
     // ---- write the tile back (absent slots carry the zeros they were loaded with)
-    for (int idx = threadIdx.x; idx < TS; idx += GT) {
+    for (int idx = tid; idx < TS; idx += GT) {
         const int ly = idx / TX, lx = idx - ly * TX;
-        xout[(int64_t)t * TS + idx] = sx[(ly + H) * RW + lx + H];
+        xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
     }
 }
 
@@ -137,23 +295,28 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) d[k] = s[k];
 }
 
-template <int NS>
-void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, bool zero) {
-    constexpr size_t smem = (size_t)Geo<NS>::RN * (2 * sizeof(double) + sizeof(uint16_t));
+template <int NS, bool PC>
+void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero) {
+    constexpr size_t smem = Geo<NS, PC>::SMEM;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_gs_fused<NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_gs<NS, PC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = true;
     }
-    k_gs_fused<NS><<<lv.ntiles, GT, smem, L.stream>>>(lv, xin, xout, b, zero ? 1 : 0);
+    k_gs<NS, PC><<<lv.ntiles, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, L.stop);
+    if (L.counter) *L.counter += 1;
 }
 
 }  // namespace
 
 void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero) {
-    if (sweeps == 2) launch_ns<2>(L, lv, x_in, x_out, b, x_in_zero);
-    else launch_ns<1>(L, lv, x_in, x_out, b, x_in_zero);
-    if (L.counter) *L.counter += 1;
+    if (sweeps == 2) launch_ns<2, false>(L, lv, x_in, x_out, b, nullptr, x_in_zero);
+    else launch_ns<1, false>(L, lv, x_in, x_out, b, nullptr, x_in_zero);
+}
+
+void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps) {
+    if (sweeps == 2) launch_ns<2, true>(L, lv, x_in, x_out, b, e_coarse, false);
+    else launch_ns<1, true>(L, lv, x_in, x_out, b, e_coarse, false);
 }
 
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n) {
