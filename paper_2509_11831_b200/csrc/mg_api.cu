@@ -31,8 +31,9 @@ mg_free_fn g_free = nullptr;
 
 struct LevelBuf {           // device arrays owned per level
     uint16_t* code = nullptr;
+    uint8_t* tflag = nullptr;
     int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
-    double *lam = nullptr, *c = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
+    double *lam = nullptr, *c = nullptr, *rd = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
 };
 
 }  // namespace
@@ -251,6 +252,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         LevelBuf& b = h->buf[l];
         TRY(upload(h, &b.code, hl.code, s));
         TRY(upload(h, &b.tnb, hl.tnb, s));
+        TRY(upload(h, &b.tflag, hl.tflag, s));
         TRY(upload(h, &b.ctab, hl.ctab, s));
         TRY(upload(h, &b.ptab, hl.ptab, s));
         std::vector<int32_t> tij(2 * (size_t)hl.ntiles);
@@ -260,6 +262,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         const size_t vb = (size_t)hl.nslots() * sizeof(double);
         TRY(dev_alloc(h, (void**)&b.lam, vb, s));
         TRY(dev_alloc(h, (void**)&b.c, vb, s));
+        TRY(dev_alloc(h, (void**)&b.rd, vb, s));
         TRY(dev_alloc(h, (void**)&b.x, vb, s));
         TRY(dev_alloc(h, (void**)&b.x2, vb, s));
         TRY(dev_alloc(h, (void**)&b.b, vb, s));
@@ -270,7 +273,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         d.ntiles_coarse = l + 1 < h->L ? h->hh.lev[l + 1].ntiles : 0;
         d.nslots = hl.nslots();
         d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
-        d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c;
+        d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c; d.rd = b.rd; d.tflag = b.tflag;
     }
     TRY(upload(h, &h->user2slot, h->hh.user2slot, s));
     const size_t v0 = (size_t)h->lev[0].nslots * sizeof(double);
@@ -312,6 +315,7 @@ int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, voi
     launch_gather(L, d_lambda, h->user2slot, h->buf[0].lam, h->n);
     launch_gather(L, d_c, h->user2slot, h->buf[0].c, h->n);
     for (int l = 0; l + 1 < h->L; l++) launch_restrict_coeff(L, h->lev[l], h->lev[l + 1]);     // rule T4
+    for (int l = 0; l < h->L; l++) launch_diag(L, h->lev[l]);                                   // U2: 1 / a_ll for the smoother
     launch_coarse_factor(L, h->lev[h->L - 1], h->cslot, h->slot2row, h->nL, h->cwork, h->Ainv);   // rule C
     CU(cudaEventRecord(h->ev[3], s));
     CU(cudaGetLastError());

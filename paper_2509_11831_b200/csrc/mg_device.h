@@ -24,8 +24,10 @@ struct LevelDev {
     const int32_t* ctab;     // 9 per tile (this level as the coarse side)
     const int32_t* ptab;     // 9 per tile (this level as the fine side): coarse tiles around the parent tile
     const int32_t* tij;      // 2 per tile: tile coordinates (TI, TJ)
+    const uint8_t* tflag;    // per tile: bit 0 / bit 1 = every cell within 2 / 4 cells of the tile is an inner point
     double* lam;
     double* c;
+    double* rd;              // 1 / a_ll on inner points (rule D1), 0 elsewhere; derived at every update (U2)
 };
 
 // A vector that may be one column of a Krylov basis selected on the device:
@@ -82,6 +84,7 @@ void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coar
 void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
                             double* e_fine_tmp, VecRef x_fine);
 void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse);
+void launch_diag(const Launch& L, const LevelDev& lv);   // U2: rd = 1 / a_ll from lambda, c
 void launch_zero(const Launch& L, VecRef x, int64_t n);
 void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n);   // dst[slot[k]] = src[k]
 void launch_scatter(const Launch& L, const double* src_tiled, const int32_t* slot, double* dst, int64_t n);  // dst[k] = src[slot[k]]

@@ -156,6 +156,30 @@ __global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev c
 }
 
 
+// ---------------------------------------------------------------------------------- U2 diagonal (rule D1)
+// rd = 1 / a_ll, a_ll = lambda + a_W + a_E + a_S + a_N summed in this order; read by the smoother instead
+// of lambda (same traffic, no division in the sweeps).
+__global__ void __launch_bounds__(NT) k_diag(LevelDev lv) {
+    __shared__ int tn[9];
+    const int t = blockIdx.x;
+    if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
+    __syncthreads();
+    const int lx = threadIdx.x % TX;
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        double r = 0.0;
+        if ((lv.code[s] & 3) == C_INNER) {
+            const double cl = lv.c[s];
+            const double aW = lv.kappa * (cl + lv.c[nslot(tn, lx - 1, ly)]), aE = lv.kappa * (cl + lv.c[nslot(tn, lx + 1, ly)]);
+            const double aS = lv.kappa * (cl + lv.c[nslot(tn, lx, ly - 1)]), aN = lv.kappa * (cl + lv.c[nslot(tn, lx, ly + 1)]);
+            r = 1.0 / (lv.lam[s] + aW + aE + aS + aN);
+        }
+        lv.rd[s] = r;
+    }
+}
+
 // ---------------------------------------------------------------------------------- S4 prolongation (rule T3)
 __device__ __forceinline__ int64_t parent_slot(const int* pt, int cx, int cy) {   // cx in [-TX, 2TX), cy in [-TY, 2TY)
     const int ox = (cx < 0) ? -1 : (cx >= TX ? 1 : 0);
@@ -255,6 +279,11 @@ void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDe
 
 void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse) {
     k_restrict_coeff<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse);
+    count(L);
+}
+
+void launch_diag(const Launch& L, const LevelDev& lv) {
+    k_diag<<<lv.ntiles, NT, 0, L.stream>>>(lv);
     count(L);
 }
 

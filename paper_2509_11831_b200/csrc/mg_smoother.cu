@@ -40,6 +40,20 @@ struct Geo {
     static constexpr size_t SMEM = (size_t)RN * (2 * sizeof(double) + sizeof(uint16_t)) + (size_t)GCAP * (sizeof(double) + sizeof(uint16_t));
 };
 
+// Interior tiles (every cell within 2*NS of the tile is an inner point; flagged by the host setup) take a
+// fast path: no guard phase, so the valid region shrinks by 2 instead of 3 cells per sweep (halo 2*NS), and
+// no point codes are needed at all.
+template <int NS>
+struct GeoF {
+    static constexpr int H = 2 * NS;
+    static constexpr int RW = TX + 2 * H;
+    static constexpr int RH = TY + 2 * H;
+    static constexpr int RWC = RW / 2;
+    static constexpr int NC = RH * RWC;
+    static constexpr int RN = 2 * NC;
+    static constexpr int ROUNDS = (NC + GT - 1) / GT;
+};
+
 // global slot of region cell (rx, ry); region origin is (-H, -H) relative to the tile
 template <int H>
 __device__ __forceinline__ int64_t region_slot(const int* tn, int rx, int ry) {
@@ -91,12 +105,12 @@ __device__ __forceinline__ int64_t parent_slot9(const int* pt, int cx, int cy) {
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
 template <int NS, bool PC>
-__global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
-                                              int xin_zero, const int* __restrict__ stop) {
+__device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
+                                           const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
+                                           unsigned char* smem_raw) {
     using G = Geo<NS, PC>;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     double* sx = reinterpret_cast<double*>(smem_raw);
     double* sc = sx + RN;
     double* gb = sc + RN;
@@ -106,8 +120,8 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
     __shared__ int pt[9];
     __shared__ int odd[2];
     __shared__ int gcount;
-    if (stop != nullptr && *stop) return;
-    const int t = blockIdx.x, tid = threadIdx.x;
+    const int tid = threadIdx.x;
+    __syncthreads();                       // shared memory may still be in use by a previous tile of this CTA
     if (tid < 9) {
         tn[tid] = lv.tnb[9 * t + tid];
         if (PC) pt[tid] = lv.ptab[9 * t + tid];
@@ -115,9 +129,6 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
     if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
     if (tid == 0) gcount = 0;
     __syncthreads();
-    const double* __restrict__ xin = resolve(xin_r);
-    double* __restrict__ xout = resolve(xout_r);
-    const double* __restrict__ b = resolve(b_r);
 
     if (PC) {
         // ---- coarse-grid correction on the whole region: e = P e_c on inner cells (bilinear, absent parents
@@ -196,7 +207,7 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
                 const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
                 const int base = 1 + col + (PC ? 1 : 0);
                 const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
-                if (nsw > 0) { breg[col][r] = b[s]; rd[col][r] = lv.lam[s]; }
+                if (nsw > 0) { breg[col][r] = b[s]; rd[col][r] = lv.rd[s]; }
                 act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
             } else if (kind != C_ABSENT) {
                 const int pos = atomicAdd(&gcount, 1);
@@ -205,20 +216,6 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
         }
     __syncthreads();
     const double kappa = lv.kappa;
-    // 1 / a_ll of the owned inner cells (rule D1: a_ll = lambda + a_W + a_E + a_S + a_N, a_X = kappa (c_l + c_X))
-#pragma unroll
-    for (int col = 0; col < 2; col++)
-#pragma unroll
-        for (int r = 0; r < ROUNDS; r++) {
-            const unsigned nib = (act >> (4 * (col * ROUNDS + r))) & 15u;
-            if ((nib & 3u) == 0) continue;
-            const int q = tid + r * GT, tpar = (nib >> 2) & 1;
-            const int own = col * NC + q, ob = (1 - col) * NC + q;
-            const double cl = sc[own];
-            const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
-            const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
-            rd[col][r] = 1.0 / (rd[col][r] + aW + aE + aS + aN);
-        }
     const int ng = gcount;
 
 #pragma unroll
@@ -287,6 +284,105 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
         const int ly = idx / TX, lx = idx - ly * TX;
         xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
     }
+}
+
+// Interior tile: all cells of the region are inner points.
+template <int NS, bool PC>
+__device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
+                                        const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
+                                        unsigned char* smem_raw) {
+    using G = GeoF<NS>;
+    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
+    static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
+    double* sx = reinterpret_cast<double*>(smem_raw);
+    double* sc = sx + RN;
+    __shared__ int tn[9];
+    __shared__ int pt[9];
+    __shared__ int odd[2];
+    const int tid = threadIdx.x;
+    __syncthreads();
+    if (tid < 9) {
+        tn[tid] = lv.tnb[9 * t + tid];
+        if (PC) pt[tid] = lv.ptab[9 * t + tid];
+    }
+    if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
+    __syncthreads();
+    double breg[2][ROUNDS], rd[2][ROUNDS];
+    unsigned act = 0;
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            breg[col][r] = 0.0; rd[col][r] = 0.0;
+            const int q = tid + r * GT;
+            if (q >= NC) continue;
+            const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
+            const int64_t s = region_slot<H>(tn, rx, ry);
+            const int idx = col * NC + q;
+            double x = xin_zero ? 0.0 : xin[s];
+            if (PC) {                                           // x <- x - P e_c (bilinear)
+                const int lx = rx - H, ly = ry - H;
+                const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
+                const int ax = lx & 1, ay = ly & 1;
+                double e;
+                if (!ax && !ay) e = ec[parent_slot9(pt, cx, cy)];
+                else if (ax && !ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx + 1, cy)];
+                else if (!ax && ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx, cy + 1)];
+                else e = 0.25 * ec[parent_slot9(pt, cx, cy)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy)] +
+                         0.25 * ec[parent_slot9(pt, cx, cy + 1)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy + 1)];
+                x -= e;
+            }
+            sx[idx] = x;
+            sc[idx] = lv.c[s];
+            const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
+            const int base = 1 + col;
+            const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
+            if (nsw > 0) { breg[col][r] = b[s]; rd[col][r] = lv.rd[s]; }
+            act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
+        }
+    __syncthreads();
+    const double kappa = lv.kappa;
+#pragma unroll
+    for (int sweep = 0; sweep < NS; sweep++)
+#pragma unroll
+        for (int col = 0; col < 2; col++) {
+#pragma unroll
+            for (int r = 0; r < ROUNDS; r++) {
+                const unsigned nib = (act >> (4 * (col * ROUNDS + r))) & 15u;
+                if (sweep < (int)(nib & 3u)) {
+                    const int q = tid + r * GT, tpar = (nib >> 2) & 1;
+                    const int own = col * NC + q, ob = (1 - col) * NC + q;
+                    const double cl = sc[own];
+                    double acc = (cl + sc[ob + tpar - 1]) * sx[ob + tpar - 1];
+                    acc = fma(cl + sc[ob + tpar], sx[ob + tpar], acc);
+                    acc = fma(cl + sc[ob - RWC], sx[ob - RWC], acc);
+                    acc = fma(cl + sc[ob + RWC], sx[ob + RWC], acc);
+                    sx[own] = fma(kappa, acc, breg[col][r]) * rd[col][r];
+                }
+            }
+            __syncthreads();
+        }
+    for (int idx = tid; idx < TS; idx += GT) {
+        const int ly = idx / TX, lx = idx - ly * TX;
+        xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
+    }
+}
+
+template <int NS, bool PC>
+__device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
+                                        const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
+                                        unsigned char* smem_raw) {
+    if (lv.tflag[t] & (NS == 2 ? 2 : 1)) gs_fast<NS, PC>(lv, t, xin, xout, b, ec, xin_zero, smem_raw);
+    else gs_general<NS, PC>(lv, t, xin, xout, b, ec, xin_zero, smem_raw);
+}
+
+// x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
+template <int NS, bool PC>
+__global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
+                                              int xin_zero, const int* __restrict__ stop) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (stop != nullptr && *stop) return;
+    gs_tile<NS, PC>(lv, blockIdx.x, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw);
 }
 
 __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
