@@ -122,8 +122,7 @@ void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
     if (x_is_zero && h->nu_pre == 0) { launch_zero(L, x, lv.nslots); x_is_zero = false; }
     VecRef cur = enqueue_smooth(L, lv, x, tmp, b, h->nu_pre, x_is_zero);
     VecRef other = (cur.base == x.base) ? tmp : x;
-    launch_apply(L, lv, cur, b, vec(h->buf[s].d), 2);                                     // P:183  d = A x - b
-    launch_restrict(L, lv, h->lev[s + 1], h->buf[s].d, h->buf[s + 1].b);
+    launch_defect_restrict(L, lv, h->lev[s + 1], cur, b, h->buf[s + 1].b);                // P:183-184  R (A x - b)
     enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), true);         // P:186-189, e0 = 0
     VecRef fin;
     if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass

@@ -81,6 +81,8 @@ void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_
 void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps);
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n);
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse);
+// d_coarse = R (A x - b), the defect never stored (rules D4 + T2)
+void launch_defect_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, VecRef x, VecRef b, double* d_coarse);
 void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
                             double* e_fine_tmp, VecRef x_fine);
 void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse);

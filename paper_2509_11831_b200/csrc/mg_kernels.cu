@@ -50,6 +50,28 @@ __device__ __forceinline__ void neumann_row(uint16_t code, const int* tn, int lx
 }
 
 // ---------------------------------------------------------------------------------- S1 apply / residual
+// (A x) at cell (lx, ly) of tile t (slot s), rules D1-D3.  Neighbours inside the tile are s +- 1, s +- TX;
+// only the tile-edge lanes go through the neighbour table.
+// Inner row of rule D1 with every load issued unconditionally (all neighbour slots exist in memory: missing
+// tiles map to the null tile), so that the loads of all cells a thread handles overlap.
+struct Nb4 { int w, e, s, n; };   // ids of the W, E, S, N neighbour tiles, held in registers (branch-free edge handling)
+__device__ __forceinline__ Nb4 nb4(const int* tn) { return Nb4{tn[3], tn[5], tn[1], tn[7]}; }
+
+__device__ __forceinline__ double inner_row(const LevelDev& lv, const Nb4 nb, int lx, int ly, int64_t s, const double* __restrict__ x) {
+    const int64_t eW = (int64_t)nb.w * TS + ly * TX + (TX - 1), eE = (int64_t)nb.e * TS + ly * TX;
+    const int64_t eS = (int64_t)nb.s * TS + (TY - 1) * TX + lx, eN = (int64_t)nb.n * TS + lx;
+    const int64_t sW = (lx > 0) ? s - 1 : eW;
+    const int64_t sE = (lx < TX - 1) ? s + 1 : eE;
+    const int64_t sS = (ly > 0) ? s - TX : eS;
+    const int64_t sN = (ly < TY - 1) ? s + TX : eN;
+    const double cl = __ldg(lv.c + s);
+    const double aW = lv.kappa * (cl + __ldg(lv.c + sW)), aE = lv.kappa * (cl + __ldg(lv.c + sE));
+    const double aS = lv.kappa * (cl + __ldg(lv.c + sS)), aN = lv.kappa * (cl + __ldg(lv.c + sN));
+    const double xl = __ldg(x + s);                                     // difference form (rule D1)
+    return __ldg(lv.lam + s) * xl + aW * (xl - __ldg(x + sW)) + aE * (xl - __ldg(x + sE)) + aS * (xl - __ldg(x + sS)) +
+           aN * (xl - __ldg(x + sN));
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr, const int* __restrict__ stop) {
     __shared__ int tn[9];
@@ -61,32 +83,35 @@ __global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br,
     const double* __restrict__ b = (MODE != 0) ? resolve(br) : nullptr;
     double* __restrict__ y = resolve(yr);
     const int lx = threadIdx.x % TX;
+    constexpr int NP = TY / ROWS_PER_PASS;
+    const Nb4 nb = nb4(tn);
+    uint16_t codes[NP];
+    double ax[NP], bv[NP];
 #pragma unroll
-    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+    for (int p = 0; p < NP; p++) {                          // all loads of the thread's four cells in one batch
         const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
         const int64_t s = (int64_t)t * TS + ly * TX + lx;
-        const uint16_t code = lv.code[s];
-        const int kind = code & 3;
-        double ax = 0.0;
-        if (kind == C_INNER) {                                          // Eq. 10 with 1/h^2 (rule D1)
-            const int64_t sW = nslot(tn, lx - 1, ly), sE = nslot(tn, lx + 1, ly), sS = nslot(tn, lx, ly - 1), sN = nslot(tn, lx, ly + 1);
-            const double cl = lv.c[s];
-            const double aW = lv.kappa * (cl + lv.c[sW]), aE = lv.kappa * (cl + lv.c[sE]);
-            const double aS = lv.kappa * (cl + lv.c[sS]), aN = lv.kappa * (cl + lv.c[sN]);
-            const double xl = x[s];                                     // difference form (rule D1)
-            ax = lv.lam[s] * xl + aW * (xl - x[sW]) + aE * (xl - x[sE]) + aS * (xl - x[sS]) + aN * (xl - x[sN]);
-        } else if (kind == C_DIR) {                                     // Eq. 11
-            ax = x[s];
-        } else if (kind == C_NEU) {                                     // Eq. 16
+        codes[p] = __ldg(lv.code + s);
+        ax[p] = inner_row(lv, nb, lx, ly, s, x);            // Eq. 10 with 1/h^2
+        bv[p] = (MODE != 0) ? __ldg(b + s) : 0.0;
+    }
+#pragma unroll
+    for (int p = 0; p < NP; p++) {
+        const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        const int kind = codes[p] & 3;
+        double v = (kind == C_INNER) ? ax[p] : 0.0;
+        if (kind == C_DIR) v = x[s];                        // Eq. 11
+        else if (kind == C_NEU) {                           // Eq. 16
             double sum, wself, delta;
-            neumann_row(code, tn, lx, ly, x, lv.h, sum, wself, delta);
+            neumann_row(codes[p], tn, lx, ly, x, lv.h, sum, wself, delta);
             const double xl = x[s];
-            ax = (sum + wself * xl - xl) / delta;
+            v = (sum + wself * xl - xl) / delta;
         }
         if (kind == C_ABSENT) y[s] = 0.0;
-        else if (MODE == 0) y[s] = ax;
-        else if (MODE == 1) y[s] = b[s] - ax;
-        else y[s] = ax - b[s];
+        else if (MODE == 0) y[s] = v;
+        else if (MODE == 1) y[s] = bv[p] - v;
+        else y[s] = v - bv[p];
     }
 }
 
@@ -125,6 +150,87 @@ __global__ void __launch_bounds__(NT) k_restrict(LevelDev fine, LevelDev coarse,
         }
         dc[s] = acc;        // coarse guard rows and absent slots: 0
     }
+}
+
+// ---------------------------------------------------------------------------------- S1 + S3 fused
+// d_c = R (A x - b): one CTA per COARSE tile computes the defect of the (2 TX + 1) x (2 TY + 1) fine cells it
+// needs into shared memory (never to HBM), then every coarse inner point gathers its 3 x 3 full-weighting
+// stencil (rule T2: fine non-inner points contribute 0, coarse guard rows are 0).
+constexpr int DRW = 2 * TX + 1, DRH = 2 * TY + 1, DRS = DRW + 1;      // fine x in [-1, 2TX), y in [-1, 2TY); padded row
+constexpr size_t DR_SMEM = (size_t)DRH * DRS * sizeof(double);
+
+__device__ __forceinline__ double defect_cell(const LevelDev& fine, const Nb4 tn, int ft, int lx, int ly, const double* __restrict__ x,
+                                              const double* __restrict__ b) {
+    const int64_t s = (int64_t)ft * TS + ly * TX + lx;
+    const uint16_t code = __ldg(fine.code + s);
+    const double d = inner_row(fine, tn, lx, ly, s, x) - __ldg(b + s);
+    return ((code & 3) == C_INNER) ? d : 0.0;
+}
+
+__device__ __forceinline__ void defect_restrict_tile(const LevelDev& fine, const LevelDev& coarse, int t, const double* __restrict__ x,
+                                                     const double* __restrict__ b, double* __restrict__ dc, unsigned char* smem_raw) {
+    double* sd = reinterpret_cast<double*>(smem_raw);
+    __shared__ int ct[9];
+    __shared__ int ftn[4][9];
+    const int tid = threadIdx.x;
+    __syncthreads();
+    if (tid < 9) ct[tid] = coarse.ctab[9 * t + tid];
+    __syncthreads();
+    if (tid < 36) {
+        const int q = tid / 9, k = tid - 9 * q;
+        const int ft = ct[((q >> 1) + 1) * 3 + (q & 1) + 1];
+        ftn[q][k] = (ft == coarse.ntiles_fine) ? ft : fine.tnb[9 * ft + k];   // the null tile has no table (and is never used)
+    }
+    __syncthreads();
+    const int lx = tid % TX;
+    // the 2 x 2 fine tiles under the coarse tile
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        const int qx = q & 1, qy = q >> 1;
+        const int ft = ct[(qy + 1) * 3 + qx + 1];
+        const Nb4 nbq = nb4(ftn[q]);
+        double dv[TY / ROWS_PER_PASS];
+#pragma unroll
+        for (int p = 0; p < TY / ROWS_PER_PASS; p++) dv[p] = defect_cell(fine, nbq, ft, lx, tid / TX + p * ROWS_PER_PASS, x, b);
+#pragma unroll
+        for (int p = 0; p < TY / ROWS_PER_PASS; p++) sd[(qy * TY + tid / TX + p * ROWS_PER_PASS + 1) * DRS + qx * TX + lx + 1] = dv[p];
+    }
+    // west column (fine x = -1) and south row (fine y = -1): cells of the neighbouring fine tiles
+    if (tid < DRH) {
+        const int fy = tid - 1;
+        const int cy = fy < 0 ? 0 : (fy < TY ? 1 : 2);
+        const int ft = ct[cy * 3 + 0];
+        sd[tid * DRS] = (ft == coarse.ntiles_fine) ? 0.0 : defect_cell(fine, nb4(fine.tnb + 9 * ft), ft, TX - 1, fy - (cy - 1) * TY, x, b);
+    } else if (tid >= 128 && tid < 128 + 2 * TX) {
+        const int fx = tid - 128;
+        const int cx = fx < TX ? 1 : 2;
+        const int ft = ct[cx];
+        sd[fx + 1] = (ft == coarse.ntiles_fine) ? 0.0 : defect_cell(fine, nb4(fine.tnb + 9 * ft), ft, fx - (cx - 1) * TX, TY - 1, x, b);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
+        const int ly = tid / TX + p * ROWS_PER_PASS;
+        const int64_t s = (int64_t)t * TS + ly * TX + lx;
+        double acc = 0.0;
+        if ((coarse.code[s] & 3) == C_INNER) {
+#pragma unroll
+            for (int dy = -1; dy <= 1; dy++)
+#pragma unroll
+                for (int dx = -1; dx <= 1; dx++) {
+                    const double w = (dx == 0 ? 2.0 : 1.0) * (dy == 0 ? 2.0 : 1.0) * 0.0625;
+                    acc += w * sd[(2 * ly + dy + 1) * DRS + 2 * lx + dx + 1];
+                }
+        }
+        dc[s] = acc;
+    }
+}
+
+__global__ void __launch_bounds__(NT) k_defect_restrict(LevelDev fine, LevelDev coarse, VecRef xr, VecRef br, double* __restrict__ dc,
+                                                        const int* __restrict__ stop) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (stop != nullptr && *stop) return;
+    defect_restrict_tile(fine, coarse, blockIdx.x, resolve(xr), resolve(br), dc, smem_raw);
 }
 
 // ---------------------------------------------------------------------------------- U1 coefficient restriction (rule T4)
@@ -266,6 +372,16 @@ void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRe
 
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse) {
     k_restrict<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse, d_fine, d_coarse, L.stop);
+    count(L);
+}
+
+void launch_defect_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, VecRef x, VecRef b, double* d_coarse) {
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_defect_restrict, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DR_SMEM);
+        configured = true;
+    }
+    k_defect_restrict<<<coarse.ntiles, NT, DR_SMEM, L.stream>>>(fine, coarse, x, b, d_coarse, L.stop);
     count(L);
 }
 

@@ -141,20 +141,20 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                 if (q >= NC) continue;
                 const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
                 const int64_t s = region_slot<H>(tn, rx, ry);
-                const uint16_t code = lv.code[s];
+                const uint16_t code = __ldg(lv.code + s);
                 const int idx = col * NC + q;
                 scode[idx] = code;
-                sx[idx] = xin[s];
+                sx[idx] = __ldg(xin + s);
                 double e = 0.0;
                 if ((code & 3) == C_INNER) {
                     const int lx = rx - H, ly = ry - H;
                     const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
                     const int ax = lx & 1, ay = ly & 1;
-                    if (!ax && !ay) e = ec[parent_slot9(pt, cx, cy)];
-                    else if (ax && !ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx + 1, cy)];
-                    else if (!ax && ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx, cy + 1)];
-                    else e = 0.25 * ec[parent_slot9(pt, cx, cy)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy)] +
-                             0.25 * ec[parent_slot9(pt, cx, cy + 1)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy + 1)];
+                    if (!ax && !ay) e = __ldg(ec + parent_slot9(pt, cx, cy));
+                    else if (ax && !ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx + 1, cy));
+                    else if (!ax && ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx, cy + 1));
+                    else e = 0.25 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy)) +
+                             0.25 * __ldg(ec + parent_slot9(pt, cx, cy + 1)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy + 1));
                 }
                 sc[idx] = e;
             }
@@ -197,21 +197,21 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
             uint16_t code;
             if (PC) code = scode[idx];
             else {
-                code = lv.code[s];
+                code = __ldg(lv.code + s);
                 scode[idx] = code;
-                sx[idx] = xin_zero ? 0.0 : xin[s];
+                sx[idx] = xin_zero ? 0.0 : __ldg(xin + s);
             }
-            sc[idx] = lv.c[s];
+            sc[idx] = __ldg(lv.c + s);
             const int kind = code & 3;
             if (kind == C_INNER) {
                 const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
                 const int base = 1 + col + (PC ? 1 : 0);
                 const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
-                if (nsw > 0) { breg[col][r] = b[s]; rd[col][r] = lv.rd[s]; }
+                if (nsw > 0) { breg[col][r] = __ldg(b + s); rd[col][r] = __ldg(lv.rd + s); }
                 act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
             } else if (kind != C_ABSENT) {
                 const int pos = atomicAdd(&gcount, 1);
-                if (pos < GCAP) { glist[pos] = (uint16_t)(ry * RW + rx); gb[pos] = b[s]; }
+                if (pos < GCAP) { glist[pos] = (uint16_t)(ry * RW + rx); gb[pos] = __ldg(b + s); }
             }
         }
     __syncthreads();
@@ -267,7 +267,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                         if (kind != C_DIR && kind != C_NEU) continue;
                         const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
                         if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) < m) continue;
-                        const double bv = b[region_slot<H>(tn, rx, ry)];
+                        const double bv = __ldg(b + region_slot<H>(tn, rx, ry));
                         if (kind == C_DIR) sx[idx] = bv;
                         else {
                             double sum, wself, delta;
@@ -319,25 +319,25 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
             const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
             const int64_t s = region_slot<H>(tn, rx, ry);
             const int idx = col * NC + q;
-            double x = xin_zero ? 0.0 : xin[s];
+            double x = xin_zero ? 0.0 : __ldg(xin + s);
             if (PC) {                                           // x <- x - P e_c (bilinear)
                 const int lx = rx - H, ly = ry - H;
                 const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
                 const int ax = lx & 1, ay = ly & 1;
                 double e;
-                if (!ax && !ay) e = ec[parent_slot9(pt, cx, cy)];
-                else if (ax && !ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx + 1, cy)];
-                else if (!ax && ay) e = 0.5 * ec[parent_slot9(pt, cx, cy)] + 0.5 * ec[parent_slot9(pt, cx, cy + 1)];
-                else e = 0.25 * ec[parent_slot9(pt, cx, cy)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy)] +
-                         0.25 * ec[parent_slot9(pt, cx, cy + 1)] + 0.25 * ec[parent_slot9(pt, cx + 1, cy + 1)];
+                if (!ax && !ay) e = __ldg(ec + parent_slot9(pt, cx, cy));
+                else if (ax && !ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx + 1, cy));
+                else if (!ax && ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx, cy + 1));
+                else e = 0.25 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy)) +
+                         0.25 * __ldg(ec + parent_slot9(pt, cx, cy + 1)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy + 1));
                 x -= e;
             }
             sx[idx] = x;
-            sc[idx] = lv.c[s];
+            sc[idx] = __ldg(lv.c + s);
             const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
             const int base = 1 + col;
             const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
-            if (nsw > 0) { breg[col][r] = b[s]; rd[col][r] = lv.rd[s]; }
+            if (nsw > 0) { breg[col][r] = __ldg(b + s); rd[col][r] = __ldg(lv.rd + s); }
             act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
         }
     __syncthreads();
