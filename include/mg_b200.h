@@ -32,6 +32,7 @@ extern "C" {
 
 typedef struct mg_handle_s* mg_handle;
 #define MG_SETUP_HOST_ONLY 1
+#define MG_SETUP_FUSED_TAIL 2
 
 enum {
     MG_OK = 0,
@@ -70,7 +71,10 @@ typedef struct {
     int max_iters; /* cap on preconditioner applications, default 200                                    */
     int flags;     /* bit 0 (MG_SETUP_HOST_ONLY): build the host hierarchy only, touch no device; only the
                       inspection calls mg_num_levels / mg_level_n / mg_level_info / mg_transfer_info work,
-                      every compute call returns MG_ECUDA.  Other bits must be 0.                        */
+                      every compute call returns MG_ECUDA.
+                      bit 1 (MG_SETUP_FUSED_TAIL): run the cycle steps of the small levels (<= 148 tiles) in one
+                      cooperative kernel instead of one kernel per step (bit-identical results; off by default).
+                      Other bits must be 0.                                                              */
 } mg_options;
 
 /* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).

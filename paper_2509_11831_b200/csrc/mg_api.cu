@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -44,6 +45,9 @@ struct mg_handle_s {
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
     int64_t n = 0;
     std::vector<LevelDev> lev;
+    LevelDev* d_lev = nullptr;            // device copy of lev[] (fused small-level kernel)
+    int tail_s0 = 1 << 30;                // first level handled by the fused small-level kernel
+    int tail_cap = 0;                     // its largest admissible grid
     std::vector<LevelBuf> buf;
     std::vector<void*> allocs;
     int32_t* user2slot = nullptr;
@@ -60,6 +64,7 @@ struct mg_handle_s {
     // host-buffer staging
     double* stage[3] = {nullptr, nullptr, nullptr};
     bool have_coeffs = false;
+    cudaError_t tail_err = cudaSuccess;
     bool host_only = false;
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t iter_graph = nullptr;
@@ -110,10 +115,43 @@ VecRef enqueue_smooth(const Launch& L, const LevelDev& lv, VecRef cur, VecRef ot
     return cur;
 }
 
+// The same schedule as enqueue_cycle below, written as a program for the fused small-level kernel.
+void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailProgram& P) {
+    auto push = [&](TailOp op) { if (P.nops < TAIL_MAX_OPS) P.op[P.nops] = op; P.nops++; };
+    const LevelDev& lv = h->lev[s];
+    if (s == h->L - 1) { TailOp op{}; op.type = TAIL_COARSE; op.level = (unsigned char)s; op.ntiles = 1; op.a = b; op.b = x; push(op); return; }
+    double *cur = x, *other = h->buf[s].x2;
+    auto gs = [&](int k, bool pc, bool zero, const double* ec) {
+        TailOp op{}; op.type = TAIL_GS; op.level = (unsigned char)s; op.ns = (unsigned char)k; op.pc = pc; op.zero = zero;
+        op.ntiles = lv.ntiles; op.a = cur; op.b = other; op.c = b; op.ec = ec; push(op);
+        std::swap(cur, other);
+    };
+    for (int nu = h->nu_pre; nu > 0;) { const int k = nu >= 2 ? 2 : 1; gs(k, false, x_is_zero, nullptr); x_is_zero = false; nu -= k; }
+    { TailOp op{}; op.type = TAIL_DR; op.level = (unsigned char)s; op.ntiles = h->lev[s + 1].ntiles; op.a = cur; op.b = h->buf[s + 1].b; op.c = b; push(op); }
+    build_tail(h, s + 1, h->buf[s + 1].x, h->buf[s + 1].b, true, P);
+    int nu = h->nu_post;
+    { const int k = nu >= 2 ? 2 : 1; gs(k, true, false, h->buf[s + 1].x); nu -= k; }
+    while (nu > 0) { const int k = nu >= 2 ? 2 : 1; gs(k, false, false, nullptr); nu -= k; }
+    if (cur != x) { TailOp op{}; op.type = TAIL_COPY; op.level = (unsigned char)s; op.a = cur; op.b = x; op.n = lv.nslots; push(op); }
+}
+
 // mg_cycle of PAPER.md:171-195 with gamma = 1, enqueued on L.stream.  x_is_zero: the initial guess is
 // the zero vector and x need not be read (nor zeroed beforehand).
 void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero) {
     const LevelDev& lv = h->lev[s];
+    if (s >= h->tail_s0) {                                            // small levels: one cooperative kernel
+        TailProgram P; P.nops = 0;
+        build_tail(h, s, TAIL_TOPX, TAIL_TOPB, x_is_zero, P);
+        if (P.nops <= TAIL_MAX_OPS) {
+            int grid = 1;
+            for (int i = 0; i < P.nops; i++) grid = std::max(grid, P.op[i].type == TAIL_COPY ? 8 : P.op[i].ntiles);
+            TailCoarse cs{h->Ainv, h->cslot, h->nL};
+            if (grid <= h->tail_cap && h->L - s <= TAIL_MAX_LEVELS) {
+                h->tail_err = launch_tail(L, h->d_lev, s, h->L, P, cs, x, b, grid);
+                return;
+            }
+        }
+    }
     if (s == h->L - 1) {                                              // P:173-177 direct solve
         launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, b, x);
         return;
@@ -164,6 +202,7 @@ int build_iter_graph(mg_handle h) {
     L.stop = &h->st->cycle_end;          // iterations are enqueued one ahead of the convergence test
     enqueue_iteration(h, L);
     CU(cudaStreamEndCapture(h->cap_stream, &g));
+    CU(h->tail_err);
     h->iter_graph_kernels = h->launches - before;
     h->launches = before;
     CU(cudaGraphInstantiate(&h->iter_graph, g, 0));
@@ -219,7 +258,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || (o.flags & ~1) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || (o.flags & ~3) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
@@ -274,6 +313,11 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
         d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c; d.rd = b.rd; d.tflag = b.tflag;
     }
+    TRY(dev_alloc(h, (void**)&h->d_lev, sizeof(LevelDev) * h->L, s));
+    CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
+    h->tail_cap = std::min(tail_max_grid(), 2 * 148);
+    if (h->tail_cap > 0 && h->nu_pre >= 1 && h->nu_post >= 1 && ((o.flags & MG_SETUP_FUSED_TAIL) || getenv("MG_B200_FUSED_TAIL")))
+        for (int l = h->L - 1; l >= 0 && h->lev[l].ntiles <= h->tail_cap; l--) h->tail_s0 = l;
     TRY(upload(h, &h->user2slot, h->hh.user2slot, s));
     const size_t v0 = (size_t)h->lev[0].nslots * sizeof(double);
     TRY(dev_alloc(h, (void**)&h->V, v0 * (h->m + 1), s));
@@ -592,6 +636,7 @@ int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stre
     launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
     launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
     enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].b), false);
+    CU(h->tail_err);
     launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
     CU(cudaGetLastError());
     return MG_OK;

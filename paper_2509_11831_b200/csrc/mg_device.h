@@ -91,6 +91,40 @@ void launch_zero(const Launch& L, VecRef x, int64_t n);
 void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n);   // dst[slot[k]] = src[k]
 void launch_scatter(const Launch& L, const double* src_tiled, const int32_t* slot, double* dst, int64_t n);  // dst[k] = src[slot[k]]
 
+// ---- fused small levels (mg_tail.cu): the cycle steps of all levels >= s0 as a program run by one
+// cooperative kernel, grid.sync() between steps
+// per (level, tile) tables a CTA of the fused kernel preloads once: ints
+//   [META_TN..+9) neighbour tiles, [META_PT..+9) coarse parent tiles, [META_ODD..+2) tile parity, [META_FLAG] interior flags,
+//   this tile as the COARSE side of a defect restriction: [META_CT..+9) fine tiles, [META_FTN..+36) neighbour tables
+//   of the 2 x 2 fine tiles, [META_RING..+20) W,E,S,N neighbours of the SW, W, W', S, S' ring tiles
+enum { META_TN = 0, META_PT = 9, META_ODD = 18, META_FLAG = 20, META_CT = 21, META_FTN = 30, META_RING = 66, META_INTS = 88 };
+constexpr int TAIL_MAX_LEVELS = 16;
+enum { TAIL_GS = 0, TAIL_DR = 1, TAIL_COARSE = 2, TAIL_COPY = 3 };
+#define TAIL_TOPX (reinterpret_cast<double*>(1))   // placeholder: the cycle's x vector (a VecRef resolved on the device)
+#define TAIL_TOPB (reinterpret_cast<double*>(2))   // placeholder: the cycle's right-hand side
+struct TailOp {
+    unsigned char type, level, ns, pc;   // level: the (fine) level the step works on
+    int zero;                            // GS: x_in is the zero vector
+    int ntiles;                          // tiles the step loops over
+    double *a, *b, *c;                   // GS: x_in, x_out, rhs; DR: x, coarse defect out, rhs; COARSE: rhs, x; COPY: src, dst
+    const double* ec;                    // GS with correction: coarse-level solution
+    int64_t n;                           // COPY: length
+};
+constexpr int TAIL_MAX_OPS = 64;
+struct TailProgram {
+    int nops;
+    TailOp op[TAIL_MAX_OPS];
+};
+struct TailCoarse {
+    const double* Ainv;
+    const int32_t* cslot;
+    int n;
+};
+int tail_max_grid();   // largest co-resident grid of the fused kernel (0: cooperative launch unavailable)
+// levels s0 .. nlev-1 take part; grid must be >= the tile count of every step (one tile per CTA)
+cudaError_t launch_tail(const Launch& L, const LevelDev* d_levs, int s0, int nlev, const TailProgram& prog, const TailCoarse& cs,
+                        VecRef topx, VecRef topb, int grid);
+
 // ---- coarsest level (mg_coarse.cu) ----
 void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
                           double* work /* n x 2n */, double* Ainv /* n x n */);

@@ -1,380 +1,10 @@
-// S2 (+S4): red-black-boundary Gauss-Seidel (gauss_seidel_rbb), NS full sweeps fused into
-// ONE pass over memory, optionally preceded in the same pass by the coarse-grid correction
-// x <- x - P e_c with set_bnds_hom (rule T3).
-//
-// One CTA per tile loads the tile plus a halo of H cells of x, c and the point codes into shared memory,
-// then runs red / black / boundary phases entirely on-chip; the region in which values are valid shrinks by
-// one cell per phase (temporal blocking), halo cells are recomputed redundantly with exactly the
-// arithmetic the owning CTA uses, so the result does not depend on the tiling.  x is double-buffered
-// (x_in -> x_out): a neighbouring CTA may still be reading the old values.
-//
-// Shared-memory layout is COLOUR-SPLIT: cell (rx, ry) of the region lives at
-// colour * NC + ry * RWC + (rx >> 1), colour = (rx + ry) & 1, so that a warp updating 32 consecutive red
-// cells reads its W/E/S/N black neighbours at unit stride (no bank conflicts, no stride-2 access).
-// Every thread owns a FIXED set of cells (ROUNDS per colour) for the whole kernel: b and 1/a_ll of its
-// inner cells stay in registers across all sweeps, the phase geometry is compile-time, and guard cells
-// are collected once into a compact list, so the colour phases contain no global loads, no integer
-// divisions and no fp64 divisions.
-//
-// HBM traffic per point and launch: x in 8 (0 when x_in is known to be zero) + c 8 + b 8 + lambda 8 +
-// x out 8 + code 2 (+ e_c 2 with the fused correction), against 64 B per sweep of the three-loop
-// formulation.
-#include "mg_device.h"
+// Kernels and launchers of the smoother; the tile-level device code is in mg_tile_gs.cuh (shared with the
+// fused small-level kernel of mg_tail.cu).
+#include "mg_tile_gs.cuh"
 
 namespace mgb {
 
 namespace {
-
-constexpr int GT = 512;     // threads per CTA
-constexpr int GCAP = 1024;  // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
-
-template <int NS, bool PC>
-struct Geo {
-    static constexpr int H = 3 * NS + (PC ? 1 : 0);
-    static constexpr int RW = TX + 2 * H;
-    static constexpr int RH = TY + 2 * H;
-    static constexpr int RWC = RW / 2;              // cells per colour and row
-    static constexpr int NC = RH * RWC;             // cells per colour
-    static constexpr int RN = 2 * NC;
-    static constexpr int ROUNDS = (NC + GT - 1) / GT;
-    static constexpr size_t SMEM = (size_t)RN * (2 * sizeof(double) + sizeof(uint16_t)) + (size_t)GCAP * (sizeof(double) + sizeof(uint16_t));
-};
-
-// Interior tiles (every cell within 2*NS of the tile is an inner point; flagged by the host setup) take a
-// fast path: no guard phase, so the valid region shrinks by 2 instead of 3 cells per sweep (halo 2*NS), and
-// no point codes are needed at all.
-template <int NS>
-struct GeoF {
-    static constexpr int H = 2 * NS;
-    static constexpr int RW = TX + 2 * H;
-    static constexpr int RH = TY + 2 * H;
-    static constexpr int RWC = RW / 2;
-    static constexpr int NC = RH * RWC;
-    static constexpr int RN = 2 * NC;
-    static constexpr int ROUNDS = (NC + GT - 1) / GT;
-};
-
-// global slot of region cell (rx, ry); region origin is (-H, -H) relative to the tile
-template <int H>
-__device__ __forceinline__ int64_t region_slot(const int* tn, int rx, int ry) {
-    const int lx = rx - H, ly = ry - H;
-    const int ox = (lx < 0) ? -1 : (lx >= TX ? 1 : 0);
-    const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
-    return (int64_t)tn[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + (lx - ox * TX);
-}
-
-template <class G>
-__device__ __forceinline__ int cidx(int rx, int ry) {
-    return ((rx + ry) & 1) * G::NC + ry * G::RWC + (rx >> 1);
-}
-
-// Rule D3 on the shared-memory region: sum over the non-self stencil nodes of w * v, weight on the point
-// itself, distance delta (h |n|, or h for the fallback).
-template <class G>
-__device__ __forceinline__ void neumann_smem(uint16_t code, int rx, int ry, const double* v, double h, double& sum, double& wself,
-                                             double& delta) {
-    const int tnR = ((code >> 2) & 7) - 2, tnZ = ((code >> 5) & 7) - 2;
-    sum = 0.0; wself = 0.0;
-    if (code & (1 << 8)) {
-        const int mask = (code >> 9) & 15;
-        if (mask & 1) sum += v[cidx<G>(rx - 1, ry)];
-        if (mask & 2) sum += v[cidx<G>(rx + 1, ry)];
-        if (mask & 4) sum += v[cidx<G>(rx, ry - 1)];
-        if (mask & 8) sum += v[cidx<G>(rx, ry + 1)];
-        sum = sum / (double)__popc(mask);
-        delta = h;
-        return;
-    }
-    int ox[2], oy[2], nx, ny; double wx, wy;
-    if (tnR & 1) { nx = 2; ox[0] = 0; ox[1] = tnR; wx = 0.5; } else { nx = 1; ox[0] = tnR / 2; ox[1] = 0; wx = 1.0; }
-    if (tnZ & 1) { ny = 2; oy[0] = 0; oy[1] = tnZ; wy = 0.5; } else { ny = 1; oy[0] = tnZ / 2; oy[1] = 0; wy = 1.0; }
-    const double wgt = wx * wy;
-    for (int bb = 0; bb < ny; bb++)
-        for (int aa = 0; aa < nx; aa++) {
-            if (ox[aa] == 0 && oy[bb] == 0) { wself += wgt; continue; }
-            sum += wgt * v[cidx<G>(rx + ox[aa], ry + oy[bb])];
-        }
-    delta = h * sqrt(0.25 * (double)(tnR * tnR + tnZ * tnZ));
-}
-
-__device__ __forceinline__ int64_t parent_slot9(const int* pt, int cx, int cy) {
-    const int ox = (cx < 0) ? -1 : (cx >= TX ? 1 : 0);
-    const int oy = (cy < 0) ? -1 : (cy >= TY ? 1 : 0);
-    return (int64_t)pt[(oy + 1) * 3 + ox + 1] * TS + (cy - oy * TY) * TX + (cx - ox * TX);
-}
-
-// x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-template <int NS, bool PC>
-__device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
-                                           const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
-                                           unsigned char* smem_raw) {
-    using G = Geo<NS, PC>;
-    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
-    static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
-    double* sx = reinterpret_cast<double*>(smem_raw);
-    double* sc = sx + RN;
-    double* gb = sc + RN;
-    uint16_t* scode = reinterpret_cast<uint16_t*>(gb + GCAP);
-    uint16_t* glist = scode + RN;
-    __shared__ int tn[9];
-    __shared__ int pt[9];
-    __shared__ int odd[2];
-    __shared__ int gcount;
-    const int tid = threadIdx.x;
-    __syncthreads();                       // shared memory may still be in use by a previous tile of this CTA
-    if (tid < 9) {
-        tn[tid] = lv.tnb[9 * t + tid];
-        if (PC) pt[tid] = lv.ptab[9 * t + tid];
-    }
-    if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
-    if (tid == 0) gcount = 0;
-    __syncthreads();
-
-    if (PC) {
-        // ---- coarse-grid correction on the whole region: e = P e_c on inner cells (bilinear, absent parents
-        // hold 0), homogeneous Eq. 11 / Eq. 16 on guards (set_bnds_hom), x <- x - e.  e is staged in sc.
-#pragma unroll
-        for (int col = 0; col < 2; col++)
-#pragma unroll
-            for (int r = 0; r < ROUNDS; r++) {
-                const int q = tid + r * GT;
-                if (q >= NC) continue;
-                const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
-                const int64_t s = region_slot<H>(tn, rx, ry);
-                const uint16_t code = __ldg(lv.code + s);
-                const int idx = col * NC + q;
-                scode[idx] = code;
-                sx[idx] = __ldg(xin + s);
-                double e = 0.0;
-                if ((code & 3) == C_INNER) {
-                    const int lx = rx - H, ly = ry - H;
-                    const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
-                    const int ax = lx & 1, ay = ly & 1;
-                    if (!ax && !ay) e = __ldg(ec + parent_slot9(pt, cx, cy));
-                    else if (ax && !ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx + 1, cy));
-                    else if (!ax && ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx, cy + 1));
-                    else e = 0.25 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy)) +
-                             0.25 * __ldg(ec + parent_slot9(pt, cx, cy + 1)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy + 1));
-                }
-                sc[idx] = e;
-            }
-        __syncthreads();
-#pragma unroll
-        for (int col = 0; col < 2; col++)
-#pragma unroll
-            for (int r = 0; r < ROUNDS; r++) {
-                const int q = tid + r * GT;
-                if (q >= NC) continue;
-                const int idx = col * NC + q;
-                const uint16_t code = scode[idx];
-                const int kind = code & 3;
-                if (kind == C_INNER) sx[idx] -= sc[idx];
-                else if (kind == C_NEU) {
-                    const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
-                    if (rx >= 1 && rx < RW - 1 && ry >= 1 && ry < RH - 1) {      // edge guards are outside the valid region anyway
-                        double sum, wself, delta;
-                        neumann_smem<G>(code, rx, ry, sc, lv.h, sum, wself, delta);
-                        sx[idx] -= sum / (1.0 - wself);
-                    }
-                }
-            }
-        __syncthreads();
-    }
-
-    // ---- stage c (and x, codes if not done above); b and lambda of the owned inner cells go to registers
-    double breg[2][ROUNDS], rd[2][ROUNDS];
-    unsigned act = 0;      // per (colour, round) nibble: bits 0-1 number of sweeps the cell takes part in, bit 2 row parity term
-#pragma unroll
-    for (int col = 0; col < 2; col++)
-#pragma unroll
-        for (int r = 0; r < ROUNDS; r++) {
-            breg[col][r] = 0.0; rd[col][r] = 0.0;
-            const int q = tid + r * GT;
-            if (q >= NC) continue;
-            const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
-            const int64_t s = region_slot<H>(tn, rx, ry);
-            const int idx = col * NC + q;
-            uint16_t code;
-            if (PC) code = scode[idx];
-            else {
-                code = __ldg(lv.code + s);
-                scode[idx] = code;
-                sx[idx] = xin_zero ? 0.0 : __ldg(xin + s);
-            }
-            sc[idx] = __ldg(lv.c + s);
-            const int kind = code & 3;
-            if (kind == C_INNER) {
-                const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
-                const int base = 1 + col + (PC ? 1 : 0);
-                const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
-                if (nsw > 0) { breg[col][r] = __ldg(b + s); rd[col][r] = __ldg(lv.rd + s); }
-                act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
-            } else if (kind != C_ABSENT) {
-                const int pos = atomicAdd(&gcount, 1);
-                if (pos < GCAP) { glist[pos] = (uint16_t)(ry * RW + rx); gb[pos] = __ldg(b + s); }
-            }
-        }
-    __syncthreads();
-    const double kappa = lv.kappa;
-    const int ng = gcount;
-
-#pragma unroll
-    for (int sweep = 0; sweep < NS; sweep++) {
-        // ---- red (colour 0), then black (colour 1)
-#pragma unroll
-        for (int col = 0; col < 2; col++) {
-#pragma unroll
-            for (int r = 0; r < ROUNDS; r++) {
-                const unsigned nib = (act >> (4 * (col * ROUNDS + r))) & 15u;
-                if (sweep < (int)(nib & 3u)) {
-                    const int q = tid + r * GT, tpar = (nib >> 2) & 1;
-                    const int own = col * NC + q, ob = (1 - col) * NC + q;
-                    const double cl = sc[own];
-                    double acc = (cl + sc[ob + tpar - 1]) * sx[ob + tpar - 1];
-                    acc = fma(cl + sc[ob + tpar], sx[ob + tpar], acc);
-                    acc = fma(cl + sc[ob - RWC], sx[ob - RWC], acc);
-                    acc = fma(cl + sc[ob + RWC], sx[ob + RWC], acc);
-                    sx[own] = fma(kappa, acc, breg[col][r]) * rd[col][r];
-                }
-            }
-            __syncthreads();
-        }
-        // ---- boundary points (Eq. 11, Eq. 16 solved for the point)
-        if (ng > 0) {
-            const int m = 3 * sweep + 3 + (PC ? 1 : 0);
-            if (ng <= GCAP) {
-                for (int g = tid; g < ng; g += GT) {
-                    const int cell = glist[g];
-                    const int ry = cell / RW, rx = cell - ry * RW;
-                    if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) < m) continue;
-                    const int idx = cidx<G>(rx, ry);
-                    const uint16_t code = scode[idx];
-                    if ((code & 3) == C_DIR) sx[idx] = gb[g];
-                    else {
-                        double sum, wself, delta;
-                        neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
-                        sx[idx] = (sum - delta * gb[g]) / (1.0 - wself);
-                    }
-                }
-            } else {                                   // list overflow: every thread scans its own cells
-                for (int col = 0; col < 2; col++)
-                    for (int r = 0; r < ROUNDS; r++) {
-                        const int q = tid + r * GT;
-                        if (q >= NC) continue;
-                        const int idx = col * NC + q;
-                        const uint16_t code = scode[idx];
-                        const int kind = code & 3;
-                        if (kind != C_DIR && kind != C_NEU) continue;
-                        const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
-                        if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) < m) continue;
-                        const double bv = __ldg(b + region_slot<H>(tn, rx, ry));
-                        if (kind == C_DIR) sx[idx] = bv;
-                        else {
-                            double sum, wself, delta;
-                            neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
-                            sx[idx] = (sum - delta * bv) / (1.0 - wself);
-                        }
-                    }
-            }
-            __syncthreads();
-        }
-    }
-    // ---- write the tile back (absent slots carry the zeros they were loaded with)
-    for (int idx = tid; idx < TS; idx += GT) {
-        const int ly = idx / TX, lx = idx - ly * TX;
-        xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
-    }
-}
-
-// Interior tile: all cells of the region are inner points.
-template <int NS, bool PC>
-__device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
-                                        const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
-                                        unsigned char* smem_raw) {
-    using G = GeoF<NS>;
-    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
-    static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
-    double* sx = reinterpret_cast<double*>(smem_raw);
-    double* sc = sx + RN;
-    __shared__ int tn[9];
-    __shared__ int pt[9];
-    __shared__ int odd[2];
-    const int tid = threadIdx.x;
-    __syncthreads();
-    if (tid < 9) {
-        tn[tid] = lv.tnb[9 * t + tid];
-        if (PC) pt[tid] = lv.ptab[9 * t + tid];
-    }
-    if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
-    __syncthreads();
-    double breg[2][ROUNDS], rd[2][ROUNDS];
-    unsigned act = 0;
-#pragma unroll
-    for (int col = 0; col < 2; col++)
-#pragma unroll
-        for (int r = 0; r < ROUNDS; r++) {
-            breg[col][r] = 0.0; rd[col][r] = 0.0;
-            const int q = tid + r * GT;
-            if (q >= NC) continue;
-            const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
-            const int64_t s = region_slot<H>(tn, rx, ry);
-            const int idx = col * NC + q;
-            double x = xin_zero ? 0.0 : __ldg(xin + s);
-            if (PC) {                                           // x <- x - P e_c (bilinear)
-                const int lx = rx - H, ly = ry - H;
-                const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
-                const int ax = lx & 1, ay = ly & 1;
-                double e;
-                if (!ax && !ay) e = __ldg(ec + parent_slot9(pt, cx, cy));
-                else if (ax && !ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx + 1, cy));
-                else if (!ax && ay) e = 0.5 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.5 * __ldg(ec + parent_slot9(pt, cx, cy + 1));
-                else e = 0.25 * __ldg(ec + parent_slot9(pt, cx, cy)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy)) +
-                         0.25 * __ldg(ec + parent_slot9(pt, cx, cy + 1)) + 0.25 * __ldg(ec + parent_slot9(pt, cx + 1, cy + 1));
-                x -= e;
-            }
-            sx[idx] = x;
-            sc[idx] = __ldg(lv.c + s);
-            const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
-            const int base = 1 + col;
-            const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
-            if (nsw > 0) { breg[col][r] = __ldg(b + s); rd[col][r] = __ldg(lv.rd + s); }
-            act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
-        }
-    __syncthreads();
-    const double kappa = lv.kappa;
-#pragma unroll
-    for (int sweep = 0; sweep < NS; sweep++)
-#pragma unroll
-        for (int col = 0; col < 2; col++) {
-#pragma unroll
-            for (int r = 0; r < ROUNDS; r++) {
-                const unsigned nib = (act >> (4 * (col * ROUNDS + r))) & 15u;
-                if (sweep < (int)(nib & 3u)) {
-                    const int q = tid + r * GT, tpar = (nib >> 2) & 1;
-                    const int own = col * NC + q, ob = (1 - col) * NC + q;
-                    const double cl = sc[own];
-                    double acc = (cl + sc[ob + tpar - 1]) * sx[ob + tpar - 1];
-                    acc = fma(cl + sc[ob + tpar], sx[ob + tpar], acc);
-                    acc = fma(cl + sc[ob - RWC], sx[ob - RWC], acc);
-                    acc = fma(cl + sc[ob + RWC], sx[ob + RWC], acc);
-                    sx[own] = fma(kappa, acc, breg[col][r]) * rd[col][r];
-                }
-            }
-            __syncthreads();
-        }
-    for (int idx = tid; idx < TS; idx += GT) {
-        const int ly = idx / TX, lx = idx - ly * TX;
-        xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
-    }
-}
-
-template <int NS, bool PC>
-__device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
-                                        const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
-                                        unsigned char* smem_raw) {
-    if (lv.tflag[t] & (NS == 2 ? 2 : 1)) gs_fast<NS, PC>(lv, t, xin, xout, b, ec, xin_zero, smem_raw);
-    else gs_general<NS, PC>(lv, t, xin, xout, b, ec, xin_zero, smem_raw);
-}
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
 template <int NS, bool PC>
@@ -382,7 +12,7 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
                                               int xin_zero, const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (stop != nullptr && *stop) return;
-    gs_tile<NS, PC>(lv, blockIdx.x, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw);
+    gs_tile<NS, PC, false>(lv, blockIdx.x, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw);
 }
 
 __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
