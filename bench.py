@@ -38,6 +38,9 @@ WORKLOADS = {
 }
 # algorithmic bytes per point (SURVEY.md 8(d) / DESIGN.md section 6): one full RB-B GS sweep
 GS_BYTES_PER_POINT = 64.0
+# DRAM bytes per launch of the roofline kernel (dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full
+# capture per config; profiles/r01d_gs_config4.md)
+GS_TRAFFIC_PER_LAUNCH = {4: 456.7e6}
 
 
 def peaks():
@@ -129,6 +132,39 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def plane_seed(cfg, rank):
+    """Every rank owns its own plane of the same geometry (planes are independent solves)."""
+    return W.SEEDS[cfg] + 7919 * rank
+
+
+def whole_job(ms_local, unknown_iters_local, world, device):
+    """Max-over-ranks time and summed work: value = all units processed by all ranks / slowest rank's time.
+    No data-path collective exists; these two reductions are the only communication of the bench."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    w = torch.tensor([unknown_iters_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(w, op=dist.ReduceOp.SUM)
+    ms, work = float(t.item()), float(w.item())
+    return ms, work, work / (ms * 1e-3)
+
+
+def make_steps(cfg, rank, nsteps):
+    """Inputs of `nsteps` consecutive steps.  Configs 1-4: the same plane every step (x0 = 0).
+    Config 5: the time-stepping sequence of BASELINE.json configs[4] (coefficients and right-hand side
+    perturbed every step, warm start from the previous solution)."""
+    pl = W.make_plane(cfg, seed=plane_seed(cfg, rank))
+    if cfg != 5:
+        return pl, [pl] * nsteps, False
+    seq, cur = [pl], pl
+    for k in range(nsteps - 1):
+        cur = W.next_step(cur, k)
+        seq.append(cur)
+    return pl, seq, True
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -144,15 +180,16 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.use_torch_allocator()
 
-    # every rank owns one plane of the same geometry with its own seed (planes are independent)
-    pl = W.make_plane(args.config, seed=W.SEEDS[args.config] + 7919 * rank)
+    nsteps = args.warmup + args.steps
+    pl, seq, warm = make_steps(args.config, rank, nsteps)
+    uniq = seq if warm else seq[:1]
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
-    d_lam, d_c, d_f, d_x0 = dev(pl.lam), dev(pl.c), dev(pl.f), dev(pl.x0)
-    d_x = torch.empty_like(d_f)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
-    h_lam, h_c, h_f, h_x0 = pin(pl.lam), pin(pl.c), pin(pl.f), pin(pl.x0)
-    h_x = torch.empty(pl.n, dtype=torch.float64).pin_memory().numpy()
+    d_in = [(dev(q.lam), dev(q.c), dev(q.f)) for q in uniq]          # resident in HBM before the timed region
+    h_in = [(pin(q.lam).numpy(), pin(q.c).numpy(), pin(q.f).numpy()) for q in uniq]
+    d_x0, d_x = dev(pl.x0), torch.empty(pl.n, dtype=torch.float64, device="cuda")
+    h_x0, h_x = pin(pl.x0).numpy(), torch.empty(pl.n, dtype=torch.float64).pin_memory().numpy()
 
     def barrier():
         torch.cuda.synchronize()
@@ -160,49 +197,54 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step_device():
-        s.update_coeffs(d_lam, d_c)
-        _, iters, relres, rc = s.solve(d_f, d_x0, RTOL, x=d_x)
+    def step_device(k):
+        lam, c, f = d_in[k if warm else 0]
+        s.update_coeffs(lam, c)
+        _, iters, relres, rc = s.solve(f, d_x if (warm and k > 0) else d_x0, RTOL, x=d_x)   # d_x may alias d_x0
         return iters, relres, rc
 
-    def step_host():
-        s.update_coeffs_host(h_lam, h_c)
-        _, iters, relres, rc = s.solve_host(h_f, h_x0, RTOL, x=h_x)
+    def step_host(k):
+        lam, c, f = h_in[k if warm else 0]
+        s.update_coeffs_host(lam, c)
+        _, iters, relres, rc = s.solve_host(f, h_x if (warm and k > 0) else h_x0, RTOL, x=h_x)
         return iters, relres, rc
 
-    def timed(step, steps):
+    def timed(step, first, steps):
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         l0 = s.kernel_launches
         ev0.record()
-        out = None
-        for _ in range(steps):
-            out = step()
+        outs, solve_ms, update_ms = [], [], []
+        for k in range(first, first + steps):
+            outs.append(step(k))
+            solve_ms.append(s.last_solve_ms); update_ms.append(s.last_update_ms)
         ev1.record()
         barrier()
-        ms = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item()), out, s.kernel_launches - l0
+        return ev0.elapsed_time(ev1), outs, s.kernel_launches - l0, solve_ms, update_ms
 
-    for _ in range(args.warmup):
-        step_device()
+    if args.roofline_only:                 # profiling aid: only the roofline kernel (after one update), nothing timed
+        s.update_coeffs(*d_in[0][:2])
+        n0 = s.level_n(0)
+        xs, bs = torch.randn(n0, dtype=torch.float64, device="cuda"), torch.randn(n0, dtype=torch.float64, device="cuda")
+        for _ in range(4):
+            s.smooth(0, xs, bs, 2)
+        torch.cuda.synchronize()
+        s.close()
+        return
+    for k in range(args.warmup):
+        step_device(k)
     sampler = ClockSampler(local) if rank == 0 else None
-    ms, (iters, relres, rc), launches = timed(step_device, args.steps)
-    solve_ms, update_ms = s.last_solve_ms, s.last_update_ms
+    ms_loc, outs, launches, solve_ms, update_ms = timed(step_device, args.warmup, args.steps)
     clocks = sampler.stop() if sampler else None
-    step_host()
-    ms_e2e, (it_e, rr_e, rc_e), _ = timed(step_host, args.steps)
+    iters_all = [o[0] for o in outs]
+    ms, work, value = whole_job(ms_loc, float(pl.n) * sum(iters_all), world, "cuda")
+    for k in range(args.warmup):
+        step_host(k)
+    ms_e_loc, outs_e, _, _, _ = timed(step_host, args.warmup, args.steps)
+    ms_e2e, _, value_e2e = whole_job(ms_e_loc, float(pl.n) * sum(o[0] for o in outs_e), world, "cuda")
 
-    # whole-job unknown*iters (every rank may take a different number of iterations)
-    work = torch.tensor([float(pl.n) * iters, float(pl.n), float(iters)], dtype=torch.float64, device="cuda")
-    work_e = torch.tensor([float(pl.n) * it_e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(work); dist.all_reduce(work_e)
-    value = float(work[0].item()) * args.steps / (ms * 1e-3)
-    value_e2e = float(work_e[0].item()) * args.steps / (ms_e2e * 1e-3)
-
-    # ---- roofline of the dominant kernel: one RB-B Gauss-Seidel sweep on the finest level, timed live
+    # ---- roofline of the dominant kernel, timed live with CUDA events on the launching stream: k_gs<2,0>, two
+    # fused red-black-boundary Gauss-Seidel sweeps on the finest level (x read), launched back to back
     peak, peak_src = peaks()
     roof = None
     if rank == 0:
@@ -215,13 +257,18 @@ def run_ours(args):
                 torch.cuda.synchronize(); e0.record(); s.smooth(0, xs, bs, k); e1.record(); torch.cuda.synchronize()
                 best = min(best, e0.elapsed_time(e1))
             return best
-        t_smooth(1, 2)
-        sweeps = 10
-        per_sweep_ms = (t_smooth(sweeps) - t_smooth(0)) / sweeps
-        achieved = GS_BYTES_PER_POINT * n0 / (per_sweep_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "gs_sweep level 0 (red + black + guard groups)", "achieved": achieved, "peak": peak,
-                "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                "algorithmic_bytes_per_launch": GS_BYTES_PER_POINT * n0, "ms_per_launch": per_sweep_ms}
+        t_smooth(2, 2)
+        launches_gs = 8
+        per_launch_ms = (t_smooth(2 * launches_gs) - t_smooth(0)) / launches_gs     # mg_smooth(0 sweeps) = the two permutation kernels
+        alg = 2 * GS_BYTES_PER_POINT * n0
+        achieved = alg / (per_launch_ms * 1e-3) / 1e9
+        traffic = GS_TRAFFIC_PER_LAUNCH.get(args.config)
+        roof = {"bound": "hbm", "kernel": "k_gs<2,0> level 0: two fused RB-B Gauss-Seidel sweeps per launch", "achieved": achieved,
+                "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                "algorithmic_bytes_per_launch": alg, "ms_per_launch": per_launch_ms,
+                "note": "algorithmic bytes = 64 B/pt per sweep of the three-loop formulation (SURVEY.md 8(d)); temporal blocking "
+                        "moves fewer (traffic, ncu), so frac can exceed 1; frac_of_traffic = traffic / time / peak",
+                "frac_of_traffic": (traffic / (per_launch_ms * 1e-3) / 1e9 / peak) if traffic else None}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -235,11 +282,14 @@ def run_ours(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config], "unknowns_per_plane": pl.n, "planes": world, "rtol": RTOL,
                            "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels,
+                           "step": "mg_update_coeffs + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
                            "l2_policy": "inputs larger than L2 (no flush)" if pl.n * 8 * 8 > 126e6 else "working set fits L2 (small config)"},
-                "iters": iters, "final_relres": relres, "status": rc, "solve_ms": solve_ms, "update_ms": update_ms,
+                "iters": iters_all[-1], "iters_per_step": iters_all, "final_relres": outs[-1][1], "status": outs[-1][2],
+                "solve_ms": float(np.median(solve_ms)), "update_ms": float(np.median(update_ms)),
+                "solve_ms_per_plane": float(np.median(solve_ms)),
                 "clocks": clocks, "gpu_launches": launches,
                 "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": 4 * pl.n * 8, "d2h_bytes_per_step": pl.n * 8,
-                        "ms_per_step": ms_e2e / args.steps, "iters": it_e},
+                        "ms_per_step": ms_e2e / args.steps, "iters": outs_e[-1][0]},
                 "roofline": roof, "cpu_baseline": cpu}
         print(json.dumps(line))
     s.close()
@@ -256,6 +306,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--ref-iters", type=int, default=2, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

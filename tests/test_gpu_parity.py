@@ -181,3 +181,33 @@ def test_fused_small_levels_bit_identical(gpu, oracle_mod, case, nu):
     o.update(pl.lam, pl.c)
     ro = o.solve(pl.f, pl.x0, 1e-10)
     assert abs(int(out[0][-1][0]) - ro["iters"]) <= 1 and rel(out[0][-2], ro["x"]) <= TOL_SOLVE
+
+
+def test_time_stepping_update_and_warm_start(gpu, oracle_mod):
+    """BASELINE.json configs[4] at reduced size: successive solves on one mesh with coefficients and right-hand
+    side perturbed every step (mg_update_coeffs + per-level coefficient restriction), each solve warm-started
+    from the previous solution, output aliasing the initial guess."""
+    pl = W.make_plane(5, 257)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    xo = pl.x0.copy()
+    xg = dev(pl.x0)
+    cur = pl
+    for k in range(4):
+        o.update(cur.lam, cur.c)
+        ro = o.solve(cur.f, xo, 1e-10)
+        s.update_coeffs(dev(cur.lam), dev(cur.c))
+        for lv in range(o.levels):                      # U1 on every level after every update
+            lo, co = o.level_coeffs(lv)
+            lg, cg = s.level_coeffs(lv)
+            assert rel(lg, lo) <= TOL_STEP and rel(cg, co) <= TOL_STEP
+        _, iters, relres, rc = s.solve(dev(cur.f), xg, 1e-10, x=xg)
+        assert rc == 0 and ro["status"] == 0 and abs(iters - ro["iters"]) <= 1
+        assert rel(host(xg), ro["x"]) <= TOL_SOLVE and relres < 1e-10
+        if k > 0:
+            assert iters < first_iters                  # the warm start pays
+        else:
+            first_iters = iters
+        xo = ro["x"]
+        cur = W.next_step(cur, k)
+    s.close()
