@@ -11,7 +11,7 @@ namespace mgb {
 namespace {
 
 template <int MODE>
-__global__ void __launch_bounds__(NT) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr, const int* __restrict__ stop) {
+__global__ void __launch_bounds__(NT, 3) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr, const int* __restrict__ stop) {
     __shared__ int tn[9];
     if (stop != nullptr && *stop) return;
     const int t = blockIdx.x;

@@ -111,10 +111,10 @@ __global__ void __launch_bounds__(GT, 1) k_tail(const LevelDev* __restrict__ lev
 
 size_t tail_smem() {
     size_t m = DR_SMEM;
-    m = std::max(m, Geo<2, true>::SMEM);
-    m = std::max(m, Geo<2, false>::SMEM);
-    m = std::max(m, Geo<1, true>::SMEM);
-    m = std::max(m, Geo<1, false>::SMEM);
+    m = std::max(m, Geo<2, true>::SMEM_COH);
+    m = std::max(m, Geo<2, false>::SMEM_COH);
+    m = std::max(m, Geo<1, true>::SMEM_COH);
+    m = std::max(m, Geo<1, false>::SMEM_COH);
     return m;
 }
 

@@ -34,7 +34,7 @@ __device__ __forceinline__ double ldv(const double* p) { return COH ? __ldca(p) 
 #endif
 
 constexpr int GT = 512;     // threads per CTA
-constexpr int GCAP = 1024;  // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
+constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
 template <int NS, bool PC>
 struct Geo {
@@ -45,7 +45,9 @@ struct Geo {
     static constexpr int NC = RH * RWC;             // cells per colour
     static constexpr int RN = 2 * NC;
     static constexpr int ROUNDS = (NC + GT - 1) / GT;
-    static constexpr size_t SMEM = (size_t)RN * ((PC ? 3 : 2) * sizeof(double) + sizeof(uint16_t)) + (size_t)GCAP * (sizeof(double) + sizeof(uint16_t));
+    static constexpr size_t SMEM = (size_t)RN * (2 * sizeof(double) + sizeof(uint16_t)) + (size_t)GCAP * (sizeof(double) + sizeof(uint16_t));
+    // the batched staging of the fused small-level kernel keeps the prolongated correction in a third array
+    static constexpr size_t SMEM_COH = SMEM + (PC ? (size_t)RN * sizeof(double) : 0);
 };
 
 // Interior tiles (every cell within 2*NS of the tile is an inner point; flagged by the host setup) take a
@@ -139,7 +141,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
     double* sc = sx + RN;
     double* gb = sc + RN;
     double* se = gb + GCAP;                                  // (PC, batched staging) prolongated correction
-    uint16_t* scode = reinterpret_cast<uint16_t*>(se + (PC ? RN : 0));
+    uint16_t* scode = reinterpret_cast<uint16_t*>(se + ((PC && COH) ? RN : 0));
     uint16_t* glist = scode + RN;
     __shared__ int tn[9];
     __shared__ int pt[9];
@@ -393,6 +395,9 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
     double* sc = sx + RN;
+    double* sce = sc + RN;                                   // (PC) coarse values under the region
+    constexpr int CM = (H + 1) / 2, CW = TX / 2 + (H - 1) / 2 + CM + 2, CHH = TY / 2 + (H - 1) / 2 + CM + 2;
+    static_assert((size_t)(2 * RN + CW * CHH) * sizeof(double) <= Geo<NS, true>::SMEM, "coarse stage must fit the PC allocation");
     __shared__ int tn[9];
     __shared__ int pt[9];
     __shared__ int odd[2];
@@ -441,6 +446,11 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
             }
         }
     } else {
+        if (PC)                                             // coarse values under the region, staged once
+            for (int i = tid; i < CW * CHH; i += GT) {
+                const int ccy = i / CW, ccx = i - ccy * CW;
+                sce[i] = ldv<COH>(ec + parent_slot9(pt, odd[0] * (TX / 2) + ccx - CM, odd[1] * (TY / 2) + ccy - CM));
+            }
     #pragma unroll
         for (int col = 0; col < 2; col++)
     #pragma unroll
@@ -451,19 +461,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
                 const int64_t s = region_slot<H>(tn, rx, ry);
                 const int idx = col * NC + q;
-                double x = xin_zero ? 0.0 : ldv<COH>(xin + s);
-                if (PC) {                                           // x <- x - P e_c (bilinear)
-                    const int lx = rx - H, ly = ry - H;
-                    const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
-                    const int ax = lx & 1, ay = ly & 1;
-                    double e;
-                    if (!ax && !ay) e = ldv<COH>(ec + parent_slot9(pt, cx, cy));
-                    else if (ax && !ay) e = 0.5 * ldv<COH>(ec + parent_slot9(pt, cx, cy)) + 0.5 * ldv<COH>(ec + parent_slot9(pt, cx + 1, cy));
-                    else if (!ax && ay) e = 0.5 * ldv<COH>(ec + parent_slot9(pt, cx, cy)) + 0.5 * ldv<COH>(ec + parent_slot9(pt, cx, cy + 1));
-                    else e = 0.25 * ldv<COH>(ec + parent_slot9(pt, cx, cy)) + 0.25 * ldv<COH>(ec + parent_slot9(pt, cx + 1, cy)) +
-                             0.25 * ldv<COH>(ec + parent_slot9(pt, cx, cy + 1)) + 0.25 * ldv<COH>(ec + parent_slot9(pt, cx + 1, cy + 1));
-                    x -= e;
-                }
+                const double x = xin_zero ? 0.0 : ldv<COH>(xin + s);
                 sx[idx] = x;
                 sc[idx] = __ldg(lv.c + s);
                 const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
@@ -474,6 +472,28 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
             }
     }
     __syncthreads();
+    if (PC && !COH) {
+        // x <- x - P e_c on the owned cells (bilinear; all cells of an interior tile are inner):
+        // weights 1 / (1/2, 1/2) / (1/4 x 4) over the parents (cx, cy), (cx+1, cy), (cx, cy+1), (cx+1, cy+1)
+#pragma unroll
+        for (int col = 0; col < 2; col++)
+#pragma unroll
+            for (int r = 0; r < ROUNDS; r++) {
+                const int q = tid + r * GT;
+                if (q >= NC) continue;
+                const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
+                const int lx = rx - H, ly = ry - H;
+                const double* p = sce + ((ly >> 1) + CM) * CW + (lx >> 1) + CM;
+                const int ax = lx & 1, ay = ly & 1;
+                double e;
+                if (!ax && !ay) e = p[0];
+                else if (ax && !ay) e = 0.5 * p[0] + 0.5 * p[1];
+                else if (!ax && ay) e = 0.5 * p[0] + 0.5 * p[CW];
+                else e = 0.25 * p[0] + 0.25 * p[1] + 0.25 * p[CW] + 0.25 * p[CW + 1];
+                sx[col * NC + q] -= e;
+            }
+        __syncthreads();
+    }
     const double kappa = lv.kappa;
 #pragma unroll
     for (int sweep = 0; sweep < NS; sweep++)
