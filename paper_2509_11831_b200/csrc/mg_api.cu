@@ -35,6 +35,8 @@ struct LevelBuf {           // device arrays owned per level
     uint8_t* tflag = nullptr;
     int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
     double *lam = nullptr, *c = nullptr, *rd = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
+    double* tb = nullptr;   // right-hand side of the single-step entry points.  The cycle's own b of a coarse level is written ONLY by
+                            // the restriction kernels: slots of coarse points under no fine tile are never written and must stay 0.
 };
 
 }  // namespace
@@ -64,6 +66,7 @@ struct mg_handle_s {
     // host-buffer staging
     double* stage[3] = {nullptr, nullptr, nullptr};
     bool have_coeffs = false;
+    bool no_fused_dr = false;             // debugging: separate defect + restriction kernel
     cudaError_t tail_err = cudaSuccess;
     bool host_only = false;
     cudaStream_t cap_stream = nullptr;
@@ -104,10 +107,12 @@ Launch LZ(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }
 
 // nu Gauss-Seidel sweeps, two per launch where possible, ping-ponging between `cur` and `other`.
 // Returns the buffer that holds the result.
-VecRef enqueue_smooth(const Launch& L, const LevelDev& lv, VecRef cur, VecRef other, VecRef b, int nu, bool cur_is_zero) {
+// With `coarse`, the last launch also writes the restricted defect of the result to d_coarse.
+VecRef enqueue_smooth(const Launch& L, const LevelDev& lv, VecRef cur, VecRef other, VecRef b, int nu, bool cur_is_zero,
+                      const LevelDev* coarse = nullptr, double* d_coarse = nullptr) {
     while (nu > 0) {
         const int k = nu >= 2 ? 2 : 1;
-        launch_gs_fused(L, lv, cur, other, b, k, cur_is_zero);
+        launch_gs_fused(L, lv, cur, other, b, k, cur_is_zero, nu == k ? coarse : nullptr, d_coarse);
         std::swap(cur, other);
         cur_is_zero = false;
         nu -= k;
@@ -121,17 +126,18 @@ void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailPr
     const LevelDev& lv = h->lev[s];
     if (s == h->L - 1) { TailOp op{}; op.type = TAIL_COARSE; op.level = (unsigned char)s; op.ntiles = 1; op.a = b; op.b = x; push(op); return; }
     double *cur = x, *other = h->buf[s].x2;
-    auto gs = [&](int k, bool pc, bool zero, const double* ec) {
-        TailOp op{}; op.type = TAIL_GS; op.level = (unsigned char)s; op.ns = (unsigned char)k; op.pc = pc; op.zero = zero;
-        op.ntiles = lv.ntiles; op.a = cur; op.b = other; op.c = b; op.ec = ec; push(op);
+    auto gs = [&](int k, int pc, bool zero, const double* ec) {
+        TailOp op{}; op.type = TAIL_GS; op.level = (unsigned char)s; op.ns = (unsigned char)k; op.pc = (unsigned char)pc; op.zero = zero;
+        op.ntiles = lv.ntiles; op.a = cur; op.b = other; op.c = b; op.ec = ec; op.dc = h->buf[s + 1].b; push(op);
         std::swap(cur, other);
     };
-    for (int nu = h->nu_pre; nu > 0;) { const int k = nu >= 2 ? 2 : 1; gs(k, false, x_is_zero, nullptr); x_is_zero = false; nu -= k; }
-    { TailOp op{}; op.type = TAIL_DR; op.level = (unsigned char)s; op.ntiles = h->lev[s + 1].ntiles; op.a = cur; op.b = h->buf[s + 1].b; op.c = b; push(op); }
+    const bool fuse_dr = !h->no_fused_dr;
+    for (int nu = h->nu_pre; nu > 0;) { const int k = nu >= 2 ? 2 : 1; gs(k, (fuse_dr && nu == k) ? 2 : 0, x_is_zero, nullptr); x_is_zero = false; nu -= k; }
+    if (!fuse_dr) { TailOp op{}; op.type = TAIL_DR; op.level = (unsigned char)s; op.ntiles = h->lev[s + 1].ntiles; op.a = cur; op.b = h->buf[s + 1].b; op.c = b; push(op); }
     build_tail(h, s + 1, h->buf[s + 1].x, h->buf[s + 1].b, true, P);
     int nu = h->nu_post;
-    { const int k = nu >= 2 ? 2 : 1; gs(k, true, false, h->buf[s + 1].x); nu -= k; }
-    while (nu > 0) { const int k = nu >= 2 ? 2 : 1; gs(k, false, false, nullptr); nu -= k; }
+    { const int k = nu >= 2 ? 2 : 1; gs(k, 1, false, h->buf[s + 1].x); nu -= k; }
+    while (nu > 0) { const int k = nu >= 2 ? 2 : 1; gs(k, 0, false, nullptr); nu -= k; }
     if (cur != x) { TailOp op{}; op.type = TAIL_COPY; op.level = (unsigned char)s; op.a = cur; op.b = x; op.n = lv.nslots; push(op); }
 }
 
@@ -158,9 +164,11 @@ void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
     }
     VecRef tmp = vec(h->buf[s].x2);
     if (x_is_zero && h->nu_pre == 0) { launch_zero(L, x, lv.nslots); x_is_zero = false; }
-    VecRef cur = enqueue_smooth(L, lv, x, tmp, b, h->nu_pre, x_is_zero);
+    const bool fuse_dr = h->nu_pre > 0 && !h->no_fused_dr;
+    VecRef cur = enqueue_smooth(L, lv, x, tmp, b, h->nu_pre, x_is_zero,                   // P:178-181 (+ P:183-184 fused)
+                                fuse_dr ? &h->lev[s + 1] : nullptr, h->buf[s + 1].b);
     VecRef other = (cur.base == x.base) ? tmp : x;
-    launch_defect_restrict(L, lv, h->lev[s + 1], cur, b, h->buf[s + 1].b);                // P:183-184  R (A x - b)
+    if (!fuse_dr) launch_defect_restrict(L, lv, h->lev[s + 1], cur, b, h->buf[s + 1].b);  // P:183-184  R (A x - b)
     enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), true);         // P:186-189, e0 = 0
     VecRef fin;
     if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass
@@ -305,6 +313,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         TRY(dev_alloc(h, (void**)&b.x2, vb, s));
         TRY(dev_alloc(h, (void**)&b.b, vb, s));
         TRY(dev_alloc(h, (void**)&b.d, vb, s));
+        TRY(dev_alloc(h, (void**)&b.tb, vb, s));
         LevelDev& d = h->lev[l];
         d.ntiles = hl.ntiles;
         d.ntiles_fine = l > 0 ? h->hh.lev[l - 1].ntiles : 0;
@@ -315,6 +324,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     }
     TRY(dev_alloc(h, (void**)&h->d_lev, sizeof(LevelDev) * h->L, s));
     CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
+    h->no_fused_dr = getenv("MG_B200_NO_FUSED_DR") != nullptr;
     h->tail_cap = std::min(tail_max_grid(), 2 * 148);
     if (h->tail_cap > 0 && h->nu_pre >= 1 && h->nu_post >= 1 && ((o.flags & MG_SETUP_FUSED_TAIL) || getenv("MG_B200_FUSED_TAIL")))
         for (int l = h->L - 1; l >= 0 && h->lev[l].ntiles <= h->tail_cap; l--) h->tail_s0 = l;
@@ -589,8 +599,8 @@ int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps
     Launch L = LZ(h, (cudaStream_t)stream);
     const int64_t n = h->hh.lev[level].n;
     launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
-    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
-    VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].b), sweeps, false);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].tb), sweeps, false);
     launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n);
     CU(cudaGetLastError());
     return MG_OK;
@@ -621,8 +631,8 @@ int mg_coarse_solve(mg_handle h, const double* d_b, double* d_x, void* stream) {
     CHECK_LEVEL(d_b && d_x);
     Launch L = LZ(h, (cudaStream_t)stream);
     const int l = h->L - 1;
-    launch_gather(L, d_b, h->buf[l].canon2slot, h->buf[l].b, h->nL);
-    launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, vec(h->buf[l].b), vec(h->buf[l].x));
+    launch_gather(L, d_b, h->buf[l].canon2slot, h->buf[l].tb, h->nL);
+    launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, vec(h->buf[l].tb), vec(h->buf[l].x));
     launch_scatter(L, h->buf[l].x, h->buf[l].canon2slot, d_x, h->nL);
     CU(cudaGetLastError());
     return MG_OK;
@@ -634,8 +644,8 @@ int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stre
     const int64_t n = h->hh.lev[level].n;
     // level buffers x/b of `level` are free here: the recursion only uses those of the coarser levels
     launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
-    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].b, n);
-    enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].b), false);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].tb), false);
     CU(h->tail_err);
     launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
     CU(cudaGetLastError());

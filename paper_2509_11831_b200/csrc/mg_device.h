@@ -24,7 +24,7 @@ struct LevelDev {
     const int32_t* ctab;     // 9 per tile (this level as the coarse side)
     const int32_t* ptab;     // 9 per tile (this level as the fine side): coarse tiles around the parent tile
     const int32_t* tij;      // 2 per tile: tile coordinates (TI, TJ)
-    const uint8_t* tflag;    // per tile: bit 0 / bit 1 = every cell within 2 / 4 cells of the tile is an inner point
+    const uint8_t* tflag;    // per tile: bits 0 / 1 / 2 = every cell within 2 / 4 / 6 cells of the tile is an inner point
     double* lam;
     double* c;
     double* rd;              // 1 / a_ll on inner points (rule D1), 0 elsewhere; derived at every update (U2)
@@ -76,7 +76,9 @@ void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRe
 // `sweeps` (1 or 2) full red-black-boundary Gauss-Seidel sweeps in ONE pass over memory: x_out = S^sweeps x_in.
 // x_in and x_out must be different buffers (halo cells are recomputed by neighbouring CTAs);
 // x_in_zero: treat x_in as the zero vector without reading it.
-void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero);
+// coarse != null: the launch also writes d_coarse = R (A x_out - b) on that level, fused.
+void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero,
+                     const LevelDev* coarse = nullptr, double* d_coarse = nullptr);
 // Same, preceded in the same pass by the coarse-grid correction x_in - P e_c with set_bnds_hom (rule T3).
 void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps);
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n);
@@ -103,14 +105,15 @@ enum { TAIL_GS = 0, TAIL_DR = 1, TAIL_COARSE = 2, TAIL_COPY = 3 };
 #define TAIL_TOPX (reinterpret_cast<double*>(1))   // placeholder: the cycle's x vector (a VecRef resolved on the device)
 #define TAIL_TOPB (reinterpret_cast<double*>(2))   // placeholder: the cycle's right-hand side
 struct TailOp {
-    unsigned char type, level, ns, pc;   // level: the (fine) level the step works on
+    unsigned char type, level, ns, pc;   // level: the (fine) level the step works on; pc: 1 correction first, 2 defect restriction after
     int zero;                            // GS: x_in is the zero vector
     int ntiles;                          // tiles the step loops over
     double *a, *b, *c;                   // GS: x_in, x_out, rhs; DR: x, coarse defect out, rhs; COARSE: rhs, x; COPY: src, dst
     const double* ec;                    // GS with correction: coarse-level solution
+    double* dc;                          // GS with fused defect restriction (pc = 2): restricted defect on level + 1
     int64_t n;                           // COPY: length
 };
-constexpr int TAIL_MAX_OPS = 64;
+constexpr int TAIL_MAX_OPS = 48;
 struct TailProgram {
     int nops;
     TailOp op[TAIL_MAX_OPS];

@@ -110,22 +110,22 @@ void build_tile_tables(HostLevel& lv) {
                 const int32_t q = lv.find_tile((int64_t)lv.tI[t] + dx, (int64_t)lv.tJ[t] + dy);
                 lv.tnb[(size_t)9 * t + (dy + 1) * 3 + (dx + 1)] = q < 0 ? lv.ntiles : q;
             }
-    // interior flags: the smoother's fast path needs every cell within 2 (one sweep) or 4 (two sweeps)
-    // cells of the tile to be an inner point
+    // interior flags: the smoother's fast path needs every cell within 2 NS (+ 2 with the fused defect
+    // restriction) cells of the tile to be an inner point: bits 0, 1, 2 = halo 2, 4, 6 all inner
     lv.tflag.assign((size_t)lv.ntiles + 1, 0);
     for (int32_t t = 0; t < lv.ntiles; t++) {
-        int reach = 4;                                       // largest halo (0, 2 or 4) that is all inner
-        for (int ly = -4; ly < TY + 4 && reach > 0; ly++)
-            for (int lx = -4; lx < TX + 4; lx++) {
+        int reach = 6;                                       // largest halo (0, 2, 4 or 6) that is all inner
+        for (int ly = -6; ly < TY + 6 && reach > 0; ly++)
+            for (int lx = -6; lx < TX + 6; lx++) {
                 const int dist = std::max(std::max(-lx, lx - (TX - 1)), std::max(-ly, ly - (TY - 1)));   // 0 inside the tile
                 if (dist > reach) continue;
                 const int ox = lx < 0 ? -1 : (lx >= TX ? 1 : 0), oy = ly < 0 ? -1 : (ly >= TY ? 1 : 0);
                 const int32_t q = lv.tnb[(size_t)9 * t + (oy + 1) * 3 + (ox + 1)];
                 const uint16_t c = lv.code[(size_t)q * TS + (ly - oy * TY) * TX + (lx - ox * TX)];
-                if (code_kind(c) != C_INNER) reach = dist <= 0 ? 0 : (dist <= 2 ? 0 : 2);
+                if (code_kind(c) != C_INNER) reach = std::min(reach, dist <= 2 ? 0 : (dist <= 4 ? 2 : 4));
                 if (reach == 0) break;
             }
-        lv.tflag[t] = (uint8_t)((reach >= 2 ? 1 : 0) | (reach >= 4 ? 2 : 0));
+        lv.tflag[t] = (uint8_t)((reach >= 2 ? 1 : 0) | (reach >= 4 ? 2 : 0) | (reach >= 6 ? 4 : 0));
     }
     // canonical order: ascending (J, I)
     lv.canon2slot.clear(); lv.canon2slot.reserve((size_t)lv.n);

@@ -7,12 +7,14 @@ namespace mgb {
 namespace {
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-template <int NS, bool PC>
+// DR: additionally d_c = R (A x_out - b) on the next coarser level (ccode = its point codes).
+template <int NS, bool PC, bool DR>
 __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
-                                              int xin_zero, const int* __restrict__ stop) {
+                                              int xin_zero, const uint16_t* __restrict__ ccode, double* __restrict__ dc,
+                                              const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (stop != nullptr && *stop) return;
-    gs_tile<NS, PC, false>(lv, blockIdx.x, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw);
+    gs_tile<NS, PC, false, DR>(lv, blockIdx.x, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc);
 }
 
 __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
@@ -21,21 +23,28 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) d[k] = s[k];
 }
 
-template <int NS, bool PC>
-void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero) {
-    constexpr size_t smem = Geo<NS, PC>::SMEM;
+template <int NS, bool PC, bool DR = false>
+void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
+               const uint16_t* ccode = nullptr, double* dc = nullptr) {
+    constexpr size_t smem = Geo<NS, PC, DR>::SMEM;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_gs<NS, PC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_gs<NS, PC, DR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = true;
     }
-    k_gs<NS, PC><<<lv.ntiles, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, L.stop);
+    k_gs<NS, PC, DR><<<lv.ntiles, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
     if (L.counter) *L.counter += 1;
 }
 
 }  // namespace
 
-void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero) {
+void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero,
+                     const LevelDev* coarse, double* d_coarse) {
+    if (coarse != nullptr) {                                  // + restricted defect of the result
+        if (sweeps == 2) launch_ns<2, false, true>(L, lv, x_in, x_out, b, nullptr, x_in_zero, coarse->code, d_coarse);
+        else launch_ns<1, false, true>(L, lv, x_in, x_out, b, nullptr, x_in_zero, coarse->code, d_coarse);
+        return;
+    }
     if (sweeps == 2) launch_ns<2, false>(L, lv, x_in, x_out, b, nullptr, x_in_zero);
     else launch_ns<1, false>(L, lv, x_in, x_out, b, nullptr, x_in_zero);
 }

@@ -22,10 +22,10 @@ __device__ __forceinline__ double* tail_ptr(double* p, double* topx, double* top
     return p == TAIL_TOPX ? topx : (p == TAIL_TOPB ? topb : p);
 }
 
-template <int NS, bool PC>
+template <int NS, bool PC, bool DR>
 __device__ __forceinline__ void tail_gs(const LevelDev& lv, const TailOp& op, const double* xin, double* xout, const double* b,
-                                        unsigned char* smem, const int* meta) {
-    if ((int)blockIdx.x < op.ntiles) gs_tile<NS, PC, true>(lv, blockIdx.x, xin, xout, b, op.ec, op.zero, smem, meta);
+                                        unsigned char* smem, const int* meta, const uint16_t* ccode) {
+    if ((int)blockIdx.x < op.ntiles) gs_tile<NS, PC, true, DR>(lv, blockIdx.x, xin, xout, b, op.ec, op.zero, smem, meta, ccode, op.dc);
 }
 
 // The grid has one CTA per tile of the largest level involved, so on every level a CTA owns at most the tile
@@ -83,8 +83,16 @@ __global__ void __launch_bounds__(GT, 1) k_tail(const LevelDev* __restrict__ lev
         double* b = tail_ptr(op.b, topx, topb);
         double* c = tail_ptr(op.c, topx, topb);
         if (op.type == TAIL_GS) {                  // a = x_in, b = x_out, c = right-hand side
-            if (op.ns == 2) { if (op.pc) tail_gs<2, true>(lv, op, a, b, c, smem_raw, meta); else tail_gs<2, false>(lv, op, a, b, c, smem_raw, meta); }
-            else            { if (op.pc) tail_gs<1, true>(lv, op, a, b, c, smem_raw, meta); else tail_gs<1, false>(lv, op, a, b, c, smem_raw, meta); }
+            const uint16_t* ccode = op.pc == 2 ? slev[op.level + 1 - s0].code : nullptr;
+            if (op.ns == 2) {
+                if (op.pc == 1) tail_gs<2, true, false>(lv, op, a, b, c, smem_raw, meta, ccode);
+                else if (op.pc == 2) tail_gs<2, false, true>(lv, op, a, b, c, smem_raw, meta, ccode);
+                else tail_gs<2, false, false>(lv, op, a, b, c, smem_raw, meta, ccode);
+            } else {
+                if (op.pc == 1) tail_gs<1, true, false>(lv, op, a, b, c, smem_raw, meta, ccode);
+                else if (op.pc == 2) tail_gs<1, false, true>(lv, op, a, b, c, smem_raw, meta, ccode);
+                else tail_gs<1, false, false>(lv, op, a, b, c, smem_raw, meta, ccode);
+            }
         } else if (op.type == TAIL_DR) {           // a = x, c = right-hand side (fine), b = restricted defect (coarse)
             if (t < op.ntiles) defect_restrict_tile<true>(lv, slev[op.level + 1 - s0], t, a, c, b, smem_raw, smeta[op.level + 1 - s0]);
         } else if (op.type == TAIL_COARSE) {       // b = A^-1 a on the coarsest level (rule C)
@@ -115,6 +123,8 @@ size_t tail_smem() {
     m = std::max(m, Geo<2, false>::SMEM_COH);
     m = std::max(m, Geo<1, true>::SMEM_COH);
     m = std::max(m, Geo<1, false>::SMEM_COH);
+    m = std::max(m, Geo<2, false, true>::SMEM_COH);
+    m = std::max(m, Geo<1, false, true>::SMEM_COH);
     return m;
 }
 

@@ -36,9 +36,10 @@ __device__ __forceinline__ double ldv(const double* p) { return COH ? __ldca(p) 
 constexpr int GT = 512;     // threads per CTA
 constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
-template <int NS, bool PC>
+// DR: the launch also restricts the defect of its result (needs x two cells beyond the tile).
+template <int NS, bool PC, bool DR = false>
 struct Geo {
-    static constexpr int H = 3 * NS + (PC ? 1 : 0);
+    static constexpr int H = 3 * NS + (PC ? 1 : 0) + (DR ? 2 : 0);
     static constexpr int RW = TX + 2 * H;
     static constexpr int RH = TY + 2 * H;
     static constexpr int RWC = RW / 2;              // cells per colour and row
@@ -53,9 +54,9 @@ struct Geo {
 // Interior tiles (every cell within 2*NS of the tile is an inner point; flagged by the host setup) take a
 // fast path: no guard phase, so the valid region shrinks by 2 instead of 3 cells per sweep (halo 2*NS), and
 // no point codes are needed at all.
-template <int NS>
+template <int NS, bool DR = false>
 struct GeoF {
-    static constexpr int H = 2 * NS;
+    static constexpr int H = 2 * NS + (DR ? 2 : 0);
     static constexpr int RW = TX + 2 * H;
     static constexpr int RH = TY + 2 * H;
     static constexpr int RWC = RW / 2;
@@ -113,6 +114,66 @@ __device__ __forceinline__ int64_t parent_slot9(const int* pt, int cx, int cy) {
     return (int64_t)pt[(oy + 1) * 3 + ox + 1] * TS + (cy - oy * TY) * TX + (cx - ox * TX);
 }
 
+// Fused defect restriction (rules D4 + T2), run after the sweeps of a pre-smoothing launch: every
+// thread forms d = A x - b (difference form of rule D1) for its own inner cells of the tile and of the one-cell
+// ring around it, parks it in the (no longer needed) c array, and the 32 x 16 coarse points under the tile
+// gather their 3 x 3 full-weighting stencils; coarse guard rows get 0.  `breg` still holds b.
+template <class G, bool GENERAL>
+__device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int* tn, const int* pt, const int* odd, const double* sx,
+                                                  double* sc, const uint16_t* scode, double (&breg)[2][G::ROUNDS], double kappa,
+                                                  const uint16_t* __restrict__ ccode, double* __restrict__ dc) {
+    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, ROUNDS = G::ROUNDS;
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            const int q = tid + r * GT;
+            double d = 0.0;
+            if (q < NC) {
+                const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
+                const int own = col * NC + q, ob = (1 - col) * NC + q;
+                const bool inner = GENERAL ? ((scode[own] & 3) == C_INNER) : true;
+                if (inner && min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) >= H - 1) {
+                    const double lam = __ldg(lv.lam + region_slot<H>(tn, rx, ry));
+                    const double cl = sc[own], xl = sx[own];
+                    const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
+                    const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
+                    d = lam * xl + aW * (xl - sx[ob + tpar - 1]) + aE * (xl - sx[ob + tpar]) + aS * (xl - sx[ob - RWC]) +
+                        aN * (xl - sx[ob + RWC]) - breg[col][r];
+                }
+            }
+            breg[col][r] = d;
+        }
+    __syncthreads();
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            const int q = tid + r * GT;
+            if (q < NC) sc[col * NC + q] = breg[col][r];
+        }
+    __syncthreads();
+    const int ptile = pt[4];                                  // the coarse tile this fine tile lies under
+    if (ptile == lv.ntiles_coarse) return;                    // no coarse point here
+    for (int i = tid; i < (TX / 2) * (TY / 2); i += GT) {
+        const int cyl = i / (TX / 2), cxl = i - cyl * (TX / 2);
+        const int rx = 2 * cxl + H, ry = 2 * cyl + H;
+        const int64_t cs = (int64_t)ptile * TS + (odd[1] * (TY / 2) + cyl) * TX + odd[0] * (TX / 2) + cxl;
+        double acc = 0.0;
+        if ((__ldg(ccode + cs) & 3) == C_INNER) {
+#pragma unroll
+            for (int dy = -1; dy <= 1; dy++)
+#pragma unroll
+                for (int dx = -1; dx <= 1; dx++) {
+                    const double w = (dx == 0 ? 2.0 : 1.0) * (dy == 0 ? 2.0 : 1.0) * 0.0625;
+                    acc += w * sc[cidx<G>(rx + dx, ry + dy)];
+                }
+        }
+        dc[cs] = acc;
+    }
+}
+
 // e = (P e_c) at fine cell (lx, ly) relative to the tile (may lie in the halo): bilinear, weights
 // 1 / (1/2, 1/2) / (1/4 x 4) in the order (cx, cy), (cx+1, cy), (cx, cy+1), (cx+1, cy+1); absent parents hold 0.
 // Branch-free (unused parents alias the first one with weight 0) so that the loads of all cells overlap.
@@ -130,11 +191,12 @@ __device__ __forceinline__ double prolong_e(const int* pt, int odd0, int odd1, i
 }
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-template <int NS, bool PC, bool COH>
+template <int NS, bool PC, bool COH, bool DR = false>
 __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                            const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
-                                           unsigned char* smem_raw, const int* meta = nullptr) {
-    using G = Geo<NS, PC>;
+                                           unsigned char* smem_raw, const int* meta = nullptr,
+                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr) {
+    using G = Geo<NS, PC, DR>;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
@@ -155,9 +217,9 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
     } else {
         if (tid < 9) {
             tn[tid] = lv.tnb[9 * t + tid];
-            if (PC) pt[tid] = lv.ptab[9 * t + tid];
+            if (PC || DR) pt[tid] = lv.ptab[9 * t + tid];
         }
-        if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
+        if (tid < 2 && (PC || DR)) odd[tid] = lv.tij[2 * t + tid] & 1;
     }
     if (tid == 0) gcount = 0;
     __syncthreads();
@@ -383,14 +445,16 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
         const int ly = idx / TX, lx = idx - ly * TX;
         xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
     }
+    if (DR) restrict_epilogue<G, true>(lv, tn, pt, odd, sx, sc, scode, breg, kappa, ccode, dc);
 }
 
 // Interior tile: all cells of the region are inner points.
-template <int NS, bool PC, bool COH>
+template <int NS, bool PC, bool COH, bool DR = false>
 __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
-                                        unsigned char* smem_raw, const int* meta = nullptr) {
-    using G = GeoF<NS>;
+                                        unsigned char* smem_raw, const int* meta = nullptr,
+                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr) {
+    using G = GeoF<NS, DR>;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
@@ -409,9 +473,9 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
     } else {
         if (tid < 9) {
             tn[tid] = lv.tnb[9 * t + tid];
-            if (PC) pt[tid] = lv.ptab[9 * t + tid];
+            if (PC || DR) pt[tid] = lv.ptab[9 * t + tid];
         }
-        if (tid < 2 && PC) odd[tid] = lv.tij[2 * t + tid] & 1;
+        if (tid < 2 && (PC || DR)) odd[tid] = lv.tij[2 * t + tid] & 1;
     }
     __syncthreads();
     double breg[2][ROUNDS], rd[2][ROUNDS];
@@ -519,15 +583,18 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
         const int ly = idx / TX, lx = idx - ly * TX;
         xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
     }
+    if (DR) restrict_epilogue<G, false>(lv, tn, pt, odd, sx, sc, nullptr, breg, kappa, ccode, dc);
 }
 
-template <int NS, bool PC, bool COH>
+template <int NS, bool PC, bool COH, bool DR = false>
 __device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
-                                        unsigned char* smem_raw, const int* meta = nullptr) {
+                                        unsigned char* smem_raw, const int* meta = nullptr,
+                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr) {
     const int flag = meta != nullptr ? meta[META_FLAG] : lv.tflag[t];
-    if (flag & (NS == 2 ? 2 : 1)) gs_fast<NS, PC, COH>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta);
-    else gs_general<NS, PC, COH>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta);
+    constexpr int need = 1 << (NS - 1 + (DR ? 1 : 0));          // interior halo 2 NS (+ 2): flag bit
+    if (flag & need) gs_fast<NS, PC, COH, DR>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc);
+    else gs_general<NS, PC, COH, DR>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc);
 }
 
 }  // namespace
