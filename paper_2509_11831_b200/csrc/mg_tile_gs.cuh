@@ -33,6 +33,8 @@ template <bool COH>
 __device__ __forceinline__ double ldv(const double* p) { return COH ? __ldca(p) : __ldg(p); }
 #endif
 
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 constexpr int GT = 512;     // threads per CTA
 constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
@@ -368,6 +370,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     const int base = 1 + col + (PC ? 1 : 0);
                     const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
                     if (nsw > 0) { breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s); }
+                    if (DR && marg >= H - 1) prefetch_l2(lv.lam + s);     // read by the restriction epilogue
                     act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
                 } else if (kind != C_ABSENT) {
                     const int pos = atomicAdd(&gcount, 1);
@@ -532,6 +535,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 const int base = 1 + col;
                 const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
                 if (nsw > 0) { breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s); }
+                if (DR && marg >= H - 1) prefetch_l2(lv.lam + s);         // read by the restriction epilogue
                 act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
             }
     }
