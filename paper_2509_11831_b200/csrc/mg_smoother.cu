@@ -1,5 +1,7 @@
 // Kernels and launchers of the smoother; the tile-level device code is in mg_tile_gs.cuh (shared with the
 // fused small-level kernel of mg_tail.cu).
+#include <cstdlib>
+
 #include "mg_tile_gs.cuh"
 
 namespace mgb {
@@ -8,13 +10,17 @@ namespace {
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
 // DR: additionally d_c = R (A x_out - b) on the next coarser level (ccode = its point codes).
-template <int NS, bool PC, bool DR>
+// BX x BY < tile: several CTAs per tile (blockIdx = tile * blocks-per-tile + block).
+template <int NS, bool PC, bool DR, int BX, int BY>
 __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
                                               int xin_zero, const uint16_t* __restrict__ ccode, double* __restrict__ dc,
                                               const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (stop != nullptr && *stop) return;
-    gs_tile<NS, PC, false, DR>(lv, blockIdx.x, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc);
+    constexpr int NBX = TX / BX, NSUB = NBX * (TY / BY);
+    const int t = blockIdx.x / NSUB, sub = blockIdx.x - t * NSUB;
+    gs_tile<NS, PC, false, DR, BX, BY>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
+                                       (sub % NBX) * BX, (sub / NBX) * BY);
 }
 
 __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
@@ -23,17 +29,29 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) d[k] = s[k];
 }
 
+// Levels of at most SUB_MAX_TILES tiles are latency bound (7-25 us per launch whatever the tile count,
+// profiles/r01c_small_levels.md): they run with one CTA per SBX x SBY block, 8 CTAs per tile.
+constexpr int SUB_MAX_TILES = 148, SBX = 16, SBY = 16;
+
+template <int NS, bool PC, bool DR, int BX, int BY>
+void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
+                const uint16_t* ccode, double* dc) {
+    constexpr size_t smem = Geo<NS, PC, DR, BX, BY>::SMEM;
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_gs<NS, PC, DR, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        configured = true;
+    }
+    const int grid = lv.ntiles * (TX / BX) * (TY / BY);
+    k_gs<NS, PC, DR, BX, BY><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
+    if (L.counter) *L.counter += 1;
+}
+
 template <int NS, bool PC, bool DR = false>
 void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
                const uint16_t* ccode = nullptr, double* dc = nullptr) {
-    constexpr size_t smem = Geo<NS, PC, DR>::SMEM;
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_gs<NS, PC, DR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = true;
-    }
-    k_gs<NS, PC, DR><<<lv.ntiles, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
-    if (L.counter) *L.counter += 1;
+    if (lv.ntiles <= SUB_MAX_TILES && !getenv("MG_B200_NO_SUBBLOCKS")) launch_blk<NS, PC, DR, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else launch_blk<NS, PC, DR, TX, TY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
 }
 
 }  // namespace

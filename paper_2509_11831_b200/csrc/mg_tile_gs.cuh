@@ -39,11 +39,14 @@ constexpr int GT = 512;     // threads per CTA
 constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
 // DR: the launch also restricts the defect of its result (needs x two cells beyond the tile).
-template <int NS, bool PC, bool DR = false>
+// BX x BY: the block of the tile one CTA produces (the whole tile, or a sub-block on small levels where
+// latency, not throughput, decides: more CTAs per tile).
+template <int NS, bool PC, bool DR = false, int BX = TX, int BY = TY>
 struct Geo {
     static constexpr int H = 3 * NS + (PC ? 1 : 0) + (DR ? 2 : 0);
-    static constexpr int RW = TX + 2 * H;
-    static constexpr int RH = TY + 2 * H;
+    static constexpr int RW = BX + 2 * H;
+    static constexpr int RH = BY + 2 * H;
+    static constexpr int BW = BX, BH = BY;
     static constexpr int RWC = RW / 2;              // cells per colour and row
     static constexpr int NC = RH * RWC;             // cells per colour
     static constexpr int RN = 2 * NC;
@@ -56,11 +59,12 @@ struct Geo {
 // Interior tiles (every cell within 2*NS of the tile is an inner point; flagged by the host setup) take a
 // fast path: no guard phase, so the valid region shrinks by 2 instead of 3 cells per sweep (halo 2*NS), and
 // no point codes are needed at all.
-template <int NS, bool DR = false>
+template <int NS, bool DR = false, int BX = TX, int BY = TY>
 struct GeoF {
     static constexpr int H = 2 * NS + (DR ? 2 : 0);
-    static constexpr int RW = TX + 2 * H;
-    static constexpr int RH = TY + 2 * H;
+    static constexpr int RW = BX + 2 * H;
+    static constexpr int RH = BY + 2 * H;
+    static constexpr int BW = BX, BH = BY;
     static constexpr int RWC = RW / 2;
     static constexpr int NC = RH * RWC;
     static constexpr int RN = 2 * NC;
@@ -123,8 +127,8 @@ __device__ __forceinline__ int64_t parent_slot9(const int* pt, int cx, int cy) {
 template <class G, bool GENERAL>
 __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int* tn, const int* pt, const int* odd, const double* sx,
                                                   double* sc, const uint16_t* scode, double (&breg)[2][G::ROUNDS], double kappa,
-                                                  const uint16_t* __restrict__ ccode, double* __restrict__ dc) {
-    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, ROUNDS = G::ROUNDS;
+                                                  const uint16_t* __restrict__ ccode, double* __restrict__ dc, int bx0, int by0) {
+    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, ROUNDS = G::ROUNDS, BX = G::BW, BY = G::BH;
     const int tid = threadIdx.x;
 #pragma unroll
     for (int col = 0; col < 2; col++)
@@ -137,7 +141,7 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
                 const int own = col * NC + q, ob = (1 - col) * NC + q;
                 const bool inner = GENERAL ? ((scode[own] & 3) == C_INNER) : true;
                 if (inner && min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) >= H - 1) {
-                    const double lam = __ldg(lv.lam + region_slot<H>(tn, rx, ry));
+                    const double lam = __ldg(lv.lam + region_slot<H>(tn, rx + bx0, ry + by0));
                     const double cl = sc[own], xl = sx[own];
                     const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
                     const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
@@ -158,10 +162,10 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
     __syncthreads();
     const int ptile = pt[4];                                  // the coarse tile this fine tile lies under
     if (ptile == lv.ntiles_coarse) return;                    // no coarse point here
-    for (int i = tid; i < (TX / 2) * (TY / 2); i += GT) {
-        const int cyl = i / (TX / 2), cxl = i - cyl * (TX / 2);
+    for (int i = tid; i < (BX / 2) * (BY / 2); i += GT) {
+        const int cyl = i / (BX / 2), cxl = i - cyl * (BX / 2);
         const int rx = 2 * cxl + H, ry = 2 * cyl + H;
-        const int64_t cs = (int64_t)ptile * TS + (odd[1] * (TY / 2) + cyl) * TX + odd[0] * (TX / 2) + cxl;
+        const int64_t cs = (int64_t)ptile * TS + (odd[1] * (TY / 2) + by0 / 2 + cyl) * TX + odd[0] * (TX / 2) + bx0 / 2 + cxl;
         double acc = 0.0;
         if ((__ldg(ccode + cs) & 3) == C_INNER) {
 #pragma unroll
@@ -193,12 +197,13 @@ __device__ __forceinline__ double prolong_e(const int* pt, int odd0, int odd1, i
 }
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-template <int NS, bool PC, bool COH, bool DR = false>
+template <int NS, bool PC, bool COH, bool DR = false, int BX = TX, int BY = TY>
 __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                            const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                            unsigned char* smem_raw, const int* meta = nullptr,
-                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr) {
-    using G = Geo<NS, PC, DR>;
+                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr,
+                                           int bx0 = 0, int by0 = 0) {
+    using G = Geo<NS, PC, DR, BX, BY>;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
@@ -239,13 +244,13 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
             for (int r = 0; r < ROUNDS; r++) {
                 const int q = min(tid + r * GT, NC - 1);
                 const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
-                const int64_t s = region_slot<H>(tn, rx, ry);
+                const int64_t s = region_slot<H>(tn, rx + bx0, ry + by0);
                 codes[r] = __ldg(lv.code + s);
                 xv[r] = (!PC && xin_zero) ? 0.0 : ldv<COH>(xin + s);
                 cv[r] = __ldg(lv.c + s);
                 breg[col][r] = ldv<COH>(b + s);
                 rd[col][r] = __ldg(lv.rd + s);
-                ev[r] = PC ? prolong_e<COH>(pt, odd[0], odd[1], rx - H, ry - H, ec) : 0.0;
+                ev[r] = PC ? prolong_e<COH>(pt, odd[0], odd[1], rx - H + bx0, ry - H + by0, ec) : 0.0;
             }
     #pragma unroll
             for (int r = 0; r < ROUNDS; r++) {
@@ -304,14 +309,14 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     const int q = tid + r * GT;
                     if (q >= NC) continue;
                     const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
-                    const int64_t s = region_slot<H>(tn, rx, ry);
+                    const int64_t s = region_slot<H>(tn, rx + bx0, ry + by0);
                     const uint16_t code = __ldg(lv.code + s);
                     const int idx = col * NC + q;
                     scode[idx] = code;
                     sx[idx] = ldv<COH>(xin + s);
                     double e = 0.0;
                     if ((code & 3) == C_INNER) {
-                        const int lx = rx - H, ly = ry - H;
+                        const int lx = rx - H + bx0, ly = ry - H + by0;
                         const int cx = odd[0] * (TX / 2) + (lx >> 1), cy = odd[1] * (TY / 2) + (ly >> 1);
                         const int ax = lx & 1, ay = ly & 1;
                         if (!ax && !ay) e = ldv<COH>(ec + parent_slot9(pt, cx, cy));
@@ -354,7 +359,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                 const int q = tid + r * GT;
                 if (q >= NC) continue;
                 const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
-                const int64_t s = region_slot<H>(tn, rx, ry);
+                const int64_t s = region_slot<H>(tn, rx + bx0, ry + by0);
                 const int idx = col * NC + q;
                 uint16_t code;
                 if (PC) code = scode[idx];
@@ -431,7 +436,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                         if (kind != C_DIR && kind != C_NEU) continue;
                         const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
                         if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) < m) continue;
-                        const double bv = ldv<COH>(b + region_slot<H>(tn, rx, ry));
+                        const double bv = ldv<COH>(b + region_slot<H>(tn, rx + bx0, ry + by0));
                         if (kind == C_DIR) sx[idx] = bv;
                         else {
                             double sum, wself, delta;
@@ -444,27 +449,28 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
         }
     }
     // ---- write the tile back (absent slots carry the zeros they were loaded with)
-    for (int idx = tid; idx < TS; idx += GT) {
-        const int ly = idx / TX, lx = idx - ly * TX;
-        xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
+    for (int idx = tid; idx < BX * BY; idx += GT) {
+        const int ly = idx / BX, lx = idx - ly * BX;
+        xout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sx[cidx<G>(lx + H, ly + H)];
     }
-    if (DR) restrict_epilogue<G, true>(lv, tn, pt, odd, sx, sc, scode, breg, kappa, ccode, dc);
+    if (DR) restrict_epilogue<G, true>(lv, tn, pt, odd, sx, sc, scode, breg, kappa, ccode, dc, bx0, by0);
 }
 
 // Interior tile: all cells of the region are inner points.
-template <int NS, bool PC, bool COH, bool DR = false>
+template <int NS, bool PC, bool COH, bool DR = false, int BX = TX, int BY = TY>
 __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                         unsigned char* smem_raw, const int* meta = nullptr,
-                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr) {
-    using G = GeoF<NS, DR>;
+                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr,
+                                           int bx0 = 0, int by0 = 0) {
+    using G = GeoF<NS, DR, BX, BY>;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
     double* sc = sx + RN;
     double* sce = sc + RN;                                   // (PC) coarse values under the region
-    constexpr int CM = (H + 1) / 2, CW = TX / 2 + (H - 1) / 2 + CM + 2, CHH = TY / 2 + (H - 1) / 2 + CM + 2;
-    static_assert((size_t)(2 * RN + CW * CHH) * sizeof(double) <= Geo<NS, true>::SMEM, "coarse stage must fit the PC allocation");
+    constexpr int CM = (H + 1) / 2, CW = BX / 2 + (H - 1) / 2 + CM + 2, CHH = BY / 2 + (H - 1) / 2 + CM + 2;
+    static_assert((size_t)(2 * RN + CW * CHH) * sizeof(double) <= Geo<NS, true, false, BX, BY>::SMEM, "coarse stage must fit the PC allocation");
     __shared__ int tn[9];
     __shared__ int pt[9];
     __shared__ int odd[2];
@@ -491,12 +497,12 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
             for (int r = 0; r < ROUNDS; r++) {
                 const int q = min(tid + r * GT, NC - 1);
                 const int ry = q / RWC, k = q - ry * RWC, rx = 2 * k + ((ry + col) & 1);
-                const int64_t s = region_slot<H>(tn, rx, ry);
+                const int64_t s = region_slot<H>(tn, rx + bx0, ry + by0);
                 xv[r] = xin_zero ? 0.0 : ldv<COH>(xin + s);
                 cv[r] = __ldg(lv.c + s);
                 breg[col][r] = ldv<COH>(b + s);
                 rd[col][r] = __ldg(lv.rd + s);
-                if (PC) xv[r] -= prolong_e<COH>(pt, odd[0], odd[1], rx - H, ry - H, ec);   // x <- x - P e_c
+                if (PC) xv[r] -= prolong_e<COH>(pt, odd[0], odd[1], rx - H + bx0, ry - H + by0, ec);   // x <- x - P e_c
             }
     #pragma unroll
             for (int r = 0; r < ROUNDS; r++) {
@@ -516,7 +522,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
         if (PC)                                             // coarse values under the region, staged once
             for (int i = tid; i < CW * CHH; i += GT) {
                 const int ccy = i / CW, ccx = i - ccy * CW;
-                sce[i] = ldv<COH>(ec + parent_slot9(pt, odd[0] * (TX / 2) + ccx - CM, odd[1] * (TY / 2) + ccy - CM));
+                sce[i] = ldv<COH>(ec + parent_slot9(pt, odd[0] * (TX / 2) + bx0 / 2 + ccx - CM, odd[1] * (TY / 2) + by0 / 2 + ccy - CM));
             }
     #pragma unroll
         for (int col = 0; col < 2; col++)
@@ -526,7 +532,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 const int q = tid + r * GT;
                 if (q >= NC) continue;
                 const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
-                const int64_t s = region_slot<H>(tn, rx, ry);
+                const int64_t s = region_slot<H>(tn, rx + bx0, ry + by0);
                 const int idx = col * NC + q;
                 const double x = xin_zero ? 0.0 : ldv<COH>(xin + s);
                 sx[idx] = x;
@@ -583,22 +589,23 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
             }
             __syncthreads();
         }
-    for (int idx = tid; idx < TS; idx += GT) {
-        const int ly = idx / TX, lx = idx - ly * TX;
-        xout[(int64_t)t * TS + idx] = sx[cidx<G>(lx + H, ly + H)];
+    for (int idx = tid; idx < BX * BY; idx += GT) {
+        const int ly = idx / BX, lx = idx - ly * BX;
+        xout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sx[cidx<G>(lx + H, ly + H)];
     }
-    if (DR) restrict_epilogue<G, false>(lv, tn, pt, odd, sx, sc, nullptr, breg, kappa, ccode, dc);
+    if (DR) restrict_epilogue<G, false>(lv, tn, pt, odd, sx, sc, nullptr, breg, kappa, ccode, dc, bx0, by0);
 }
 
-template <int NS, bool PC, bool COH, bool DR = false>
+template <int NS, bool PC, bool COH, bool DR = false, int BX = TX, int BY = TY>
 __device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                         unsigned char* smem_raw, const int* meta = nullptr,
-                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr) {
+                                           const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr,
+                                           int bx0 = 0, int by0 = 0) {
     const int flag = meta != nullptr ? meta[META_FLAG] : lv.tflag[t];
     constexpr int need = 1 << (NS - 1 + (DR ? 1 : 0));          // interior halo 2 NS (+ 2): flag bit
-    if (flag & need) gs_fast<NS, PC, COH, DR>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc);
-    else gs_general<NS, PC, COH, DR>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc);
+    if (flag & need) gs_fast<NS, PC, COH, DR, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
+    else gs_general<NS, PC, COH, DR, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
 }
 
 }  // namespace
