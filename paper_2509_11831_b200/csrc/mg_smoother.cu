@@ -31,7 +31,8 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
 
 // Levels of at most SUB_MAX_TILES tiles are latency bound (7-25 us per launch whatever the tile count,
 // profiles/r01c_small_levels.md): they run with one CTA per SBX x SBY block, 8 CTAs per tile.
-constexpr int SUB_MAX_TILES = 148, SBX = 16, SBY = 16;
+constexpr int SUB_MAX_TILES = 40, SBX = 16, SBY = 16;      // 8 CTAs per tile
+constexpr int MID_MAX_TILES = 148, MBX = 32, MBY = 16;     // 4 CTAs per tile
 
 template <int NS, bool PC, bool DR, int BX, int BY>
 void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
@@ -50,7 +51,9 @@ void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, Ve
 template <int NS, bool PC, bool DR = false>
 void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
                const uint16_t* ccode = nullptr, double* dc = nullptr) {
-    if (lv.ntiles <= SUB_MAX_TILES && !getenv("MG_B200_NO_SUBBLOCKS")) launch_blk<NS, PC, DR, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    static const bool no_sub = getenv("MG_B200_NO_SUBBLOCKS") != nullptr;
+    if (lv.ntiles <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, DR, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else if (lv.ntiles <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, DR, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else launch_blk<NS, PC, DR, TX, TY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
 }
 
