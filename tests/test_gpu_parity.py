@@ -211,3 +211,38 @@ def test_time_stepping_update_and_warm_start(gpu, oracle_mod):
         xo = ro["x"]
         cur = W.next_step(cur, k)
     s.close()
+
+
+def test_full_size_config4_in_bench_configuration(gpu, oracle_mod):
+    """BASELINE.json configs[3] at its full size (4097^2 lattice, 11.3 M points, 10 levels), exactly as bench.py
+    runs it: index construction against the oracle, single applications on the two finest levels
+    element by element, and the solve through a property that holds at any size: the true residual of
+    the returned x, recomputed by the ORACLE's operator, meets Eq. 23 (the oracle's own full solve takes
+    minutes and is covered at reduced size)."""
+    import torch
+    pl = W.make_plane(4)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    assert s.levels == o.levels == 10
+    for lv in range(o.levels):
+        assert s.level_n(lv) == o.level_n(lv)
+    a, g = o.level_arrays(1), s.level_info(1)
+    for k in ("I", "J", "kind", "colour", "nbr", "ns_fallback"):
+        assert np.array_equal(a[k], g[k])
+    rng = np.random.default_rng(21)
+    for lv in (0, 1):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        assert rel(host(s.apply(lv, dev(x))), o.apply(lv, x)) <= TOL_STEP
+        assert rel(host(s.smooth(lv, dev(x), dev(b), 2)), o.smooth(lv, x, b, 2)) <= TOL_STEP
+    lo, co = o.level_coeffs(3)
+    lg, cg = s.level_coeffs(3)
+    assert rel(lg, lo) <= TOL_STEP and rel(cg, co) <= TOL_STEP
+    x, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert rc == 0 and relres < 1e-10 and 20 <= iters <= 60
+    xc, fc = H.canon(o, host(x)), H.canon(o, pl.f)
+    true = np.linalg.norm(fc - o.apply(0, xc)) / np.linalg.norm(fc)
+    assert true < 1.05e-10 and relres == pytest.approx(true, rel=1e-2)
+    s.close()
