@@ -188,14 +188,14 @@ void enqueue_iteration(mg_handle h, const Launch& L) {
     VecRef zj{h->Z, ns, &h->st->j, 0}, vj{h->V, ns, &h->st->j, 0};
     enqueue_cycle(h, L, 0, zj, vj, true);
     launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
-    launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
+    launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial, h->m);
     if (h->m <= MAX_M_FUSED) {                                     // three passes over the basis
         launch_update_dot(L, h->w, h->V, ns, ns, h->st, h->partial);
         launch_final_v(L, h->w, h->V, ns, ns, h->st);
         return;
     }
     launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 0);
-    launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial);
+    launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial, h->m);
     launch_update_w(L, h->w, h->V, ns, ns, h->st, h->partial, 1);
     launch_givens(L, h->st);
     launch_next_v(L, h->w, h->V, ns, ns, h->st);

@@ -136,7 +136,7 @@ void launch_coarse_solve(const Launch& L, const double* Ainv, const int32_t* csl
 // ---- fGMRES vector kernels (mg_krylov.cu) ----
 void launch_norm2(const Launch& L, const double* v, int64_t n, GmresState* st, double* partial, int which);  // which: 0 -> bn, 1 -> beta
 void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double* V0, int64_t n);
-void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial);
+void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int m);
 void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass);
 void launch_givens(const Launch& L, GmresState* st);
 // fused CGS2 for restart lengths m <= MAX_M_FUSED (three passes over the basis, Givens inside the second)

@@ -283,6 +283,62 @@ __global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ 
     }
 }
 
+// Pass 1 with the same register tiling: all nv <= 32 dot products in ONE pass over w (the chunked k_multidot
+// re-reads w once per 8 vectors and keeps only 9 loads per thread in flight).
+template <int NV, int EPT>
+__device__ __forceinline__ void multidot_body(const double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
+                                              int nv, double (&acc)[FUSED_NV]) {
+    const int64_t G = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k0 < n; k0 += G * EPT) {
+        double v[EPT][NV], wk[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+            const int64_t k = k0 + e * G;
+            const bool ok = k < n;
+            wk[e] = ok ? w[k] : 0.0;
+#pragma unroll
+            for (int c = 0; c < NV; c++) v[e][c] = (ok && c < nv) ? V[(int64_t)c * stride + k] : 0.0;
+        }
+#pragma unroll
+        for (int e = 0; e < EPT; e++)
+#pragma unroll
+            for (int c = 0; c < NV; c++) acc[c] += wk[e] * v[e][c];
+    }
+}
+
+constexpr int MD_THREADS = 256;
+__global__ void __launch_bounds__(MD_THREADS, 2) k_multidot_t(const double* __restrict__ w, const double* __restrict__ V, int64_t stride,
+                                                              int64_t n, GmresState* st, double* __restrict__ partial) {
+    __shared__ double red[MD_THREADS / 32][FUSED_NV];
+    if (st->cycle_end) return;
+    const int nv = st->j + 1;
+    double acc[FUSED_NV];
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) acc[c] = 0.0;
+    if (nv <= 8) multidot_body<8, 4>(w, V, stride, n, nv, acc);
+    else if (nv <= 16) multidot_body<16, 2>(w, V, stride, n, nv, acc);
+    else multidot_body<32, 1>(w, V, stride, n, nv, acc);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) {
+        const double r = warp_sum(acc[c]);
+        if (lane == 0) red[warp][c] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < FUSED_NV) {
+        double r = 0.0;
+        for (int q = 0; q < MD_THREADS / 32; q++) r += red[q][threadIdx.x];
+        partial[(size_t)blockIdx.x * (MAX_M + 2) + threadIdx.x] = r;
+    }
+    if (last_block(st)) {
+        if ((int)threadIdx.x < nv) {
+            double r = 0.0;
+            for (int b = 0; b < (int)gridDim.x; b++) r += ((volatile double*)partial)[(size_t)b * (MAX_M + 2) + threadIdx.x];
+            st->red[threadIdx.x] = r;
+        }
+    }
+}
+
 template <int NV, int EPT>
 __device__ __forceinline__ void final_v_body(const double* __restrict__ w, const double* __restrict__ V, double* __restrict__ out,
                                              int64_t stride, int64_t n, int nv, const double* hh, double inv) {
@@ -366,8 +422,10 @@ void launch_norm2(const Launch& L, const double* v, int64_t n, GmresState* st, d
 void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double* V0, int64_t n) {
     k_start_cycle<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
 }
-void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial) {
-    k_multidot<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial); count(L);
+void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int m) {
+    if (m <= FUSED_NV) k_multidot_t<<<148 * 2, MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    else k_multidot<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    count(L);
 }
 void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass) {
     k_update_w<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
