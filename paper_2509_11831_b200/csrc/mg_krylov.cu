@@ -8,6 +8,8 @@
 // v_0..v_j), fused update + norm; twice.  Same Krylov iterates as the oracle's modified Gram-Schmidt up
 // to rounding.  Grid reductions: per-block partials + last-block-done ticket, summed in a fixed order
 // (deterministic run to run).
+#include <cstdlib>
+
 #include "mg_device.h"
 
 namespace mgb {
@@ -232,22 +234,12 @@ __device__ __forceinline__ void update_dot_body(double* __restrict__ w, const do
     }
 }
 
-__global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
-                                                            int64_t n, GmresState* st, double* __restrict__ partial) {
-    __shared__ double hh[FUSED_NV];
-    __shared__ double red[UD_THREADS / 32][FUSED_NV + 1];
+// Block + grid reduction of the second projection and the Givens step in the last block to arrive.
+template <int THREADS>
+__device__ __forceinline__ void ud_finish(double (&acc)[FUSED_NV], double accn, int nv, const double* hh, GmresState* st,
+                                          double* __restrict__ partial) {
+    __shared__ double red[THREADS / 32][FUSED_NV + 1];
     __shared__ double tot[FUSED_NV + 1];
-    if (st->cycle_end) return;
-    const int nv = st->j + 1;
-    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
-    __syncthreads();
-    double acc[FUSED_NV], accn = 0.0;
-#pragma unroll
-    for (int c = 0; c < FUSED_NV; c++) acc[c] = 0.0;
-    if (nv <= 8) update_dot_body<8, 4>(w, V, stride, n, nv, hh, acc, accn);
-    else if (nv <= 16) update_dot_body<16, 2>(w, V, stride, n, nv, hh, acc, accn);
-    else update_dot_body<32, 1>(w, V, stride, n, nv, hh, acc, accn);
-    // block reduction: warp shuffles, then one thread per value over the warps
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
     for (int c = 0; c < FUSED_NV; c++) {
@@ -259,7 +251,7 @@ __global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ 
     __syncthreads();
     if (threadIdx.x <= FUSED_NV) {
         double r = 0.0;
-        for (int q = 0; q < UD_THREADS / 32; q++) r += red[q][threadIdx.x];
+        for (int q = 0; q < THREADS / 32; q++) r += red[q][threadIdx.x];
         partial[(size_t)blockIdx.x * (MAX_M + 2) + threadIdx.x] = r;
     }
     if (last_block(st)) {
@@ -283,8 +275,117 @@ __global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ 
     }
 }
 
-// Pass 1 with the same register tiling: all nv <= 32 dot products in ONE pass over w (the chunked k_multidot
-// re-reads w once per 8 vectors and keeps only 9 loads per thread in flight).
+__global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
+                                                            int64_t n, GmresState* st, double* __restrict__ partial) {
+    __shared__ double hh[FUSED_NV];
+    if (st->cycle_end) return;
+    const int nv = st->j + 1;
+    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
+    __syncthreads();
+    double acc[FUSED_NV], accn = 0.0;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) acc[c] = 0.0;
+    if (nv <= 8) update_dot_body<8, 4>(w, V, stride, n, nv, hh, acc, accn);
+    else if (nv <= 16) update_dot_body<16, 2>(w, V, stride, n, nv, hh, acc, accn);
+    else update_dot_body<32, 1>(w, V, stride, n, nv, hh, acc, accn);
+    ud_finish<UD_THREADS>(acc, accn, nv, hh, st, partial);
+}
+
+// ---- the same pass with the basis chunk staged in shared memory by TMA bulk copies (cp.async.bulk +
+// mbarrier, three stages): the bytes in flight no longer depend on registers (two 72 KB stages per SM are
+// always outstanding), and both uses of the basis values (update, second projection) read shared memory.
+constexpr int UDT_THREADS = 256, UDT_STAGES = 3;
+constexpr int UDT_STAGE_DOUBLES = (8 + 1) * UDT_THREADS * 4;          // largest (NV + 1) * K over the three tilings
+constexpr size_t UDT_SMEM = (size_t)UDT_STAGES * UDT_STAGE_DOUBLES * sizeof(double) + 64;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    } while (!done);
+}
+
+template <int NV, int EPT>
+__device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
+                                                    int nv, const double* hh, double (&acc)[FUSED_NV], double& accn, double* stage0,
+                                                    uint64_t* bars) {
+    constexpr int K = UDT_THREADS * EPT;                    // elements per chunk
+    static_assert((NV + 1) * K <= UDT_STAGE_DOUBLES, "stage too small");
+    const int64_t nchunks = n / K;                          // n is a multiple of the tile size 2048
+    const int tid = threadIdx.x;
+    auto issue = [&](int64_t i) {                           // chunk i of this CTA -> stage i % STAGES
+        const int64_t ci = (int64_t)blockIdx.x + i * gridDim.x;
+        if (ci >= nchunks || tid != 0) return;
+        const int sg = (int)(i % UDT_STAGES);
+        double* sv = stage0 + (size_t)sg * UDT_STAGE_DOUBLES;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(&bars[sg], (uint32_t)((nv + 1) * K * sizeof(double)));
+        for (int c = 0; c < nv; c++) bulk_g2s(sv + c * K, V + (int64_t)c * stride + ci * K, K * sizeof(double), &bars[sg]);
+        bulk_g2s(sv + NV * K, w + ci * K, K * sizeof(double), &bars[sg]);
+    };
+    issue(0);
+    issue(1);
+    for (int64_t i = 0; (int64_t)blockIdx.x + i * gridDim.x < nchunks; i++) {
+        const int64_t ci = (int64_t)blockIdx.x + i * gridDim.x;
+        const int sg = (int)(i % UDT_STAGES);
+        const double* sv = stage0 + (size_t)sg * UDT_STAGE_DOUBLES;
+        mbar_wait(&bars[sg], (uint32_t)((i / UDT_STAGES) & 1));
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+            const int k = tid + e * UDT_THREADS;
+            double s = sv[NV * K + k];
+#pragma unroll
+            for (int c = 0; c < NV; c++)
+                if (c < nv) s -= hh[c] * sv[c * K + k];
+            w[ci * K + k] = s;
+            accn += s * s;
+#pragma unroll
+            for (int c = 0; c < NV; c++)
+                if (c < nv) acc[c] += s * sv[c * K + k];
+        }
+        __syncthreads();                                    // everyone is done with this stage and with stage (i + 2) % 3's old data
+        issue(i + 2);
+    }
+}
+
+__global__ void __launch_bounds__(UDT_THREADS, 1) k_update_dot_tma(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
+                                                                   int64_t n, GmresState* st, double* __restrict__ partial) {
+    extern __shared__ __align__(128) unsigned char udt_smem[];
+    __shared__ double hh[FUSED_NV];
+    if (st->cycle_end) return;
+    double* stage0 = reinterpret_cast<double*>(udt_smem);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(udt_smem + (size_t)UDT_STAGES * UDT_STAGE_DOUBLES * sizeof(double));
+    const int nv = st->j + 1;
+    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
+    if (threadIdx.x == 0) {
+        for (int sgi = 0; sgi < UDT_STAGES; sgi++) mbar_init(&bars[sgi], 1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    double acc[FUSED_NV], accn = 0.0;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) acc[c] = 0.0;
+    if (nv <= 8) update_dot_tma_body<8, 4>(w, V, stride, n, nv, hh, acc, accn, stage0, bars);
+    else if (nv <= 16) update_dot_tma_body<16, 2>(w, V, stride, n, nv, hh, acc, accn, stage0, bars);
+    else update_dot_tma_body<32, 1>(w, V, stride, n, nv, hh, acc, accn, stage0, bars);
+    ud_finish<UDT_THREADS>(acc, accn, nv, hh, st, partial);
+}
+
 template <int NV, int EPT>
 __device__ __forceinline__ void multidot_body(const double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
                                               int nv, double (&acc)[FUSED_NV]) {
@@ -431,7 +532,15 @@ void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride
     k_update_w<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
 }
 void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial) {
-    k_update_dot<<<UD_BLOCKS, UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial); count(L);
+    static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
+    static bool configured = false;
+    if (!no_tma && !configured) {
+        cudaFuncSetAttribute(k_update_dot_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UDT_SMEM);
+        configured = true;
+    }
+    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<148, UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
+    else k_update_dot<<<UD_BLOCKS, UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    count(L);
 }
 void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
     k_final_v<<<148 * 2, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
