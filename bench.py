@@ -37,10 +37,10 @@ WORKLOADS = {
     5: "configs[4]: D-shape 2049x2049 (~2.8M unknowns), 9 levels, time stepping",
 }
 # algorithmic bytes per point (SURVEY.md 8(d) / DESIGN.md section 6): one full RB-B GS sweep
-GS_BYTES_PER_POINT = 64.0
+ROOF_BYTES_PER_POINT = 2 * 64.0 + 61.0
 # DRAM bytes per launch of the roofline kernel (dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full
-# capture per config; profiles/r01d_gs_config4.md)
-GS_TRAFFIC_PER_LAUNCH = {4: 456.7e6}
+# capture per config; profiles/r01e_roofline_kernel_config4.md)
+ROOF_TRAFFIC_PER_LAUNCH = {4: 583.9e6}
 
 
 def peaks():
@@ -227,7 +227,7 @@ def run_ours(args):
         n0 = s.level_n(0)
         xs, bs = torch.randn(n0, dtype=torch.float64, device="cuda"), torch.randn(n0, dtype=torch.float64, device="cuda")
         for _ in range(4):
-            s.smooth(0, xs, bs, 2)
+            s.smooth_restrict(0, xs, bs, 2)
         torch.cuda.synchronize()
         s.close()
         return
@@ -243,31 +243,28 @@ def run_ours(args):
     ms_e_loc, outs_e, _, _, _ = timed(step_host, args.warmup, args.steps)
     ms_e2e, _, value_e2e = whole_job(ms_e_loc, float(pl.n) * sum(o[0] for o in outs_e), world, "cuda")
 
-    # ---- roofline of the dominant kernel, timed live with CUDA events on the launching stream: k_gs<2,0>, two
-    # fused red-black-boundary Gauss-Seidel sweeps on the finest level (x read), launched back to back
+    # ---- roofline of the dominant kernel (profiles/r01e_launches_config4.md): k_gs<2,false,true> on level 0, i.e.
+    # two fused red-black-boundary Gauss-Seidel sweeps + defect + full-weighting restriction in one launch.
+    # Timed live: CUDA events on the launching stream around exactly that launch (mg_last_step_ms).
     peak, peak_src = peaks()
     roof = None
     if rank == 0:
         n0 = s.level_n(0)
         xs, bs = torch.randn(n0, dtype=torch.float64, device="cuda"), torch.randn(n0, dtype=torch.float64, device="cuda")
-        def t_smooth(k, reps=5):
-            best = 1e30
-            for _ in range(reps):
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                torch.cuda.synchronize(); e0.record(); s.smooth(0, xs, bs, k); e1.record(); torch.cuda.synchronize()
-                best = min(best, e0.elapsed_time(e1))
-            return best
-        t_smooth(2, 2)
-        launches_gs = 8
-        per_launch_ms = (t_smooth(2 * launches_gs) - t_smooth(0)) / launches_gs     # mg_smooth(0 sweeps) = the two permutation kernels
-        alg = 2 * GS_BYTES_PER_POINT * n0
+        t = []
+        for _ in range(12):
+            s.smooth_restrict(0, xs, bs, 2)
+            t.append(s.last_step_ms)
+        per_launch_ms = float(np.median(t[2:]))
+        alg = ROOF_BYTES_PER_POINT * n0
         achieved = alg / (per_launch_ms * 1e-3) / 1e9
-        traffic = GS_TRAFFIC_PER_LAUNCH.get(args.config)
-        roof = {"bound": "hbm", "kernel": "k_gs<2,0> level 0: two fused RB-B Gauss-Seidel sweeps per launch", "achieved": achieved,
-                "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+        traffic = ROOF_TRAFFIC_PER_LAUNCH.get(args.config)
+        roof = {"bound": "hbm", "kernel": "k_gs<2,false,true> level 0: two fused RB-B Gauss-Seidel sweeps + defect + FW restriction per launch",
+                "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "algorithmic_bytes_per_launch": alg, "ms_per_launch": per_launch_ms,
-                "note": "algorithmic bytes = 64 B/pt per sweep of the three-loop formulation (SURVEY.md 8(d)); temporal blocking "
-                        "moves fewer (traffic, ncu), so frac can exceed 1; frac_of_traffic = traffic / time / peak",
+                "note": "algorithmic bytes = 2 x 64 B/pt (two sweeps of the three-loop formulation) + 61 B/pt (defect + restriction), "
+                        "SURVEY.md 8(d); temporal blocking and fusion move far fewer (traffic, ncu), so frac can exceed 1; "
+                        "frac_of_traffic = traffic / time / peak",
                 "frac_of_traffic": (traffic / (per_launch_ms * 1e-3) / 1e9 / peak) if traffic else None}
 
     cpu = None

@@ -131,6 +131,9 @@ int mg_level_coeffs(mg_handle h, int level, double* h_lambda, double* h_c, void*
 int mg_apply(mg_handle h, int level, const double* d_x, double* d_y, void* stream);            /* y = A x (D1-D3) */
 int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, void* stream); /* GS rbb        */
 int mg_restrict(mg_handle h, int level, const double* d_fine, double* d_coarse, void* stream);  /* rule T2        */
+/* The cycle's fused step: x <- S^sweeps x (sweeps >= 1), then d_coarse = R (A x - b) on level + 1,
+ * in one pass per two sweeps; this is the kernel bench.py reports its roofline for. */
+int mg_smooth_restrict(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, double* d_coarse, void* stream);
 int mg_prolong_correct(mg_handle h, int level, const double* d_coarse_e, double* d_x_fine, void* stream); /* T3   */
 int mg_coarse_solve(mg_handle h, const double* d_b, double* d_x, void* stream);                 /* rule C         */
 int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stream);
@@ -141,6 +144,9 @@ int64_t mg_kernel_launches(mg_handle h);
  * launching stream), in milliseconds; negative if not available. */
 double mg_last_solve_ms(mg_handle h);
 double mg_last_update_ms(mg_handle h);
+/* Device time of the smoothing kernels alone (without the in/out permutations) of the last mg_smooth or
+ * mg_smooth_restrict call, CUDA events on the launching stream; synchronises on the second event. */
+double mg_last_step_ms(mg_handle h);
 
 const char* mg_strerror(int code);
 const char* mg_last_error(void);

@@ -42,8 +42,8 @@ class _Options(C.Structure):
 
 EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_solve", "mg_update_coeffs_host",
            "mg_solve_host", "mg_destroy", "mg_num_levels", "mg_level_n", "mg_level_info", "mg_transfer_info",
-           "mg_level_coeffs", "mg_apply", "mg_smooth", "mg_restrict", "mg_prolong_correct", "mg_coarse_solve",
-           "mg_vcycle", "mg_kernel_launches", "mg_last_solve_ms", "mg_last_update_ms", "mg_strerror",
+           "mg_level_coeffs", "mg_apply", "mg_smooth", "mg_restrict", "mg_smooth_restrict", "mg_prolong_correct", "mg_coarse_solve",
+           "mg_vcycle", "mg_kernel_launches", "mg_last_solve_ms", "mg_last_update_ms", "mg_last_step_ms", "mg_strerror",
            "mg_last_error"]
 
 
@@ -61,6 +61,7 @@ def lib():
         L.mg_kernel_launches.restype = C.c_int64
         L.mg_last_solve_ms.restype = C.c_double
         L.mg_last_update_ms.restype = C.c_double
+        L.mg_last_step_ms.restype = C.c_double
         _lib = L
     return _lib
 
@@ -218,6 +219,13 @@ class Solver:
         self._call("mg_smooth", int(s), _dptr(x), _dptr(b), int(sweeps), _stream_ptr(stream))
         return x
 
+    def smooth_restrict(self, s, x, b, sweeps=2, stream=None):
+        import torch
+        x = x.clone()
+        dc = torch.empty(self.level_n(s + 1), dtype=torch.float64, device=x.device)
+        self._call("mg_smooth_restrict", int(s), _dptr(x), _dptr(b), int(sweeps), _dptr(dc), _stream_ptr(stream))
+        return x, dc
+
     def restrict(self, s, d, stream=None):
         import torch
         out = torch.empty(self.level_n(s + 1), dtype=torch.float64, device=d.device)
@@ -247,6 +255,10 @@ class Solver:
     @property
     def last_solve_ms(self):
         return float(lib().mg_last_solve_ms(self._h))
+
+    @property
+    def last_step_ms(self):
+        return float(lib().mg_last_step_ms(self._h))
 
     @property
     def last_update_ms(self):

@@ -73,9 +73,9 @@ struct mg_handle_s {
     cudaGraphExec_t iter_graph = nullptr;
     int64_t iter_graph_kernels = 0;
     int64_t launches = 0;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // solve, update, single step
     cudaEvent_t hev[2] = {nullptr, nullptr};   // header copies of the two Arnoldi steps in flight
-    bool solve_timed = false, update_timed = false;
+    bool solve_timed = false, update_timed = false, step_timed = false;
 };
 
 namespace {
@@ -467,6 +467,11 @@ double mg_last_solve_ms(mg_handle h) {
     if (!h || !h->solve_timed || cudaEventElapsedTime(&ms, h->ev[0], h->ev[1]) != cudaSuccess) { cudaGetLastError(); return -1.0; }
     return ms;
 }
+double mg_last_step_ms(mg_handle h) {
+    float ms = -1.f;
+    if (!h || !h->step_timed || cudaEventSynchronize(h->ev[5]) != cudaSuccess || cudaEventElapsedTime(&ms, h->ev[4], h->ev[5]) != cudaSuccess) { cudaGetLastError(); return -1.0; }
+    return ms;
+}
 double mg_last_update_ms(mg_handle h) {
     float ms = -1.f;
     if (!h || !h->update_timed || cudaEventSynchronize(h->ev[3]) != cudaSuccess || cudaEventElapsedTime(&ms, h->ev[2], h->ev[3]) != cudaSuccess) { cudaGetLastError(); return -1.0; }
@@ -600,8 +605,28 @@ int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps
     const int64_t n = h->hh.lev[level].n;
     launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
     launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    CU(cudaEventRecord(h->ev[4], L.stream));
     VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].tb), sweeps, false);
+    CU(cudaEventRecord(h->ev[5], L.stream));
+    h->step_timed = true;
     launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int mg_smooth_restrict(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, double* d_coarse, void* stream) {
+    CHECK_LEVEL(level >= 0 && level + 1 < h->L && d_x && d_b && d_coarse && sweeps >= 1);
+    Launch L = LZ(h, (cudaStream_t)stream);
+    const int64_t n = h->hh.lev[level].n;
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    CU(cudaEventRecord(h->ev[4], L.stream));
+    VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].tb), sweeps, false,
+                                &h->lev[level + 1], h->buf[level + 1].b);
+    CU(cudaEventRecord(h->ev[5], L.stream));
+    h->step_timed = true;
+    launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n);
+    launch_scatter(L, h->buf[level + 1].b, h->buf[level + 1].canon2slot, d_coarse, h->hh.lev[level + 1].n);
     CU(cudaGetLastError());
     return MG_OK;
 }

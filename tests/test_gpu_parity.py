@@ -102,6 +102,23 @@ def test_transfers(pair):
         assert rel(host(s.prolong_correct(lv, dev(ec), dev(x))), o.prolong_correct(lv, ec, x)) <= TOL_STEP
 
 
+def test_smooth_restrict_fused(pair):
+    """The cycle's fused step: sweeps, then the restricted defect of the result."""
+    pl, o, s = pair
+    rng = np.random.default_rng(6)
+    for lv in range(o.levels - 1):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        for sweeps in (1, 2, 3):
+            xo = o.smooth(lv, x, b, sweeps)
+            do = o.restrict(lv, o.apply(lv, xo) - b)
+            xg, dg = s.smooth_restrict(lv, dev(x), dev(b), sweeps)
+            assert rel(host(xg), xo) <= TOL_STEP
+            # d = A x - b is a difference of O(a_ll |x|) terms: 1e-13 relative to that scale
+            scale = np.linalg.norm(o.restrict(lv, np.abs(o.apply(lv, xo)) + np.abs(b)))
+            assert np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
+
+
 def test_coarse_solve(pair):
     pl, o, s = pair
     b = np.random.default_rng(4).standard_normal(o.level_n(o.levels - 1))
