@@ -301,7 +301,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
-    ap.add_argument("--ref-iters", type=int, default=2, help="iteration cap of the oracle sample")
+    ap.add_argument("--ref-iters", type=int, default=5, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
     args = ap.parse_args()
