@@ -294,6 +294,90 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_planes(args):
+    """several planes per GPU solved concurrently — one handle, one stream and one host thread per
+    plane (16 independent poloidal planes per time step).  Production planes have 1e5-2e6 points
+    (PAPER.md:256): alone they leave most of a B200 idle (latency bound), together they fill it.  Secondary bench line:
+    HBM-resident inputs only."""
+    import threading
+    import torch
+    import torch.distributed as dist
+    from paper_2509_11831_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.use_torch_allocator()
+    P = args.planes
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    streams = [torch.cuda.Stream() for _ in range(P)]
+    planes = [W.make_plane(args.config, seed=plane_seed(args.config, rank * P + p)) for p in range(P)]
+    solvers, data = [], []
+    for p, pl in enumerate(planes):
+        with torch.cuda.stream(streams[p]):
+            solvers.append(B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, stream=streams[p]))
+            data.append((dev(pl.lam), dev(pl.c), dev(pl.f), dev(pl.x0), torch.empty(pl.n, dtype=torch.float64, device="cuda")))
+    torch.cuda.synchronize()
+    iters = [[] for _ in range(P)]
+
+    def work(p, steps, keep):
+        lam, c, f, x0, x = data[p]
+        torch.cuda.set_device(local)
+        for _ in range(steps):
+            solvers[p].update_coeffs(lam, c, stream=streams[p])
+            _, it, rr, rc = solvers[p].solve(f, x0, RTOL, x=x, stream=streams[p])
+            if keep:
+                iters[p].append(it)
+
+    def round_(steps, keep):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ev0.record()
+        for st in streams:
+            st.wait_event(ev0)
+        th = [threading.Thread(target=work, args=(p, steps, keep)) for p in range(P)]
+        [t.start() for t in th]
+        [t.join() for t in th]
+        for st in streams:
+            torch.cuda.current_stream().wait_stream(st)
+        ev1.record()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        return ev0.elapsed_time(ev1)
+
+    l0 = sum(s.kernel_launches for s in solvers)
+    round_(args.warmup, False)
+    l1 = sum(s.kernel_launches for s in solvers)
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms_loc = round_(args.steps, True)
+    clocks = sampler.stop() if sampler else None
+    work_loc = float(sum(pl.n * sum(iters[p]) for p, pl in enumerate(planes)))
+    ms, work, value = whole_job(ms_loc, work_loc, world, "cuda")
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": WORKLOADS[args.config], "unknowns_per_plane": planes[0].n, "planes": P * world,
+                           "planes_per_gpu": P, "concurrency": "one handle + stream + host thread per plane", "rtol": RTOL,
+                           "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": solvers[0].levels,
+                           "step": "mg_update_coeffs + mg_solve on every plane"},
+                "iters": iters[0][-1], "ms_per_plane_solve": ms / args.steps / P, "clocks": clocks,
+                "gpu_launches": sum(s.kernel_launches for s in solvers) - l1, "e2e": None, "roofline": None, "cpu_baseline": None}
+        print(json.dumps(line))
+    for s in solvers:
+        s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -304,9 +388,12 @@ def main():
     ap.add_argument("--ref-iters", type=int, default=5, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
+    ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved concurrently (secondary line, SURVEY.md 8(f) NEXT-1)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.planes > 1:
+        run_planes(args)
     else:
         run_ours(args)
 

@@ -263,3 +263,43 @@ def test_full_size_config4_in_bench_configuration(gpu, oracle_mod):
     true = np.linalg.norm(fc - o.apply(0, xc)) / np.linalg.norm(fc)
     assert true < 1.05e-10 and relres == pytest.approx(true, rel=1e-2)
     s.close()
+
+
+def test_concurrent_planes_on_one_gpu(gpu, oracle_mod):
+    """SURVEY.md 8(f) NEXT-1 / PAPER.md:211, 320-324: poloidal planes are independent solves.  Several handles, each on
+    its own stream and driven by its own host thread, must give bit-identical results to solving one after another
+    (handles share no mutable state), and every one must match the oracle."""
+    import threading
+    import torch
+    P = 4
+    planes = [W.make_plane(2, 129, seed=W.SEEDS[2] + 31 * p) for p in range(P)]
+    streams = [torch.cuda.Stream() for _ in range(P)]
+    solvers, data = [], []
+    for p, pl in enumerate(planes):
+        with torch.cuda.stream(streams[p]):
+            solvers.append(gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, stream=streams[p]))
+            data.append((dev(pl.lam), dev(pl.c), dev(pl.f), dev(pl.x0)))
+    torch.cuda.synchronize()
+
+    def run(p, out):
+        lam, c, f, x0 = data[p]
+        for _ in range(3):
+            solvers[p].update_coeffs(lam, c, stream=streams[p])
+            x, iters, relres, rc = solvers[p].solve(f, x0, 1e-10, stream=streams[p])
+        streams[p].synchronize()
+        out[p] = (host(x), iters, rc)
+
+    seq, par = [None] * P, [None] * P
+    for p in range(P):
+        run(p, seq)
+    th = [threading.Thread(target=run, args=(p, par)) for p in range(P)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    for p, pl in enumerate(planes):
+        assert par[p][1:] == seq[p][1:] and np.array_equal(par[p][0], seq[p][0])
+        o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+        o.update(pl.lam, pl.c)
+        ro = o.solve(pl.f, pl.x0, 1e-10)
+        assert par[p][2] == 0 and abs(par[p][1] - ro["iters"]) <= 1 and rel(par[p][0], ro["x"]) <= TOL_SOLVE
+    for s in solvers:
+        s.close()
