@@ -303,3 +303,38 @@ def test_concurrent_planes_on_one_gpu(gpu, oracle_mod):
         assert par[p][2] == 0 and abs(par[p][1] - ro["iters"]) <= 1 and rel(par[p][0], ro["x"]) <= TOL_SOLVE
     for s in solvers:
         s.close()
+
+
+def test_solve_edge_cases(gpu, oracle_mod):
+    """Degenerate cases of rules K1-K5 through the C ABI: zero right-hand side, initial guess that already
+    solves the system, a one-level hierarchy (the cycle is the direct solve: one iteration), solve before
+    update, and aliasing of x with x0."""
+    import torch
+    pl = H.small_annulus(33, 2)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=2)
+    o.update(pl.lam, pl.c)
+    ro = o.solve(pl.f, pl.x0, 1e-12)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=2)
+    with pytest.raises(gpu.MgError) as e:
+        s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert e.value.code == -4                                   # MG_ENOTREADY
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    x, iters, relres, rc = s.solve(dev(np.zeros(pl.n)), dev(np.ones(pl.n)), 1e-10)
+    assert rc == 0 and iters == 0 and not host(x).any()         # K1: b = 0 -> x = 0
+    x, iters, relres, rc = s.solve(dev(pl.f), dev(ro["x"]), 1e-10)
+    assert rc == 0 and iters == 0 and rel(host(x), ro["x"]) == 0.0   # K1: x0 already converged
+    xa = dev(pl.x0)
+    _, iters, relres, rc = s.solve(dev(pl.f), xa, 1e-10, x=xa)   # x aliases x0
+    assert rc == 0 and abs(iters - o.solve(pl.f, pl.x0, 1e-10)["iters"]) <= 1 and rel(host(xa), ro["x"]) <= TOL_SOLVE
+    with pytest.raises(gpu.MgError):
+        s.solve(dev(pl.f), dev(pl.x0), 0.0)                     # rtol must be > 0
+    s.close()
+    pl1 = H.small_annulus(17, 1)
+    o1 = oracle_mod.Oracle(pl1.i, pl1.j, pl1.kind, pl1.h, levels=1)
+    o1.update(pl1.lam, pl1.c)
+    r1 = o1.solve(pl1.f, pl1.x0, 1e-10)
+    s1 = gpu.Solver(pl1.i, pl1.j, pl1.kind, pl1.h, levels=1)
+    s1.update_coeffs(dev(pl1.lam), dev(pl1.c))
+    x, iters, relres, rc = s1.solve(dev(pl1.f), dev(pl1.x0), 1e-10)
+    assert rc == 0 and iters == r1["iters"] == 1 and rel(host(x), r1["x"]) <= TOL_SOLVE
+    s1.close()
