@@ -130,8 +130,11 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
                                                   const uint16_t* __restrict__ ccode, double* __restrict__ dc, int bx0, int by0) {
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, ROUNDS = G::ROUNDS, BX = G::BW, BY = G::BH;
     const int tid = threadIdx.x;
+    // Interior tiles (no boundary phase): the black cells were updated last from the current red values, so
+    // their defect is zero up to rounding; only the red defects are formed and gathered.
+    constexpr int NCOL = GENERAL ? 2 : 1;
 #pragma unroll
-    for (int col = 0; col < 2; col++)
+    for (int col = 0; col < NCOL; col++)
 #pragma unroll
         for (int r = 0; r < ROUNDS; r++) {
             const int q = tid + r * GT;
@@ -153,7 +156,7 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
         }
     __syncthreads();
 #pragma unroll
-    for (int col = 0; col < 2; col++)
+    for (int col = 0; col < NCOL; col++)
 #pragma unroll
         for (int r = 0; r < ROUNDS; r++) {
             const int q = tid + r * GT;
@@ -172,6 +175,7 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
             for (int dy = -1; dy <= 1; dy++)
 #pragma unroll
                 for (int dx = -1; dx <= 1; dx++) {
+                    if (!GENERAL && ((dx + dy) & 1)) continue;      // black neighbours of a (red) coarse point: zero
                     const double w = (dx == 0 ? 2.0 : 1.0) * (dy == 0 ? 2.0 : 1.0) * 0.0625;
                     acc += w * sc[cidx<G>(rx + dx, ry + dy)];
                 }
