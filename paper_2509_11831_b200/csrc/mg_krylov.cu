@@ -320,7 +320,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     } while (!done);
 }
 
-template <int NV, int EPT>
+// UPDATE = false: pass 1 only (acc = V^T w; w untouched, hh unused).
+template <int NV, int EPT, bool UPDATE = true>
 __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
                                                     int nv, const double* hh, double (&acc)[FUSED_NV], double& accn, double* stage0,
                                                     uint64_t* bars) {
@@ -349,11 +350,13 @@ __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, cons
         for (int e = 0; e < EPT; e++) {
             const int k = tid + e * UDT_THREADS;
             double s = sv[NV * K + k];
+            if (UPDATE) {
 #pragma unroll
-            for (int c = 0; c < NV; c++)
-                if (c < nv) s -= hh[c] * sv[c * K + k];
-            w[ci * K + k] = s;
-            accn += s * s;
+                for (int c = 0; c < NV; c++)
+                    if (c < nv) s -= hh[c] * sv[c * K + k];
+                w[ci * K + k] = s;
+                accn += s * s;
+            }
 #pragma unroll
             for (int c = 0; c < NV; c++)
                 if (c < nv) acc[c] += s * sv[c * K + k];
@@ -429,6 +432,47 @@ __global__ void __launch_bounds__(MD_THREADS, 2) k_multidot_t(const double* __re
     if (threadIdx.x < FUSED_NV) {
         double r = 0.0;
         for (int q = 0; q < MD_THREADS / 32; q++) r += red[q][threadIdx.x];
+        partial[(size_t)blockIdx.x * (MAX_M + 2) + threadIdx.x] = r;
+    }
+    if (last_block(st)) {
+        if ((int)threadIdx.x < nv) {
+            double r = 0.0;
+            for (int b = 0; b < (int)gridDim.x; b++) r += ((volatile double*)partial)[(size_t)b * (MAX_M + 2) + threadIdx.x];
+            st->red[threadIdx.x] = r;
+        }
+    }
+}
+
+// Pass 1 through the same TMA pipeline.
+__global__ void __launch_bounds__(UDT_THREADS, 1) k_multidot_tma(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
+                                                                 int64_t n, GmresState* st, double* __restrict__ partial) {
+    extern __shared__ __align__(128) unsigned char udt_smem[];
+    __shared__ double red[UDT_THREADS / 32][FUSED_NV];
+    if (st->cycle_end) return;
+    double* stage0 = reinterpret_cast<double*>(udt_smem);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(udt_smem + (size_t)UDT_STAGES * UDT_STAGE_DOUBLES * sizeof(double));
+    const int nv = st->j + 1;
+    if (threadIdx.x == 0) {
+        for (int sgi = 0; sgi < UDT_STAGES; sgi++) mbar_init(&bars[sgi], 1);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    double acc[FUSED_NV], accn = 0.0;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) acc[c] = 0.0;
+    if (nv <= 8) update_dot_tma_body<8, 4, false>(w, V, stride, n, nv, nullptr, acc, accn, stage0, bars);
+    else if (nv <= 16) update_dot_tma_body<16, 2, false>(w, V, stride, n, nv, nullptr, acc, accn, stage0, bars);
+    else update_dot_tma_body<32, 1, false>(w, V, stride, n, nv, nullptr, acc, accn, stage0, bars);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int c = 0; c < FUSED_NV; c++) {
+        const double r = warp_sum(acc[c]);
+        if (lane == 0) red[warp][c] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < FUSED_NV) {
+        double r = 0.0;
+        for (int q = 0; q < UDT_THREADS / 32; q++) r += red[q][threadIdx.x];
         partial[(size_t)blockIdx.x * (MAX_M + 2) + threadIdx.x] = r;
     }
     if (last_block(st)) {
@@ -524,7 +568,15 @@ void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double
     k_start_cycle<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
 }
 void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int m) {
-    if (m <= FUSED_NV) k_multidot_t<<<148 * 2, MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
+    static bool configured = false;
+    if (!no_tma && !configured) {
+        cudaFuncSetAttribute(k_multidot_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UDT_SMEM);
+        configured = true;
+    }
+    if (m <= FUSED_NV && !no_tma && n % (UDT_THREADS * 4) == 0)
+        k_multidot_tma<<<148, UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
+    else if (m <= FUSED_NV) k_multidot_t<<<148 * 2, MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     else k_multidot<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
 }
