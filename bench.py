@@ -40,7 +40,7 @@ WORKLOADS = {
 ROOF_BYTES_PER_POINT = 2 * 64.0 + 61.0
 # DRAM bytes per launch of the roofline kernel (dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full
 # capture per config; profiles/r01e_roofline_kernel_config4.md)
-ROOF_TRAFFIC_PER_LAUNCH = {4: 583.9e6}
+ROOF_TRAFFIC_PER_LAUNCH = {4: 582.5e6}
 
 
 def peaks():
