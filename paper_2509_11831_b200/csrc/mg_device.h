@@ -146,6 +146,5 @@ void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride,
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st);
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol);
-void launch_final_check(const Launch& L, GmresState* st);
 
 }  // namespace mgb

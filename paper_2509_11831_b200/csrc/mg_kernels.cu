@@ -1,7 +1,9 @@
-// Tile kernels of the multigrid hierarchy (sm_100a): operator apply / residual (S1), red-black-boundary
-// Gauss-Seidel (S2), full-weighting restriction (S3), bilinear prolongation + set_bnds_hom + correction
-// (S4), coefficient restriction (U1).  One CTA per active tile; halo values come from the neighbour
-// tiles through the per-tile 3x3 table (missing tiles map to the all-absent null tile).
+// Tile kernels of the multigrid hierarchy (sm_100a) other than the smoother: operator apply / residual (S1),
+// the unfused transfers used by the single-step entry points and by cycles with nu_pre = 0 or nu_post = 0
+// (defect + restriction S1+S3, restriction S3, prolongation + set_bnds_hom + correction S4), coefficient
+// restriction (U1), diagonal (U2), permutations (B1).  One CTA per active tile; halo values come from the
+// neighbour tiles through the per-tile 3x3 table (missing tiles map to the all-absent null tile).  Inside the
+// cycle S3 and S4 are fused into the smoother launches (mg_tile_gs.cuh).
 #include "mg_tile_ops.cuh"
 
 #include <algorithm>

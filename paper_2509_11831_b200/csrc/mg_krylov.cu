@@ -4,10 +4,12 @@
 // on the device in GmresState; every kernel reads the running column index j from it, so one captured
 // graph serves all iterations.
 //
-// Orthogonalisation: classical Gram-Schmidt applied twice (CGS2): fused multi-dot (one pass over w and
-// v_0..v_j), fused update + norm; twice.  Same Krylov iterates as the oracle's modified Gram-Schmidt up
-// to rounding.  Grid reductions: per-block partials + last-block-done ticket, summed in a fixed order
-// (deterministic run to run).
+// Orthogonalisation: classical Gram-Schmidt applied twice (CGS2).  Same Krylov iterates as the oracle's modified
+// Gram-Schmidt (also applied twice) up to rounding.  For restart lengths m <= 32 the two projections take
+// THREE passes over the basis (k_multidot_tma, k_update_dot_tma, k_final_v: see the block comment further down),
+// the first two staged through shared memory by TMA bulk copies; longer restarts use the plain four-pass
+// form (k_multidot, k_update_w twice, k_givens, k_next_v).  Grid reductions: per-block partials +
+// last-block-done ticket, summed in a fixed order (deterministic run to run).
 #include <cstdlib>
 
 #include "mg_device.h"
@@ -85,8 +87,6 @@ __global__ void k_start_cycle(GmresState* st, const double* __restrict__ r, doub
         for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) V0[k] = r[k] * inv;
     }
     // the header is rewritten by one thread after every block has read it
-    __shared__ int dummy;
-    (void)dummy;
     if (last_block(st) && threadIdx.x == 0) {
         st->relres = relres;
         if (bn == 0.0) { st->status = 4; st->cycle_end = 1; }           // zero right-hand side: x = 0 (K1)
@@ -607,6 +607,5 @@ void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol) {
     k_init_state<<<1, 32, 0, L.stream>>>(st, m, max_iters, rtol); count(L);
 }
-void launch_final_check(const Launch&, GmresState*) {}
 
 }  // namespace mgb
