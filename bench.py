@@ -151,11 +151,11 @@ def whole_job(ms_local, unknown_iters_local, world, device):
     return ms, work, work / (ms * 1e-3)
 
 
-def make_steps(cfg, rank, nsteps):
+def make_steps(cfg, rank, nsteps, lattice=None):
     """Inputs of `nsteps` consecutive steps.  Configs 1-4: the same plane every step (x0 = 0).
     Config 5: the time-stepping sequence of BASELINE.json configs[4] (coefficients and right-hand side
     perturbed every step, warm start from the previous solution)."""
-    pl = W.make_plane(cfg, seed=plane_seed(cfg, rank))
+    pl = W.make_plane(cfg, lattice, seed=plane_seed(cfg, rank))
     if cfg != 5:
         return pl, [pl] * nsteps, False
     seq, cur = [pl], pl
@@ -181,7 +181,7 @@ def run_ours(args):
     B.use_torch_allocator()
 
     nsteps = args.warmup + args.steps
-    pl, seq, warm = make_steps(args.config, rank, nsteps)
+    pl, seq, warm = make_steps(args.config, rank, nsteps, args.lattice)
     uniq = seq if warm else seq[:1]
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -258,7 +258,7 @@ def run_ours(args):
         per_launch_ms = float(np.median(t[2:]))
         alg = ROOF_BYTES_PER_POINT * n0
         achieved = alg / (per_launch_ms * 1e-3) / 1e9
-        traffic = ROOF_TRAFFIC_PER_LAUNCH.get(args.config)
+        traffic = ROOF_TRAFFIC_PER_LAUNCH.get(args.config) if args.lattice is None else None
         roof = {"bound": "hbm", "kernel": "k_gs<2,false,true> level 0: two fused RB-B Gauss-Seidel sweeps + defect + FW restriction per launch",
                 "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "algorithmic_bytes_per_launch": alg, "ms_per_launch": per_launch_ms,
@@ -277,7 +277,8 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": WORKLOADS[args.config], "unknowns_per_plane": pl.n, "planes": world, "rtol": RTOL,
+                "config": {"workload": WORKLOADS[args.config] + (f" [geometry on a {args.lattice}^2 lattice]" if args.lattice else ""),
+                           "unknowns_per_plane": pl.n, "planes": world, "rtol": RTOL,
                            "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels,
                            "step": "mg_update_coeffs + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
                            "l2_policy": "inputs larger than L2 (no flush)" if pl.n * 8 * 8 > 126e6 else "working set fits L2 (small config)"},
@@ -388,6 +389,7 @@ def main():
     ap.add_argument("--ref-iters", type=int, default=5, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
+    ap.add_argument("--lattice", type=int, default=None, help="same geometry on an n x n lattice (2^k + 1; O(N) scaling runs)")
     ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved concurrently (secondary line, SURVEY.md 8(f) NEXT-1)")
     args = ap.parse_args()
     if args.impl == "reference":
