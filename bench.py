@@ -126,7 +126,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "unknowns": pl.n, "rtol": RTOL, "cycle": "V(2,2)", "restart_m": 30},
+            "config": {"workload": WORKLOADS[args.config], "unknowns_per_plane": pl.n, "planes": 1, "rtol": RTOL,
+                       "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": pl.levels, "step": "mg_update_coeffs + mg_solve (oracle, bounded sample)"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -386,7 +387,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
-    ap.add_argument("--ref-iters", type=int, default=5, help="iteration cap of the oracle sample")
+    ap.add_argument("--ref-iters", type=int, default=8, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
     ap.add_argument("--lattice", type=int, default=None, help="same geometry on an n x n lattice (2^k + 1; O(N) scaling runs)")
