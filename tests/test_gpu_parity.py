@@ -338,3 +338,40 @@ def test_solve_edge_cases(gpu, oracle_mod):
     x, iters, relres, rc = s1.solve(dev(pl1.f), dev(pl1.x0), 1e-10)
     assert rc == 0 and iters == r1["iters"] == 1 and rel(host(x), r1["x"]) <= TOL_SOLVE
     s1.close()
+
+
+def test_guard_list_overflow_path(gpu, oracle_mod):
+    """A mesh whose every other lattice row consists of guard points (valid under rule M2: each is 4-adjacent to an
+    inner point): far more than 512 guards fall into one smoother region, so the per-CTA guard list overflows
+    and the boundary phase falls back to scanning the owned cells.  Mixed Dirichlet / Neumann guards."""
+    n = 833                                           # 14 x 27 tiles: above the block tiers, whole-tile CTAs
+    inner = np.zeros((n, n), bool)
+    inner[2:-2:2, 2:-2] = True                        # inner rows 2, 4, ..., separated by guard rows
+    yy, xx = np.mgrid[0:n, 0:n]
+    neu = (xx > n // 2)                               # guards in the right half are Neumann
+    rng = np.random.default_rng(17)
+    lam = 0.5 + rng.uniform(0, 1, (n, n))
+    c = np.exp(0.3 * rng.standard_normal((n, n)))
+    f = rng.standard_normal((n, n))
+    pl = W.mask_plane(inner, neu, 1.0 / (n - 1), lam, c, f, levels=7)
+    assert (pl.kind != 0).sum() > 300000
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=7)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=7)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    for lv in range(7):
+        a, g = o.level_arrays(lv), s.level_info(lv)
+        for k in ("I", "J", "kind", "colour", "nbr", "ns_fallback"):
+            assert np.array_equal(a[k], g[k])
+    nn = o.level_n(0)
+    x, b = rng.standard_normal(nn), rng.standard_normal(nn)
+    assert rel(host(s.apply(0, dev(x))), o.apply(0, x)) <= TOL_STEP
+    for sweeps in (1, 2, 3):
+        assert rel(host(s.smooth(0, dev(x), dev(b), sweeps)), o.smooth(0, x, b, sweeps)) <= TOL_STEP
+    xo = o.smooth(0, x, b, 2)
+    xg, dg = s.smooth_restrict(0, dev(x), dev(b), 2)
+    do = o.restrict(0, o.apply(0, xo) - b)
+    scale = np.linalg.norm(o.restrict(0, np.abs(o.apply(0, xo)) + np.abs(b)))
+    assert rel(host(xg), xo) <= TOL_STEP and np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    s.close()
