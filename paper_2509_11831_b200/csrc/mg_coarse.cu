@@ -66,12 +66,21 @@ __global__ void k_coarse_assemble(LevelDev lv, const int32_t* __restrict__ cslot
 }
 
 // In-place Gauss-Jordan with partial pivoting (first maximum wins ties) on W = [A | I] -> [I | A^-1].
-__global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict__ W, double* __restrict__ Ainv) {
+// One CTA; when [A | I] fits (n <= ~110) it is worked on in shared memory, so a pivot step costs three
+// barriers instead of three global-memory round trips.
+__global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict__ Wg, double* __restrict__ Ainv, int in_smem) {
+    extern __shared__ __align__(16) double wsm[];
     __shared__ double fac[1024];
     __shared__ double redv[CT / 32];
     __shared__ int redi[CT / 32];
     __shared__ int piv;
     const int tid = threadIdx.x, n2 = 2 * n;
+    double* W = Wg;
+    if (in_smem) {
+        for (int e = tid; e < n * n2; e += CT) wsm[e] = Wg[e];
+        W = wsm;
+        __syncthreads();
+    }
     for (int k = 0; k < n; k++) {
         // pivot search over rows k..n-1 of column k
         double best = -1.0; int bi = n;
@@ -139,7 +148,14 @@ __global__ void __launch_bounds__(CT) k_coarse_solve(const double* __restrict__ 
 void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
                           double* work, double* Ainv) {
     k_coarse_assemble<<<(n + 127) / 128, 128, 0, L.stream>>>(lv, cslot, slot2row, n, work);
-    k_coarse_invert<<<1, CT, 0, L.stream>>>(n, work, Ainv);
+    const size_t wbytes = (size_t)n * 2 * n * sizeof(double);
+    const int in_smem = wbytes <= 200 * 1024;
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_coarse_invert, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        configured = true;
+    }
+    k_coarse_invert<<<1, CT, in_smem ? wbytes : 0, L.stream>>>(n, work, Ainv, in_smem);
     if (L.counter) *L.counter += 2;
 }
 
