@@ -339,8 +339,7 @@ __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, cons
         for (int c = 0; c < nv; c++) bulk_g2s(sv + c * K, V + (int64_t)c * stride + ci * K, K * sizeof(double), &bars[sg]);
         bulk_g2s(sv + NV * K, w + ci * K, K * sizeof(double), &bars[sg]);
     };
-    issue(0);
-    issue(1);
+    for (int i = 0; i < UDT_STAGES; i++) issue(i);           // all stages in flight; a stage is refilled as soon as it is consumed
     for (int64_t i = 0; (int64_t)blockIdx.x + i * gridDim.x < nchunks; i++) {
         const int64_t ci = (int64_t)blockIdx.x + i * gridDim.x;
         const int sg = (int)(i % UDT_STAGES);
@@ -361,8 +360,8 @@ __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, cons
             for (int c = 0; c < NV; c++)
                 if (c < nv) acc[c] += s * sv[c * K + k];
         }
-        __syncthreads();                                    // everyone is done with this stage and with stage (i + 2) % 3's old data
-        issue(i + 2);
+        __syncthreads();                                    // everyone is done with this stage: refill it
+        issue(i + UDT_STAGES);
     }
 }
 
