@@ -261,7 +261,9 @@ def test_full_size_config4_in_bench_configuration(gpu, oracle_mod):
     assert rc == 0 and relres < 1e-10 and 20 <= iters <= 60
     xc, fc = H.canon(o, host(x)), H.canon(o, pl.f)
     true = np.linalg.norm(fc - o.apply(0, xc)) / np.linalg.norm(fc)
-    assert true < 1.05e-10 and relres == pytest.approx(true, rel=1e-2)
+    # at 1e-10 the residual itself carries rounding noise of order eps * a_ll |x| / |f| ~ 1e-12: two evaluations
+    # (tile kernel vs oracle loop) agree to a few per cent, not to 1e-3
+    assert true < 1.05e-10 and relres == pytest.approx(true, rel=5e-2)
     s.close()
 
 
