@@ -536,13 +536,15 @@ void orc_transfer_tables(void* h, int s, int32_t* fine9, int32_t* parent, double
 }
 
 // "update": coefficients in USER order on all points; T4 to all coarser levels;
-// LU-factorise the coarsest operator.  Returns 0, or -1 if a coefficient is not admissible,
+// LU-factorise the coarsest operator.  Returns 0, or -1 if a coefficient is not admissible (c <= 0 or non-finite),
 // -2 if the coarsest matrix is singular.
 int orc_update(void* h, const double* lam, const double* c) {
     Oracle* o = (Oracle*)h;
     Level& l0 = o->lev[0];
     for (int64_t k = 0; k < l0.n; k++) {
-        if (!(c[k] > 0.0) || !(lam[k] >= 0.0) || !std::isfinite(c[k]) || !std::isfinite(lam[k])) { g_err = "need c>0, lambda>=0"; return -1; }
+        // c > 0 is required; lambda >= 0 is only the paper's sufficient condition for positive definiteness and its own
+        // verification case has lambda = r sin(theta) of both signs (Eq. 21), so lambda is only required to be finite
+        if (!(c[k] > 0.0) || !std::isfinite(c[k]) || !std::isfinite(lam[k])) { g_err = "need c>0 and finite lambda"; return -1; }
         l0.lam[o->user2canon[k]] = lam[k];
         l0.c[o->user2canon[k]] = c[k];
     }

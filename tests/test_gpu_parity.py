@@ -377,3 +377,31 @@ def test_guard_list_overflow_path(gpu, oracle_mod):
     assert rel(host(xg), xo) <= TOL_STEP and np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
     assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
     s.close()
+
+
+@pytest.mark.parametrize("neumann", [False, True])
+def test_paper_annulus_mms_v55(gpu, oracle_mod, neumann):
+    """The paper's own verification case (Eq. 19-22: lambda of both signs, V(5,5)) on the GPU path:
+    parity with the oracle, and the discretisation error against the manufactured solution is the oracle's."""
+    from tests.test_oracle_paper_mms import discrete_offsets
+    h, levels = 2e-3, 5
+    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
+    f = pl.f
+    if neumann:
+        oR, oZ = discrete_offsets(o.level_arrays(0), pl.n)
+        f = W.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
+    o.update(pl.lam, pl.c)
+    ro = o.solve(f, pl.x0, 1e-10)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    rng = np.random.default_rng(9)
+    n0 = o.level_n(0)
+    x, b = rng.standard_normal(n0), rng.standard_normal(n0)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    xg, iters, relres, rc = s.solve(dev(f), dev(pl.x0), 1e-10)
+    assert rc == 0 and ro["status"] == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
+    m = pl.kind == 0
+    err = np.linalg.norm(host(xg)[m] - pl.meta["phi"][m]) / np.linalg.norm(pl.meta["phi"][m])
+    assert err < (1.2e-2 if neumann else 1e-4)              # O(h) / O(h^2) at h = 2e-3 (PAPER.md:274)
+    s.close()
