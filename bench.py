@@ -380,6 +380,48 @@ def run_planes(args):
         dist.destroy_process_group()
 
 
+def run_paper_mms(args):
+    """The paper's own scaling experiment: annulus of Eq. 19-22, h halved from 4e-3 with one more
+    level per refinement (4 ... 9 levels, N = 2.4e4 ... 2.4e7), V-cycle with five pre- and post-smoothing sweeps, stop at 1e-8,
+    Dirichlet or Neumann conditions on the inner circle.  One JSON line per case: iterations, update / solve time (CUDA
+    events), error against the manufactured solution.  Context for BASELINE.md, not the headline metric."""
+    import torch
+    from paper_2509_11831_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    B.use_torch_allocator()
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for k in range(args.paper_mms):
+        h, levels = 4e-3 / 2 ** k, 4 + k
+        for neumann in (False, True):
+            pl = W.make_paper_annulus(h, levels, neumann_inner=neumann)
+            s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
+            f = pl.f
+            if neumann:
+                lv = s.level_info(0)
+                oR, oZ = W.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
+                f = W.neumann_gamma(pl, oR[lv["user2canon"]], oZ[lv["user2canon"]])
+            d_lam, d_c, d_f, d_x0 = dev(pl.lam), dev(pl.c), dev(f), dev(pl.x0)
+            sol, upd = [], []
+            for _ in range(args.warmup + args.steps):
+                s.update_coeffs(d_lam, d_c)
+                x, iters, relres, rc = s.solve(d_f, d_x0, 1e-8)
+                sol.append(s.last_solve_ms); upd.append(s.last_update_ms)
+            m = pl.kind == 0
+            e = x.cpu().numpy()[m] - pl.meta["phi"][m]
+            print(json.dumps({"workload": "PAPER.md Eq. 19-22 annulus MMS, V(5,5), rtol 1e-8", "h": h, "levels": levels,
+                              "inner_bc": "neumann" if neumann else "dirichlet", "points": pl.n, "iters": iters, "status": rc,
+                              "final_relres": relres, "solve_ms": float(np.median(sol[args.warmup:])),
+                              "update_ms": float(np.median(upd[args.warmup:])),
+                              "unknown_iters_per_s": pl.n * iters / (float(np.median(sol[args.warmup:])) * 1e-3),
+                              "err_l2": float(np.linalg.norm(e) / np.linalg.norm(pl.meta["phi"][m])), "err_linf": float(np.abs(e).max())}),
+                  flush=True)
+            s.close()
+            del d_lam, d_c, d_f, d_x0, x
+            torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -391,10 +433,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
     ap.add_argument("--lattice", type=int, default=None, help="same geometry on an n x n lattice (2^k + 1; O(N) scaling runs)")
+    ap.add_argument("--paper-mms", type=int, default=0, metavar="R",
+                    help="run the paper's annulus MMS scaling experiment over R refinements (6 reaches its 24 M points) instead")
     ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved concurrently (secondary line, SURVEY.md 8(f) NEXT-1)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.paper_mms > 0:
+        run_paper_mms(args)
     elif args.planes > 1:
         run_planes(args)
     else:

@@ -344,7 +344,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         for (int r = 0; r < h->nL; r++) s2r[cl.canon2slot[r]] = r;
         h->cslot = h->buf[h->L - 1].canon2slot;
         TRY(upload(h, &h->slot2row, s2r, s));
-        TRY(dev_alloc(h, (void**)&h->cwork, sizeof(double) * 2 * (size_t)h->nL * h->nL, s));
+        TRY(dev_alloc(h, (void**)&h->cwork, sizeof(double) * (2 * (size_t)h->nL * h->nL + 2 * (size_t)h->nL + 2), s));   // [A | I] + published column (x2) + pivots
         TRY(dev_alloc(h, (void**)&h->Ainv, sizeof(double) * (size_t)h->nL * h->nL, s));
     }
     CUF(cudaStreamSynchronize(s));

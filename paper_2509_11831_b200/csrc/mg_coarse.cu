@@ -2,6 +2,10 @@
 // coarsest matrix on the CPU at every update and round-trips the right-hand side at every cycle
 // (PAPER.md:217); here the dense operator is assembled, inverted (Gauss-Jordan with partial pivoting,
 // one CTA) at update time, and the cycle applies the inverse with one small kernel: no host step.
+#include <cooperative_groups.h>
+
+#include <algorithm>
+
 #include "mg_device.h"
 
 namespace mgb {
@@ -125,6 +129,75 @@ __global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict_
     for (int e = tid; e < n * n; e += CT) Ainv[e] = W[(size_t)(e / n) * n2 + n + (e % n)];
 }
 
+// The same elimination for coarsest levels that do not fit one CTA's shared memory (n > ~110; the paper keeps
+// ~400 points on its coarsest level): a cooperative grid in which every CTA owns a slab of COLUMNS of
+// [A | I] in shared memory for the whole elimination.  A pivot step needs only column k and the pivot index
+// from the CTA that owns column k: it publishes them (double-buffered) before the one grid barrier of the
+// step.  Same arithmetic and pivot rule as k_coarse_invert.
+constexpr int CIT = 256;
+__global__ void __launch_bounds__(CIT) k_coarse_invert_coop(int n, int cpb, const double* __restrict__ Wg, double* __restrict__ Ainv,
+                                                            double* colbuf, int* pivbuf) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    extern __shared__ __align__(16) double csm[];
+    double* sc = csm;                       // [cpb][n], column-major slab
+    double* fac = sc + (size_t)cpb * n;     // column k as published
+    double* rowk = fac + n;                 // [cpb] scaled pivot-row entries of the own columns
+    double* oldk = rowk + cpb;              // [cpb] row-k entries before the swap
+    __shared__ double redv[CIT / 32];
+    __shared__ int redi[CIT / 32];
+    const int tid = threadIdx.x, n2 = 2 * n;
+    const int c0 = blockIdx.x * cpb, nc = max(0, min(cpb, n2 - c0));
+    for (int e = tid; e < nc * n; e += CIT) { const int c = e / n, r = e - c * n; sc[e] = Wg[(size_t)r * n2 + c0 + c]; }
+    __syncthreads();
+    auto publish = [&](int k) {             // called by every thread of the CTA that owns column k
+        const double* col = sc + (size_t)(k - c0) * n;
+        double best = -1.0; int bi = n;
+        for (int r = k + tid; r < n; r += CIT) { const double v = fabs(col[r]); if (v > best) { best = v; bi = r; } }
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_down_sync(0xffffffffu, best, o);
+            const int oi = __shfl_down_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if ((tid & 31) == 0) { redv[tid >> 5] = best; redi[tid >> 5] = bi; }
+        __syncthreads();
+        if (tid == 0) {
+            double b = redv[0]; int i = redi[0];
+            for (int w = 1; w < CIT / 32; w++)
+                if (redv[w] > b || (redv[w] == b && redi[w] < i)) { b = redv[w]; i = redi[w]; }
+            pivbuf[k & 1] = i;
+        }
+        for (int r = tid; r < n; r += CIT) colbuf[(size_t)(k & 1) * n + r] = col[r];
+        __syncthreads();
+    };
+    if (0 >= c0 && 0 < c0 + nc) publish(0);
+    grid.sync();
+    for (int k = 0; k < n; k++) {
+        for (int r = tid; r < n; r += CIT) fac[r] = __ldcg(colbuf + (size_t)(k & 1) * n + r);
+        const int p = __ldcg(pivbuf + (k & 1));
+        __syncthreads();
+        const double inv = 1.0 / fac[p];
+        const double fk = fac[k];           // after the swap this is the column-k entry of row p
+        if (tid < nc) { oldk[tid] = sc[(size_t)tid * n + k]; rowk[tid] = sc[(size_t)tid * n + p] * inv; }
+        __syncthreads();
+        for (int e = tid; e < nc * n; e += CIT) {
+            const int c = e / n, r = e - c * n;
+            double v;
+            if (r == k) v = rowk[c];
+            else if (r == p) v = (fk != 0.0) ? oldk[c] - fk * rowk[c] : oldk[c];
+            else { const double f = fac[r]; v = (f != 0.0) ? sc[e] - f * rowk[c] : sc[e]; }
+            sc[e] = v;
+        }
+        __syncthreads();
+        if (k + 1 < n && k + 1 >= c0 && k + 1 < c0 + nc) publish(k + 1);
+        grid.sync();
+    }
+    for (int e = tid; e < nc * n; e += CIT) {
+        const int c = e / n, r = e - c * n;
+        if (c0 + c >= n) Ainv[(size_t)r * n + (c0 + c - n)] = sc[e];
+    }
+}
+
 // x = A^-1 b on the coarsest level; vectors in the tile layout, rows addressed through cslot.
 __global__ void __launch_bounds__(CT) k_coarse_solve(const double* __restrict__ Ainv, const int32_t* __restrict__ cslot, int n,
                                                      VecRef br, VecRef xr, const int* __restrict__ stop) {
@@ -151,9 +224,31 @@ void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cs
     const size_t wbytes = (size_t)n * 2 * n * sizeof(double);
     const int in_smem = wbytes <= 200 * 1024;
     static bool configured = false;
+    static int coop_sms = 0;
     if (!configured) {
         cudaFuncSetAttribute(k_coarse_invert, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_coarse_invert_coop, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        int dev = 0, coop = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        coop_sms = coop ? sms : 0;
         configured = true;
+    }
+    if (!in_smem && coop_sms > 0) {                           // column slabs over a cooperative grid
+        int G = std::min(coop_sms, (2 * n + 3) / 4);
+        int cpb = (2 * n + G - 1) / G;
+        G = (2 * n + cpb - 1) / cpb;
+        const size_t smem = ((size_t)cpb * n + n + 2 * (size_t)cpb) * sizeof(double);
+        if (smem <= 200 * 1024) {
+            double* colbuf = work + (size_t)2 * n * n;        // 2 n doubles + 2 ints behind [A | I] (allocated by mg_setup)
+            int* pivbuf = reinterpret_cast<int*>(colbuf + 2 * n);
+            const double* Wg = work;
+            void* args[] = {(void*)&n, (void*)&cpb, (void*)&Wg, (void*)&Ainv, (void*)&colbuf, (void*)&pivbuf};
+            cudaLaunchCooperativeKernel((const void*)k_coarse_invert_coop, dim3(G), dim3(CIT), args, smem, L.stream);
+            if (L.counter) *L.counter += 2;
+            return;
+        }
     }
     k_coarse_invert<<<1, CT, in_smem ? wbytes : 0, L.stream>>>(n, work, Ainv, in_smem);
     if (L.counter) *L.counter += 2;

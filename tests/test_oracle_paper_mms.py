@@ -15,18 +15,7 @@ H0 = 4e-3
 
 
 def discrete_offsets(lv, n):
-    """Offset (in units of h) from every Neumann guard to the point where rule D3 evaluates the upstream value, from
-    the mesh classification alone: n/|n| (Eq. 13), or the mean offset of the inner 4-neighbours for the fallback."""
-    oR, oZ = np.zeros(n), np.zeros(n)
-    tn = lv["ns_tn"].astype(float) / 2.0
-    nrm = np.hypot(tn[:, 0], tn[:, 1])
-    reg = (lv["kind"] == 2) & (lv["ns_fallback"] == 0)
-    oR[reg], oZ[reg] = tn[reg, 0] / nrm[reg], tn[reg, 1] / nrm[reg]
-    D = [(-1, 0), (1, 0), (0, -1), (0, 1)]
-    for l in np.nonzero((lv["kind"] == 2) & (lv["ns_fallback"] == 1))[0]:
-        nb = [d for d, q in zip(D, lv["nbr"][l]) if q >= 0 and lv["kind"][q] == 0]
-        oR[l], oZ[l] = np.mean([d[0] for d in nb]), np.mean([d[1] for d in nb])
-    return oR, oZ
+    return W.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
 
 
 def solve_case(om, h, levels, neumann):
