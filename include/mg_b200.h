@@ -75,6 +75,7 @@ typedef struct {
                       bit 1 (MG_SETUP_FUSED_TAIL): run the cycle steps of the small levels (<= 148 tiles) in one
                       cooperative kernel instead of one kernel per step (bit-identical results; off by default).
                       Other bits must be 0.                                                              */
+    int gamma;     /* cycle index of PAPER.md:187-189, 197: 0 or 1 = V-cycle (default), 2 = W-cycle             */
 } mg_options;
 
 /* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).

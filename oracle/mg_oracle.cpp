@@ -71,6 +71,7 @@ struct Oracle {
     std::vector<Level> lev;
     std::vector<int64_t> user2canon;          // user index -> canonical index on level 0
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
+    int gamma = 1;                            // cycle index: 1 V-cycle, 2 W-cycle
     bool have_coeffs = false;
     // coarse factorisation
     std::vector<double> lu;
@@ -408,7 +409,7 @@ static void lu_solve(const std::vector<double>& A, const std::vector<int32_t>& p
     std::memcpy(x, y.data(), sizeof(double) * n);
 }
 
-// ------------------------------------------------------------------ mg_cycle, gamma = 1
+// ------------------------------------------------------------------ mg_cycle
 static void mg_cycle(Oracle& o, int s, double* x, const double* b) {
     Level& lv = o.lev[s];
     if (s == o.L - 1) { lu_solve(o.lu, o.piv, lv.n, b, x); return; }
@@ -419,7 +420,7 @@ static void mg_cycle(Oracle& o, int s, double* x, const double* b) {
     Level& cv = o.lev[s + 1];
     std::vector<double> dc(cv.n), ec(cv.n, 0.0);                             // P:186 e = 0
     restrict_defect(lv, cv, d.data(), dc.data());
-    mg_cycle(o, s + 1, ec.data(), dc.data());                                // P:187-189, gamma = 1
+    for (int g = 0; g < o.gamma; g++) mg_cycle(o, s + 1, ec.data(), dc.data());   // gamma visits, e carried over
     std::vector<double> e;
     prolong_correct(lv, ec.data(), x, e);
     for (int k = 0; k < o.nu_post; k++) gs_sweep(lv, x, b);
@@ -495,6 +496,9 @@ void* orc_create(int64_t n, const int32_t* i, const int32_t* j, const uint8_t* k
     for (auto& lv : o->lev) { lv.lam.assign(lv.n, 0.0); lv.c.assign(lv.n, 0.0); }
     return o;
 }
+
+// cycle index gamma of P:187-189 (1 = V, 2 = W); default 1
+void orc_set_gamma(void* h, int gamma) { ((Oracle*)h)->gamma = gamma < 1 ? 1 : gamma; }
 
 int orc_num_levels(void* h) { return ((Oracle*)h)->L; }
 int64_t orc_level_n(void* h, int s) { return ((Oracle*)h)->lev[s].n; }

@@ -55,7 +55,7 @@ def _d(a):
 class Oracle:
     """create / update / solve plus single-step entry points for the pins."""
 
-    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, m=30, max_iters=200):
+    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, m=30, max_iters=200, gamma=1):
         L = lib()
         i = np.ascontiguousarray(i, dtype=np.int32)
         j = np.ascontiguousarray(j, dtype=np.int32)
@@ -66,6 +66,7 @@ class Oracle:
         if not self._h:
             raise ValueError("oracle: " + L.orc_last_error().decode())
         self._h = C.c_void_p(self._h)
+        L.orc_set_gamma(self._h, int(gamma))
         self.levels = L.orc_num_levels(self._h)
         self.m = m
         perm = np.empty(self.n, dtype=np.int64)

@@ -37,7 +37,7 @@ class _Bc(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("levels", C.c_int), ("nu_pre", C.c_int), ("nu_post", C.c_int), ("restart_m", C.c_int),
-                ("max_iters", C.c_int), ("flags", C.c_int)]
+                ("max_iters", C.c_int), ("flags", C.c_int), ("gamma", C.c_int)]
 
 
 EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_solve", "mg_update_coeffs_host",
@@ -103,7 +103,7 @@ def _dptr(t):
 class Solver:
     """create / update / solve on one mesh."""
 
-    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False):
+    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1):
         import torch
         if not host_only and not torch.cuda.is_available():
             raise RuntimeError("paper_2509_11831_b200 needs a CUDA device (no CPU fallback)")
@@ -114,7 +114,7 @@ class Solver:
         self.n = int(i.shape[0])
         mesh = _Mesh(self.n, i.ctypes.data, j.ctypes.data, float(h))
         bc = _Bc(kind.ctypes.data)
-        opt = _Options(int(levels), int(nu_pre), int(nu_post), int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0))
+        opt = _Options(int(levels), int(nu_pre), int(nu_post), int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0), int(gamma))
         hd = C.c_void_p()
         rc = L.mg_setup(C.byref(mesh), C.byref(bc), C.byref(opt), None if host_only else _stream_ptr(stream), C.byref(hd))
         if rc:

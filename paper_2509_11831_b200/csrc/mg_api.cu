@@ -45,6 +45,7 @@ struct mg_handle_s {
     HostHierarchy hh;
     int L = 0;
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
+    int gamma = 1;                        // cycle index: 1 V-cycle, 2 W-cycle
     int64_t n = 0;
     std::vector<LevelDev> lev;
     LevelDev* d_lev = nullptr;            // device copy of lev[] (fused small-level kernel)
@@ -134,7 +135,7 @@ void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailPr
     const bool fuse_dr = !h->no_fused_dr;
     for (int nu = h->nu_pre; nu > 0;) { const int k = nu >= 2 ? 2 : 1; gs(k, (fuse_dr && nu == k) ? 2 : 0, x_is_zero, nullptr); x_is_zero = false; nu -= k; }
     if (!fuse_dr) { TailOp op{}; op.type = TAIL_DR; op.level = (unsigned char)s; op.ntiles = h->lev[s + 1].ntiles; op.a = cur; op.b = h->buf[s + 1].b; op.c = b; push(op); }
-    build_tail(h, s + 1, h->buf[s + 1].x, h->buf[s + 1].b, true, P);
+    for (int g = 0; g < h->gamma; g++) build_tail(h, s + 1, h->buf[s + 1].x, h->buf[s + 1].b, g == 0, P);
     int nu = h->nu_post;
     { const int k = nu >= 2 ? 2 : 1; gs(k, 1, false, h->buf[s + 1].x); nu -= k; }
     while (nu > 0) { const int k = nu >= 2 ? 2 : 1; gs(k, 0, false, nullptr); nu -= k; }
@@ -169,7 +170,8 @@ void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
                                 fuse_dr ? &h->lev[s + 1] : nullptr, h->buf[s + 1].b);
     VecRef other = (cur.base == x.base) ? tmp : x;
     if (!fuse_dr) launch_defect_restrict(L, lv, h->lev[s + 1], cur, b, h->buf[s + 1].b);  // P:183-184  R (A x - b)
-    enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), true);         // P:186-189, e0 = 0
+    for (int g = 0; g < h->gamma; g++)                                                    // e0 = 0, gamma visits
+        enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), g == 0);
     VecRef fin;
     if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass
         const int k = h->nu_post >= 2 ? 2 : 1;
@@ -266,7 +268,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || (o.flags & ~3) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 2 || (o.flags & ~3) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
@@ -276,6 +278,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     h->nu_post = o.nu_post ? o.nu_post : 2;
     h->m = o.restart_m ? o.restart_m : 30;
     h->max_iters = o.max_iters ? o.max_iters : 200;
+    h->gamma = o.gamma > 1 ? o.gamma : 1;
     h->n = mesh->n;
     int rc = build_hierarchy(mesh->n, mesh->i, mesh->j, bc->kind, mesh->h, o.levels, h->hh);
     if (rc) { g_last_error = h->hh.err; delete h; return rc; }

@@ -405,3 +405,20 @@ def test_paper_annulus_mms_v55(gpu, oracle_mod, neumann):
     err = np.linalg.norm(host(xg)[m] - pl.meta["phi"][m]) / np.linalg.norm(pl.meta["phi"][m])
     assert err < (1.2e-2 if neumann else 1e-4)              # O(h) / O(h^2) at h = 2e-3
     s.close()
+
+
+def test_w_cycle_gamma2(gpu, oracle_mod):
+    """gamma = 2 (W-cycle): cycle and solve parity with the oracle."""
+    pl = W.make_plane(3, 129)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, gamma=2)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, gamma=2)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    rng = np.random.default_rng(8)
+    n = o.level_n(0)
+    x, b = rng.standard_normal(n), rng.standard_normal(n)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
+    s.close()

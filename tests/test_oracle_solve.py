@@ -202,3 +202,33 @@ def test_solve_edge_cases(oracle_mod):
     assert r4["status"] == 1 and r4["iters"] == 2
     with pytest.raises(ValueError):
         o.update(pl.lam, -pl.c)                                     # c > 0 required
+
+
+def test_w_cycle_gamma2(oracle_mod):
+    """Cycle index gamma of PAPER.md:187-189, 197 (gamma = 2: W-cycle).  With two levels a W-cycle equals a V-cycle (the second
+    exact coarse solve changes nothing).  With three levels the level-1 sub-cycle of a W-cycle is again a V-cycle, so the
+    W-cycle can be composed from the oracle's single steps with gamma = 1: pre-smoothing, defect, restriction, TWO
+    carried-over level-1 cycles, prolongation + correction, post-smoothing.  And it must contract at least as fast."""
+    pl = H.small_annulus(65, 3)
+    rng = np.random.default_rng(3)
+    ov = H.make_oracle(oracle_mod, pl, levels=3)
+    ow = H.make_oracle(oracle_mod, pl, levels=3, gamma=2)
+    n = ov.level_n(0)
+    x, b = rng.standard_normal(n), rng.standard_normal(n)
+    xs = ov.smooth(0, x, b, 2)
+    dc = ov.restrict(0, ov.apply(0, xs) - b)
+    e = ov.cycle(1, np.zeros(ov.level_n(1)), dc)
+    e = ov.cycle(1, e, dc)
+    ref = ov.smooth(0, ov.prolong_correct(0, e, xs), b, 2)
+    got = ow.cycle(0, x, b)
+    assert np.linalg.norm(got - ref) <= 1e-13 * np.linalg.norm(ref)
+    o2v, o2w = H.make_oracle(oracle_mod, pl, levels=2), H.make_oracle(oracle_mod, pl, levels=2, gamma=2)
+    assert np.linalg.norm(o2w.cycle(0, x, b) - o2v.cycle(0, x, b)) <= 1e-12 * np.linalg.norm(x)
+    # contraction of the error of A x = 0
+    zero = np.zeros(n)
+    ev, ew = x.copy(), x.copy()
+    for _ in range(6):
+        ev, ew = ov.cycle(0, ev, zero), ow.cycle(0, ew, zero)
+    assert np.linalg.norm(ew) <= 1.05 * np.linalg.norm(ev)
+    rv, rw = ov.solve(pl.f, pl.x0, 1e-10), ow.solve(pl.f, pl.x0, 1e-10)
+    assert rw["status"] == 0 and rw["iters"] <= rv["iters"]
