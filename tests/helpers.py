@@ -52,6 +52,24 @@ def small_dshape(n=33, levels=2, seed=7, order="rowmajor"):
     return W.mask_plane(inner, neu, h, lam, c, f, levels=levels, order=order, seed=seed)
 
 
+def random_blob_plane(seed, n=97):
+    """Ragged random domain: thresholded smooth noise with holes, islands and thin necks; random Dirichlet / Neumann
+    guards; random coefficients and right-hand side; odd negative lattice origin; auto level count.  Stresses the
+    coarse levels (inner sets that split, degenerate normals, guards that coincide with no fine point)."""
+    rng = np.random.default_rng(seed)
+    h = 2.0 / (n - 1)
+    g = W.gaussian_field(rng, n, 0.12 + 0.1 * rng.uniform(), h)
+    inner = g > rng.uniform(-0.4, 0.3)
+    inner[:2, :] = inner[-2:, :] = False
+    inner[:, :2] = inner[:, -2:] = False
+    neu = W.gaussian_field(rng, n, 0.3, h) > 0
+    lam = 0.2 + rng.uniform(0, 1, (n, n))
+    c = np.exp(0.7 * W.gaussian_field(rng, n, 0.1, h))
+    f = rng.standard_normal((n, n))
+    return W.mask_plane(inner, neu, h, lam, c, f, levels=0, i0=-41 - seed, j0=-13 + 2 * seed, seed=seed,
+                        order="shuffle" if seed % 2 else "rowmajor")
+
+
 def brute_hierarchy(i, j, kind, levels):
     """Re-derive every level (rules M1-M6) with dicts keyed on (I,J).
     Returns a list of dicts: pts (sorted by (J,I)), kind, colour, nbr."""

@@ -45,6 +45,8 @@ CASES = {
     "cfg3_dshape257": lambda: W.make_plane(3, 257),
     "cfg4_dshape257": lambda: W.make_plane(4, 257),
     "annulus65_negative_origin": lambda: H.small_annulus(65, 4, i0=-37, j0=-22),
+    "random_blob_101": lambda: H.random_blob_plane(101),
+    "random_blob_104_193": lambda: H.random_blob_plane(104, 193),
 }
 
 

@@ -54,6 +54,10 @@ CASES = {
 }
 
 
+for _k in range(8):
+    CASES[f"random_blob_{_k}"] = (lambda k: (lambda: H.random_blob_plane(100 + k)))(_k)
+
+
 @pytest.mark.parametrize("case", list(CASES))
 def test_hierarchy_bit_exact_vs_oracle(oracle_mod, case):
     pl = CASES[case]()
