@@ -108,12 +108,12 @@ Launch LZ(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }
 
 // nu Gauss-Seidel sweeps, two per launch where possible, ping-ponging between `cur` and `other`.
 // Returns the buffer that holds the result.
-// With `coarse`, the last launch also writes the restricted defect of the result to d_coarse.
+// With `coarse`, the last launch also writes the restricted defect of the result to d_coarse; with `w_out`, A times the result.
 VecRef enqueue_smooth(const Launch& L, const LevelDev& lv, VecRef cur, VecRef other, VecRef b, int nu, bool cur_is_zero,
-                      const LevelDev* coarse = nullptr, double* d_coarse = nullptr) {
+                      const LevelDev* coarse = nullptr, double* d_coarse = nullptr, double* w_out = nullptr) {
     while (nu > 0) {
         const int k = nu >= 2 ? 2 : 1;
-        launch_gs_fused(L, lv, cur, other, b, k, cur_is_zero, nu == k ? coarse : nullptr, d_coarse);
+        launch_gs_fused(L, lv, cur, other, b, k, cur_is_zero, nu == k ? coarse : nullptr, d_coarse, nu == k ? w_out : nullptr);
         std::swap(cur, other);
         cur_is_zero = false;
         nu -= k;
@@ -143,8 +143,9 @@ void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailPr
 }
 
 // mg_cycle of PAPER.md:171-195 with gamma = 1, enqueued on L.stream.  x_is_zero: the initial guess is
-// the zero vector and x need not be read (nor zeroed beforehand).
-void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero) {
+// the zero vector and x need not be read (nor zeroed beforehand).  w_out: also produce w_out = A x for the
+// result (fused into the last smoothing launch); returns whether it was written.
+bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero, double* w_out = nullptr) {
     const LevelDev& lv = h->lev[s];
     if (s >= h->tail_s0) {                                            // small levels: one cooperative kernel
         TailProgram P; P.nops = 0;
@@ -155,13 +156,13 @@ void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
             TailCoarse cs{h->Ainv, h->cslot, h->nL};
             if (grid <= h->tail_cap && h->L - s <= TAIL_MAX_LEVELS) {
                 h->tail_err = launch_tail(L, h->d_lev, s, h->L, P, cs, x, b, grid);
-                return;
+                return false;
             }
         }
     }
     if (s == h->L - 1) {                                              // P:173-177 direct solve
         launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, b, x);
-        return;
+        return false;
     }
     VecRef tmp = vec(h->buf[s].x2);
     if (x_is_zero && h->nu_pre == 0) { launch_zero(L, x, lv.nslots); x_is_zero = false; }
@@ -173,23 +174,27 @@ void enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
     for (int g = 0; g < h->gamma; g++)                                                    // e0 = 0, gamma visits
         enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), g == 0);
     VecRef fin;
+    bool wrote_w = false;
     if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass
-        const int k = h->nu_post >= 2 ? 2 : 1;
-        launch_gs_correct(L, lv, h->buf[s + 1].x, cur, other, b, k);
-        fin = enqueue_smooth(L, lv, other, cur, b, h->nu_post - k, false);
+        const int k = h->nu_post >= 2 ? 2 : 1, rem = h->nu_post - k;
+        launch_gs_correct(L, lv, h->buf[s + 1].x, cur, other, b, k, rem == 0 ? w_out : nullptr);
+        fin = enqueue_smooth(L, lv, other, cur, b, rem, false, nullptr, nullptr, w_out);
+        wrote_w = w_out != nullptr;
     } else {
         launch_prolong_correct(L, lv, h->lev[s + 1], h->buf[s + 1].x, h->buf[s].d, cur);
         fin = cur;
     }
     if (fin.base != x.base) launch_copy(L, fin, x, lv.nslots);
+    return wrote_w;
 }
 
 // One Arnoldi step (rule K2): z_j = MG(v_j), w = A z_j, CGS2, Givens + stop test, v_{j+1}.
 void enqueue_iteration(mg_handle h, const Launch& L) {
     const int64_t ns = h->lev[0].nslots;
     VecRef zj{h->Z, ns, &h->st->j, 0}, vj{h->V, ns, &h->st->j, 0};
-    enqueue_cycle(h, L, 0, zj, vj, true);
-    launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
+    static const bool no_fused_apply = getenv("MG_B200_NO_FUSED_APPLY") != nullptr;
+    if (!enqueue_cycle(h, L, 0, zj, vj, true, no_fused_apply ? nullptr : h->w))          // w = A z_j fused into the cycle's last launch
+        launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
     launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial, h->m);
     if (h->m <= MAX_M_FUSED) {                                     // three passes over the basis
         launch_update_dot(L, h->w, h->V, ns, ns, h->st, h->partial);

@@ -78,9 +78,11 @@ void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRe
 // x_in_zero: treat x_in as the zero vector without reading it.
 // coarse != null: the launch also writes d_coarse = R (A x_out - b) on that level, fused.
 void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero,
-                     const LevelDev* coarse = nullptr, double* d_coarse = nullptr);
+                     const LevelDev* coarse = nullptr, double* d_coarse = nullptr, double* w_out = nullptr);
 // Same, preceded in the same pass by the coarse-grid correction x_in - P e_c with set_bnds_hom (rule T3).
-void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps);
+// w_out != null (either call): the launch also writes w_out = A x_out (the Arnoldi step's operator apply, fused).
+void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps,
+                       double* w_out = nullptr);
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n);
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse);
 // d_coarse = R (A x - b), the defect never stored (rules D4 + T2)

@@ -9,9 +9,10 @@ namespace mgb {
 namespace {
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-// DR: additionally d_c = R (A x_out - b) on the next coarser level (ccode = its point codes).
+// EPI = 1: additionally d_c = R (A x_out - b) on the next coarser level (ccode = its point codes, dc = d_c).
+// EPI = 2: additionally w = A x_out (dc = w).
 // BX x BY < tile: several CTAs per tile (blockIdx = tile * blocks-per-tile + block).
-template <int NS, bool PC, bool DR, int BX, int BY>
+template <int NS, bool PC, int EPI, int BX, int BY>
 __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
                                               int xin_zero, const uint16_t* __restrict__ ccode, double* __restrict__ dc,
                                               const int* __restrict__ stop) {
@@ -19,7 +20,7 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
     if (stop != nullptr && *stop) return;
     constexpr int NBX = TX / BX, NSUB = NBX * (TY / BY);
     const int t = blockIdx.x / NSUB, sub = blockIdx.x - t * NSUB;
-    gs_tile<NS, PC, false, DR, BX, BY>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
+    gs_tile<NS, PC, false, EPI, BX, BY>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
                                        (sub % NBX) * BX, (sub / NBX) * BY);
 }
 
@@ -34,43 +35,54 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
 constexpr int SUB_MAX_TILES = 40, SBX = 16, SBY = 16;      // 8 CTAs per tile
 constexpr int MID_MAX_TILES = 148, MBX = 32, MBY = 16;     // 4 CTAs per tile
 
-template <int NS, bool PC, bool DR, int BX, int BY>
+template <int NS, bool PC, int EPI, int BX, int BY>
 void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
                 const uint16_t* ccode, double* dc) {
-    constexpr size_t smem = Geo<NS, PC, DR, BX, BY>::SMEM;
+    constexpr size_t smem = Geo<NS, PC, EPI, BX, BY>::SMEM;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_gs<NS, PC, DR, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_gs<NS, PC, EPI, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = true;
     }
     const int grid = lv.ntiles * (TX / BX) * (TY / BY);
-    k_gs<NS, PC, DR, BX, BY><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
+    k_gs<NS, PC, EPI, BX, BY><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
     if (L.counter) *L.counter += 1;
 }
 
-template <int NS, bool PC, bool DR = false>
+template <int NS, bool PC, int EPI = 0>
 void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
                const uint16_t* ccode = nullptr, double* dc = nullptr) {
     static const bool no_sub = getenv("MG_B200_NO_SUBBLOCKS") != nullptr;
-    if (lv.ntiles <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, DR, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
-    else if (lv.ntiles <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, DR, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
-    else launch_blk<NS, PC, DR, TX, TY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    if (lv.ntiles <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else if (lv.ntiles <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else launch_blk<NS, PC, EPI, TX, TY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
 }
 
 }  // namespace
 
 void launch_gs_fused(const Launch& L, const LevelDev& lv, VecRef x_in, VecRef x_out, VecRef b, int sweeps, bool x_in_zero,
-                     const LevelDev* coarse, double* d_coarse) {
+                     const LevelDev* coarse, double* d_coarse, double* w_out) {
     if (coarse != nullptr) {                                  // + restricted defect of the result
-        if (sweeps == 2) launch_ns<2, false, true>(L, lv, x_in, x_out, b, nullptr, x_in_zero, coarse->code, d_coarse);
-        else launch_ns<1, false, true>(L, lv, x_in, x_out, b, nullptr, x_in_zero, coarse->code, d_coarse);
+        if (sweeps == 2) launch_ns<2, false, 1>(L, lv, x_in, x_out, b, nullptr, x_in_zero, coarse->code, d_coarse);
+        else launch_ns<1, false, 1>(L, lv, x_in, x_out, b, nullptr, x_in_zero, coarse->code, d_coarse);
+        return;
+    }
+    if (w_out != nullptr) {                                   // + w = A x_out
+        if (sweeps == 2) launch_ns<2, false, 2>(L, lv, x_in, x_out, b, nullptr, x_in_zero, nullptr, w_out);
+        else launch_ns<1, false, 2>(L, lv, x_in, x_out, b, nullptr, x_in_zero, nullptr, w_out);
         return;
     }
     if (sweeps == 2) launch_ns<2, false>(L, lv, x_in, x_out, b, nullptr, x_in_zero);
     else launch_ns<1, false>(L, lv, x_in, x_out, b, nullptr, x_in_zero);
 }
 
-void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps) {
+void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coarse, VecRef x_in, VecRef x_out, VecRef b, int sweeps,
+                       double* w_out) {
+    if (w_out != nullptr) {                                   // + w = A x_out
+        if (sweeps == 2) launch_ns<2, true, 2>(L, lv, x_in, x_out, b, e_coarse, false, nullptr, w_out);
+        else launch_ns<1, true, 2>(L, lv, x_in, x_out, b, e_coarse, false, nullptr, w_out);
+        return;
+    }
     if (sweeps == 2) launch_ns<2, true>(L, lv, x_in, x_out, b, e_coarse, false);
     else launch_ns<1, true>(L, lv, x_in, x_out, b, e_coarse, false);
 }

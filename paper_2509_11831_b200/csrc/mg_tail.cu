@@ -123,8 +123,8 @@ size_t tail_smem() {
     m = std::max(m, Geo<2, false>::SMEM_COH);
     m = std::max(m, Geo<1, true>::SMEM_COH);
     m = std::max(m, Geo<1, false>::SMEM_COH);
-    m = std::max(m, Geo<2, false, true>::SMEM_COH);
-    m = std::max(m, Geo<1, false, true>::SMEM_COH);
+    m = std::max(m, Geo<2, false, 1>::SMEM_COH);
+    m = std::max(m, Geo<1, false, 1>::SMEM_COH);
     return m;
 }
 

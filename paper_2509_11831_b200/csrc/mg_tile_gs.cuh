@@ -38,12 +38,14 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 constexpr int GT = 512;     // threads per CTA
 constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
-// DR: the launch also restricts the defect of its result (needs x two cells beyond the tile).
+// EPI: epilogue after the sweeps.  1 (DR): the launch also restricts the defect of its result (needs x two cells beyond
+// the tile).  2 (AP): the launch also writes w = A x_out (needs one cell beyond the tile): the operator apply of the
+// Arnoldi step, fused into the last smoothing launch of the preconditioner cycle.
 // BX x BY: the block of the tile one CTA produces (the whole tile, or a sub-block on small levels where
 // latency, not throughput, decides: more CTAs per tile).
-template <int NS, bool PC, bool DR = false, int BX = TX, int BY = TY>
+template <int NS, bool PC, int EPI = 0, int BX = TX, int BY = TY>
 struct Geo {
-    static constexpr int H = 3 * NS + (PC ? 1 : 0) + (DR ? 2 : 0);
+    static constexpr int H = 3 * NS + (PC ? 1 : 0) + (EPI == 1 ? 2 : (EPI == 2 ? 1 : 0));
     static constexpr int RW = BX + 2 * H;
     static constexpr int RH = BY + 2 * H;
     static constexpr int BW = BX, BH = BY;
@@ -59,9 +61,9 @@ struct Geo {
 // Interior tiles (every cell within 2*NS of the tile is an inner point; flagged by the host setup) take a
 // fast path: no guard phase, so the valid region shrinks by 2 instead of 3 cells per sweep (halo 2*NS), and
 // no point codes are needed at all.
-template <int NS, bool DR = false, int BX = TX, int BY = TY>
+template <int NS, int EPI = 0, int BX = TX, int BY = TY>
 struct GeoF {
-    static constexpr int H = 2 * NS + (DR ? 2 : 0);
+    static constexpr int H = 2 * NS + (EPI == 1 ? 2 : (EPI == 2 ? 1 : 0));
     static constexpr int RW = BX + 2 * H;
     static constexpr int RH = BY + 2 * H;
     static constexpr int BW = BX, BH = BY;
@@ -184,6 +186,59 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
     }
 }
 
+// Fused operator apply (rules D1-D3, the same rows as k_apply): every thread forms (A x) for its own cells of the tile
+// from the smoothed x in shared memory (lambda is the only extra load), parks it in the no longer needed c array,
+// and the tile is written out coalesced.  `breg` is reused as scratch.
+template <class G, bool GENERAL>
+__device__ __forceinline__ void apply_epilogue(const LevelDev& lv, int t, const int* tn, const double* sx, double* sc, const uint16_t* scode,
+                                               double (&breg)[2][G::ROUNDS], double kappa, double* __restrict__ wout, int bx0, int by0) {
+    constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, ROUNDS = G::ROUNDS, BX = G::BW, BY = G::BH;
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            const int q = tid + r * GT;
+            double v = 0.0;
+            if (q < NC) {
+                const int ry = q / RWC, k = q - ry * RWC, tpar = (ry + col) & 1, rx = 2 * k + tpar;
+                if (min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) >= H) {          // a cell of the tile (block)
+                    const int own = col * NC + q, ob = (1 - col) * NC + q;
+                    const uint16_t code = GENERAL ? scode[own] : (uint16_t)C_INNER;
+                    const int kind = code & 3;
+                    if (kind == C_INNER) {
+                        const double lam = __ldg(lv.lam + region_slot<H>(tn, rx + bx0, ry + by0));
+                        const double cl = sc[own], xl = sx[own];
+                        const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
+                        const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
+                        v = lam * xl + aW * (xl - sx[ob + tpar - 1]) + aE * (xl - sx[ob + tpar]) + aS * (xl - sx[ob - RWC]) +
+                            aN * (xl - sx[ob + RWC]);
+                    } else if (kind == C_DIR) v = sx[own];
+                    else if (kind == C_NEU) {
+                        double sum, wself, delta;
+                        neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
+                        const double xl = sx[own];
+                        v = (sum + wself * xl - xl) / delta;
+                    }
+                }
+            }
+            breg[col][r] = v;
+        }
+    __syncthreads();
+#pragma unroll
+    for (int col = 0; col < 2; col++)
+#pragma unroll
+        for (int r = 0; r < ROUNDS; r++) {
+            const int q = tid + r * GT;
+            if (q < NC) sc[col * NC + q] = breg[col][r];
+        }
+    __syncthreads();
+    for (int idx = tid; idx < BX * BY; idx += GT) {
+        const int ly = idx / BX, lx = idx - ly * BX;
+        wout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sc[cidx<G>(lx + H, ly + H)];
+    }
+}
+
 // e = (P e_c) at fine cell (lx, ly) relative to the tile (may lie in the halo): bilinear, weights
 // 1 / (1/2, 1/2) / (1/4 x 4) in the order (cx, cy), (cx+1, cy), (cx, cy+1), (cx+1, cy+1); absent parents hold 0.
 // Branch-free (unused parents alias the first one with weight 0) so that the loads of all cells overlap.
@@ -201,13 +256,14 @@ __device__ __forceinline__ double prolong_e(const int* pt, int odd0, int odd1, i
 }
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-template <int NS, bool PC, bool COH, bool DR = false, int BX = TX, int BY = TY>
+template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY>
 __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                            const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                            unsigned char* smem_raw, const int* meta = nullptr,
                                            const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr,
                                            int bx0 = 0, int by0 = 0) {
-    using G = Geo<NS, PC, DR, BX, BY>;
+    using G = Geo<NS, PC, EPI, BX, BY>;
+    constexpr bool DR = EPI == 1, AP = EPI == 2;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
@@ -379,7 +435,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     const int base = 1 + col + (PC ? 1 : 0);
                     const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
                     if (nsw > 0) { breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s); }
-                    if (DR && marg >= H - 1) prefetch_l2(lv.lam + s);     // read by the restriction epilogue
+                    if ((DR && marg >= H - 1) || (AP && marg >= H)) prefetch_l2(lv.lam + s);     // read by the restriction epilogue
                     act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
                 } else if (kind != C_ABSENT) {
                     const int pos = atomicAdd(&gcount, 1);
@@ -458,23 +514,25 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
         xout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sx[cidx<G>(lx + H, ly + H)];
     }
     if (DR) restrict_epilogue<G, true>(lv, tn, pt, odd, sx, sc, scode, breg, kappa, ccode, dc, bx0, by0);
+    if (AP) apply_epilogue<G, true>(lv, t, tn, sx, sc, scode, breg, kappa, dc, bx0, by0);
 }
 
 // Interior tile: all cells of the region are inner points.
-template <int NS, bool PC, bool COH, bool DR = false, int BX = TX, int BY = TY>
+template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY>
 __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                         unsigned char* smem_raw, const int* meta = nullptr,
                                            const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr,
                                            int bx0 = 0, int by0 = 0) {
-    using G = GeoF<NS, DR, BX, BY>;
+    using G = GeoF<NS, EPI, BX, BY>;
+    constexpr bool DR = EPI == 1, AP = EPI == 2;
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, RN = G::RN, ROUNDS = G::ROUNDS;
     static_assert(ROUNDS * 2 * 4 <= 32, "activity nibbles must fit one word");
     double* sx = reinterpret_cast<double*>(smem_raw);
     double* sc = sx + RN;
     double* sce = sc + RN;                                   // (PC) coarse values under the region
     constexpr int CM = (H + 1) / 2, CW = BX / 2 + (H - 1) / 2 + CM + 2, CHH = BY / 2 + (H - 1) / 2 + CM + 2;
-    static_assert((size_t)(2 * RN + CW * CHH) * sizeof(double) <= Geo<NS, true, false, BX, BY>::SMEM, "coarse stage must fit the PC allocation");
+    static_assert((size_t)(2 * RN + CW * CHH) * sizeof(double) <= Geo<NS, true, EPI, BX, BY>::SMEM, "coarse stage must fit the PC allocation");
     __shared__ int tn[9];
     __shared__ int pt[9];
     __shared__ int odd[2];
@@ -545,7 +603,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 const int base = 1 + col;
                 const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
                 if (nsw > 0) { breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s); }
-                if (DR && marg >= H - 1) prefetch_l2(lv.lam + s);         // read by the restriction epilogue
+                if ((DR && marg >= H - 1) || (AP && marg >= H)) prefetch_l2(lv.lam + s);         // read by the restriction epilogue
                 act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
             }
     }
@@ -598,18 +656,19 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
         xout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sx[cidx<G>(lx + H, ly + H)];
     }
     if (DR) restrict_epilogue<G, false>(lv, tn, pt, odd, sx, sc, nullptr, breg, kappa, ccode, dc, bx0, by0);
+    if (AP) apply_epilogue<G, false>(lv, t, tn, sx, sc, nullptr, breg, kappa, dc, bx0, by0);
 }
 
-template <int NS, bool PC, bool COH, bool DR = false, int BX = TX, int BY = TY>
+template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY>
 __device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                         unsigned char* smem_raw, const int* meta = nullptr,
                                            const uint16_t* __restrict__ ccode = nullptr, double* __restrict__ dc = nullptr,
                                            int bx0 = 0, int by0 = 0) {
     const int flag = meta != nullptr ? meta[META_FLAG] : lv.tflag[t];
-    constexpr int need = 1 << (NS - 1 + (DR ? 1 : 0));          // interior halo 2 NS (+ 2): flag bit
-    if (flag & need) gs_fast<NS, PC, COH, DR, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
-    else gs_general<NS, PC, COH, DR, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
+    constexpr int need = 1 << (NS - 1 + (EPI ? 1 : 0));         // interior halo 2 NS (+ 1 or 2, rounded up to the next flag)
+    if (flag & need) gs_fast<NS, PC, COH, EPI, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
+    else gs_general<NS, PC, COH, EPI, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
 }
 
 }  // namespace
