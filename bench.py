@@ -186,7 +186,7 @@ def run_ours(args):
     uniq = seq if warm else seq[:1]
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, full_cgs2=args.full_cgs2)
     d_in = [(dev(q.lam), dev(q.c), dev(q.f)) for q in uniq]          # resident in HBM before the timed region
     h_in = [(pin(q.lam).numpy(), pin(q.c).numpy(), pin(q.f).numpy()) for q in uniq]
     d_x0, d_x = dev(pl.x0), torch.empty(pl.n, dtype=torch.float64, device="cuda")
@@ -239,6 +239,7 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None
     iters_all = [o[0] for o in outs]
     ms, work, value = whole_job(ms_loc, float(pl.n) * sum(iters_all), world, "cuda")
+    reorth = s.last_reorth
     for k in range(args.warmup):
         step_host(k)
     ms_e_loc, outs_e, _, _, _ = timed(step_host, args.warmup, args.steps)
@@ -284,6 +285,7 @@ def run_ours(args):
                            "step": "mg_update_coeffs + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
                            "l2_policy": "inputs larger than L2 (no flush)" if pl.n * 8 * 8 > 126e6 else "working set fits L2 (small config)"},
                 "iters": iters_all[-1], "iters_per_step": iters_all, "final_relres": outs[-1][1], "status": outs[-1][2],
+                "second_gs_updates": reorth,      # Arnoldi steps of the last solve whose second update ran (G23)
                 "solve_ms": float(np.median(solve_ms)), "update_ms": float(np.median(update_ms)),
                 "solve_ms_per_plane": float(np.median(solve_ms)),
                 "clocks": clocks, "gpu_launches": launches,
@@ -431,6 +433,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--ref-iters", type=int, default=8, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--full-cgs2", action="store_true", help="always run the second Gram-Schmidt update (MG_SETUP_FULL_CGS2)")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
     ap.add_argument("--lattice", type=int, default=None, help="same geometry on an n x n lattice (2^k + 1; O(N) scaling runs)")
     ap.add_argument("--paper-mms", type=int, default=0, metavar="R",

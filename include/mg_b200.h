@@ -33,6 +33,7 @@ extern "C" {
 typedef struct mg_handle_s* mg_handle;
 #define MG_SETUP_HOST_ONLY 1
 #define MG_SETUP_FUSED_TAIL 2
+#define MG_SETUP_FULL_CGS2 4
 
 enum {
     MG_OK = 0,
@@ -74,6 +75,9 @@ typedef struct {
                       every compute call returns MG_ECUDA.
                       bit 1 (MG_SETUP_FUSED_TAIL): run the cycle steps of the small levels (<= 148 tiles) in one
                       cooperative kernel instead of one kernel per step (bit-identical results; off by default).
+                      bit 2 (MG_SETUP_FULL_CGS2): always run the second Gram-Schmidt update of the Arnoldi step;
+                      by default it is skipped in the steps where the measured defect ||V^T w'|| is already
+                      <= 1e-13 ||w'|| (G23; same iterates to that level).
                       Other bits must be 0.                                                              */
     int gamma;     /* cycle index of PAPER.md:187-189, 197: 0 or 1 = V-cycle (default), 2 = W-cycle             */
 } mg_options;
@@ -148,6 +152,14 @@ double mg_last_update_ms(mg_handle h);
 /* Device time of the smoothing kernels alone (without the in/out permutations) of the last mg_smooth or
  * mg_smooth_restrict call, CUDA events on the launching stream; synchronises on the second event. */
 double mg_last_step_ms(mg_handle h);
+/* Arnoldi steps of the last mg_solve whose second Gram-Schmidt update ran (see MG_SETUP_FULL_CGS2); -1 before
+ * the first solve. */
+int mg_last_reorth(mg_handle h);
+/* Per-iteration history of the last mg_solve (first min(iters, 512, cap) iterations), HOST arrays, either may be
+ * NULL: relres[k] = the recurrence residual |g_{k+1}| / ||f|| after iteration k+1 (Eq. 23; monotone
+ * within a restart cycle), orth[k] = ||V^T w'|| / ||w'|| measured after the first Gram-Schmidt projection of that
+ * iteration (0 on the unfused path, restart_m > 32).  Returns the number of entries written. */
+int mg_last_history(mg_handle h, double* relres, double* orth, int cap);
 
 const char* mg_strerror(int code);
 const char* mg_last_error(void);

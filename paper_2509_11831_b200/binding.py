@@ -43,7 +43,7 @@ class _Options(C.Structure):
 EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_solve", "mg_update_coeffs_host",
            "mg_solve_host", "mg_destroy", "mg_num_levels", "mg_level_n", "mg_level_info", "mg_transfer_info",
            "mg_level_coeffs", "mg_apply", "mg_smooth", "mg_restrict", "mg_smooth_restrict", "mg_prolong_correct", "mg_coarse_solve",
-           "mg_vcycle", "mg_kernel_launches", "mg_last_solve_ms", "mg_last_update_ms", "mg_last_step_ms", "mg_strerror",
+           "mg_vcycle", "mg_kernel_launches", "mg_last_solve_ms", "mg_last_update_ms", "mg_last_step_ms", "mg_last_reorth", "mg_last_history", "mg_strerror",
            "mg_last_error"]
 
 
@@ -103,7 +103,7 @@ def _dptr(t):
 class Solver:
     """create / update / solve on one mesh."""
 
-    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1):
+    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1, full_cgs2=False):
         import torch
         if not host_only and not torch.cuda.is_available():
             raise RuntimeError("paper_2509_11831_b200 needs a CUDA device (no CPU fallback)")
@@ -114,7 +114,7 @@ class Solver:
         self.n = int(i.shape[0])
         mesh = _Mesh(self.n, i.ctypes.data, j.ctypes.data, float(h))
         bc = _Bc(kind.ctypes.data)
-        opt = _Options(int(levels), int(nu_pre), int(nu_post), int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0), int(gamma))
+        opt = _Options(int(levels), int(nu_pre), int(nu_post), int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma))
         hd = C.c_void_p()
         rc = L.mg_setup(C.byref(mesh), C.byref(bc), C.byref(opt), None if host_only else _stream_ptr(stream), C.byref(hd))
         if rc:
@@ -259,6 +259,19 @@ class Solver:
     @property
     def last_step_ms(self):
         return float(lib().mg_last_step_ms(self._h))
+
+    def last_history(self):
+        """(relres, orth) per iteration of the last solve, see mg_last_history."""
+        import numpy as np
+        r, o = np.zeros(512), np.zeros(512)
+        n = lib().mg_last_history(self._h, r.ctypes.data_as(C.c_void_p), o.ctypes.data_as(C.c_void_p), 512)
+        if n < 0:
+            raise RuntimeError(f"mg_last_history: {n}")
+        return r[:n].copy(), o[:n].copy()
+
+    @property
+    def last_reorth(self):
+        return int(lib().mg_last_reorth(self._h))
 
     @property
     def last_update_ms(self):

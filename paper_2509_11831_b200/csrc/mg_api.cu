@@ -46,6 +46,7 @@ struct mg_handle_s {
     int L = 0;
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
     int gamma = 1;                        // cycle index: 1 V-cycle, 2 W-cycle
+    bool full_cgs2 = false;               // MG_SETUP_FULL_CGS2
     int64_t n = 0;
     std::vector<LevelDev> lev;
     LevelDev* d_lev = nullptr;            // device copy of lev[] (fused small-level kernel)
@@ -273,7 +274,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 2 || (o.flags & ~3) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 2 || (o.flags & ~7) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
@@ -284,6 +285,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     h->m = o.restart_m ? o.restart_m : 30;
     h->max_iters = o.max_iters ? o.max_iters : 200;
     h->gamma = o.gamma > 1 ? o.gamma : 1;
+    h->full_cgs2 = (o.flags & MG_SETUP_FULL_CGS2) != 0;
     h->n = mesh->n;
     int rc = build_hierarchy(mesh->n, mesh->i, mesh->j, bc->kind, mesh->h, o.levels, h->hh);
     if (rc) { g_last_error = h->hh.err; delete h; return rc; }
@@ -395,7 +397,7 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
     if (rc) return rc;
     const int64_t ns = h->lev[0].nslots;
     CU(cudaEventRecord(h->ev[0], s));
-    launch_init_state(L, h->st, h->m, h->max_iters, rtol);
+    launch_init_state(L, h->st, h->m, h->max_iters, rtol, h->full_cgs2);
     launch_gather(L, d_f, h->user2slot, h->bs, h->n);                 // B1: user order -> tile layout
     launch_gather(L, d_x0, h->user2slot, h->xs, h->n);
     launch_norm2(L, h->bs, ns, h->st, h->partial, 0);                 // K1: bn = ||b||
@@ -469,6 +471,19 @@ int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_
 }
 
 int64_t mg_kernel_launches(mg_handle h) { return h ? h->launches : 0; }
+
+int mg_last_history(mg_handle h, double* relres, double* orth, int cap) {
+    if (!h || cap < 0) return MG_EINVAL;
+    if (!h->solve_timed) return 0;
+    const int n = std::min(std::min(h->h_state->iters, 512), cap);
+    for (int k = 0; k < n; k++) {
+        if (relres) relres[k] = h->h_state->hist[k];
+        if (orth) orth[k] = h->h_state->orth[k];
+    }
+    return n;
+}
+
+int mg_last_reorth(mg_handle h) { return (h && h->solve_timed) ? h->h_state->nreorth : -1; }
 
 double mg_last_solve_ms(mg_handle h) {
     float ms = -1.f;

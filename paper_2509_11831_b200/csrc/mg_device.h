@@ -54,13 +54,17 @@ struct GmresState {
     int cycle_end;    // 1: the running cycle ended (converged, j == m, max_iters or breakdown)
     int m, max_iters;
     int ticket;       // last-block-done counter of the grid reductions
+    int nreorth;      // Arnoldi steps of this solve whose second Gram-Schmidt update ran
+    int skip2;        // 1: the step in flight needs no second update (k_final_v only normalises)
     int pad;
+    double reorth_tol;  // second update skipped when ||V^T w'|| <= reorth_tol ||w'||; < 0: never (MG_SETUP_FULL_CGS2)
     double rtol, bn, beta, relres, hn, inv_hn;
     double red[MAX_M + 2];          // results of the last multi-reduction
     double hcol[MAX_M + 2];         // Hessenberg column being built (h_0j .. h_j+1,j)
     double H[(MAX_M + 1) * MAX_M];  // rotated Hessenberg (upper triangular R), row-major, ld = MAX_M
     double g[MAX_M + 1], cs[MAX_M], sn[MAX_M], y[MAX_M];
     double hist[512];               // |g_{k+1}| / bn per iteration
+    double orth[512];               // ||V^T w'|| / ||w'|| after the first Gram-Schmidt projection, per iteration (fused path)
 };
 
 struct Launch {
@@ -147,6 +151,6 @@ void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stri
 void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st);
-void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol);
+void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol, bool full_cgs2);
 
 }  // namespace mgb

@@ -203,6 +203,7 @@ __global__ void k_givens(GmresState* st) {
 //   pass 3  k_final_v       v_{j+1} = (w' - V h2) / h_{j+1,j}, written straight into the basis
 // Traffic at column j: 8(j+2) + (16 + 8(j+1)) + (16 + 8(j+1)) = 24 j + 64 B/pt against 32 j + 96.
 constexpr int FUSED_NV = 32;
+constexpr double REORTH_TOL = 1e-13;   // second update skipped when ||V^T w'|| <= REORTH_TOL ||w'|| (G23)
 constexpr int UD_THREADS = 128;
 constexpr int UD_BLOCKS = 148 * 2;   // 254 registers x 128 threads: two blocks per SM, one wave
 
@@ -263,13 +264,20 @@ __device__ __forceinline__ void ud_finish(double (&acc)[FUSED_NV], double accn, 
         __syncthreads();
         if (threadIdx.x == 0) {
             double s2 = 0.0;
+            for (int i = 0; i < nv; i++) s2 += tot[i] * tot[i];
+            // h2 = V^T w' IS the orthogonality defect of w' against the basis: when it is below REORTH_TOL
+            // relative to ||w'|| the second update would change nothing above that level and is skipped
+            // (k_final_v then only normalises: 16 B/pt instead of 8(j+3)).
+            const bool skip = st->reorth_tol > 0.0 && s2 <= st->reorth_tol * st->reorth_tol * tot[FUSED_NV];
             for (int i = 0; i < nv; i++) {
-                st->hcol[i] = hh[i] + tot[i];     // h_ij = first + second projection
-                st->red[i] = tot[i];              // h2, consumed by k_final_v
-                s2 += tot[i] * tot[i];
+                st->hcol[i] = skip ? hh[i] : hh[i] + tot[i];     // h_ij = first (+ second) projection
+                st->red[i] = tot[i];                             // h2, consumed by k_final_v
             }
-            const double hn2 = tot[FUSED_NV] - s2;
+            const double hn2 = skip ? tot[FUSED_NV] : tot[FUSED_NV] - s2;
             st->hcol[nv] = hn2 > 0.0 ? sqrt(hn2) : 0.0;
+            st->skip2 = skip ? 1 : 0;
+            if (!skip) st->nreorth += 1;
+            if (st->iters < 512) st->orth[st->iters] = tot[FUSED_NV] > 0.0 ? sqrt(s2 / tot[FUSED_NV]) : 0.0;
             givens_step(st);
         }
     }
@@ -511,15 +519,33 @@ __device__ __forceinline__ void final_v_body(const double* __restrict__ w, const
 __global__ void __launch_bounds__(RED_THREADS) k_final_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n,
                                                         GmresState* st) {
     __shared__ double hh[FUSED_NV];
-    if (st->cycle_end) return;
+    if (st->cycle_end || st->skip2) return;
     const int nv = st->j;
-    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
-    __syncthreads();
     double* out = V + (int64_t)nv * stride;
     const double inv = st->inv_hn;
+    if (threadIdx.x < FUSED_NV) hh[threadIdx.x] = threadIdx.x < nv ? st->red[threadIdx.x] : 0.0;
+    __syncthreads();
     if (nv <= 8) final_v_body<8, 4>(w, V, out, stride, n, nv, hh, inv);
     else if (nv <= 16) final_v_body<16, 2>(w, V, out, stride, n, nv, hh, inv);
     else final_v_body<32, 1>(w, V, out, stride, n, nv, hh, inv);
+}
+
+// The step needs no second update (skip2, see ud_finish): v_{j+1} = w' / h_{j+1,j}.  n is a multiple of the tile size.
+constexpr int SV_THREADS = 256, SV_UNROLL = 4;
+__global__ void __launch_bounds__(SV_THREADS) k_scale_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n,
+                                                        GmresState* st) {
+    if (st->cycle_end || !st->skip2) return;
+    const double inv = st->inv_hn;
+    const double2* __restrict__ w2 = reinterpret_cast<const double2*>(w);
+    double2* __restrict__ o2 = reinterpret_cast<double2*>(V + (int64_t)st->j * stride);
+    const int64_t n2 = n >> 1, G = (int64_t)gridDim.x * SV_THREADS;
+    for (int64_t k0 = (int64_t)blockIdx.x * SV_THREADS + threadIdx.x; k0 < n2; k0 += G * SV_UNROLL) {
+        double2 a[SV_UNROLL];
+#pragma unroll
+        for (int e = 0; e < SV_UNROLL; e++) if (k0 + e * G < n2) a[e] = w2[k0 + e * G];
+#pragma unroll
+        for (int e = 0; e < SV_UNROLL; e++) if (k0 + e * G < n2) o2[k0 + e * G] = make_double2(a[e].x * inv, a[e].y * inv);
+    }
 }
 
 // v_{j+1} = w / h_{j+1,j}
@@ -550,8 +576,9 @@ __global__ void __launch_bounds__(256) k_update_x(double* __restrict__ x, const 
     }
 }
 
-__global__ void k_init_state(GmresState* st, int m, int max_iters, double rtol) {
+__global__ void k_init_state(GmresState* st, int m, int max_iters, double rtol, double reorth_tol) {
     if (threadIdx.x != 0) return;
+    st->nreorth = 0; st->skip2 = 0; st->reorth_tol = reorth_tol;
     st->j = 0; st->iters = 0; st->status = 0; st->cycle_end = 0; st->m = m; st->max_iters = max_iters;
     st->ticket = 0; st->rtol = rtol; st->bn = 0.0; st->beta = 0.0; st->relres = 0.0; st->hn = 0.0; st->inv_hn = 0.0;
 }
@@ -595,6 +622,7 @@ void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stri
 }
 void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
     k_final_v<<<148 * 2, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_scale_v<<<148 * 8, SV_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
 }
 void launch_givens(const Launch& L, GmresState* st) { k_givens<<<1, 32, 0, L.stream>>>(st); count(L); }
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
@@ -603,8 +631,10 @@ void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, 
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st) {
     k_update_x<<<RED_BLOCKS, 256, 0, L.stream>>>(x, Z, stride, n, st); count(L);
 }
-void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol) {
-    k_init_state<<<1, 32, 0, L.stream>>>(st, m, max_iters, rtol); count(L);
+void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol, bool full_cgs2) {
+    static const char* env = getenv("MG_B200_REORTH_TOL");          // experiments only
+    const double tol = full_cgs2 ? -1.0 : (env ? atof(env) : REORTH_TOL);
+    k_init_state<<<1, 32, 0, L.stream>>>(st, m, max_iters, rtol, tol); count(L);
 }
 
 }  // namespace mgb

@@ -424,3 +424,31 @@ def test_w_cycle_gamma2(gpu, oracle_mod):
     xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
     assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
     s.close()
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 257), (3, 129)])
+def test_selective_second_gram_schmidt_update(gpu, oracle_mod, cfg, n):
+    """DESIGN.md G23: skipping the second Gram-Schmidt update where the measured defect ||V^T w'|| <= 1e-13 ||w'||
+    gives the same iterates as running it in every step (MG_SETUP_FULL_CGS2), and both match the oracle."""
+    pl = W.make_plane(cfg, n)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    o.update(pl.lam, pl.c)
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    res = []
+    for full in (False, True):
+        s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, full_cgs2=full)
+        assert s.last_reorth == -1
+        s.update_coeffs(dev(pl.lam), dev(pl.c))
+        x, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+        res.append((host(x), iters, relres, s.last_reorth))
+        assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(x), ro["x"]) <= TOL_SOLVE
+        # mg_last_history: the recurrence residual never increases inside a restart cycle and ends below rtol;
+        # the measured orthogonality defect stays at rounding level (full) / near the skip threshold (selective)
+        r, orth = s.last_history()
+        assert len(r) == iters and len(orth) == iters and r[-1] < 1e-10
+        assert np.all(np.diff(r[:30]) <= 1e-15) and np.all(r > 0)
+        assert orth.max() < (1e-13 if full else 2e-11)
+        s.close()
+    (xa, ia, ra, na), (xb, ib, rb, nb) = res
+    assert nb == ib and 0 <= na <= ia              # full: every step; selective: a subset
+    assert ia == ib and rel(xa, xb) <= 1e-10 and ra == pytest.approx(rb, rel=1e-6)
