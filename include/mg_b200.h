@@ -79,7 +79,8 @@ typedef struct {
                       by default it is skipped in the steps where the measured defect ||V^T w'|| is already
                       <= 1e-13 ||w'|| (G23; same iterates to that level).
                       Other bits must be 0.                                                              */
-    int gamma;     /* cycle index of PAPER.md:187-189, 197: 0 or 1 = V-cycle (default), 2 = W-cycle             */
+    int gamma;     /* cycle index of PAPER.md:187-189, 197: 0 or 1 = V-cycle (default), 2 = W-cycle; 3 = F-cycle
+                      (one F-cycle visit, then one V-cycle visit of the next coarser level)   */
 } mg_options;
 
 /* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).

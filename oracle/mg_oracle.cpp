@@ -71,7 +71,7 @@ struct Oracle {
     std::vector<Level> lev;
     std::vector<int64_t> user2canon;          // user index -> canonical index on level 0
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
-    int gamma = 1;                            // cycle index: 1 V-cycle, 2 W-cycle
+    int gamma = 1;                            // cycle type: 1 V-cycle, 2 W-cycle, 3 F-cycle
     bool have_coeffs = false;
     // coarse factorisation
     std::vector<double> lu;
@@ -410,7 +410,9 @@ static void lu_solve(const std::vector<double>& A, const std::vector<int32_t>& p
 }
 
 // ------------------------------------------------------------------ mg_cycle
-static void mg_cycle(Oracle& o, int s, double* x, const double* b) {
+// kind: 1 = V (gamma = 1), 2 = W (gamma = 2); 3 = F: the next coarser level is visited twice like gamma = 2,
+// first by an F-cycle, then by a V-cycle (the paper names F-cycles at P:258 and defers to its ref. [33]).
+static void mg_cycle(Oracle& o, int s, double* x, const double* b, int kind) {
     Level& lv = o.lev[s];
     if (s == o.L - 1) { lu_solve(o.lu, o.piv, lv.n, b, x); return; }
     for (int k = 0; k < o.nu_pre; k++) gs_sweep(lv, x, b);
@@ -420,7 +422,12 @@ static void mg_cycle(Oracle& o, int s, double* x, const double* b) {
     Level& cv = o.lev[s + 1];
     std::vector<double> dc(cv.n), ec(cv.n, 0.0);                             // P:186 e = 0
     restrict_defect(lv, cv, d.data(), dc.data());
-    for (int g = 0; g < o.gamma; g++) mg_cycle(o, s + 1, ec.data(), dc.data());   // gamma visits, e carried over
+    if (kind == 3) {
+        mg_cycle(o, s + 1, ec.data(), dc.data(), 3);
+        mg_cycle(o, s + 1, ec.data(), dc.data(), 1);
+    } else {
+        for (int g = 0; g < kind; g++) mg_cycle(o, s + 1, ec.data(), dc.data(), kind);   // gamma visits, e carried over
+    }
     std::vector<double> e;
     prolong_correct(lv, ec.data(), x, e);
     for (int k = 0; k < o.nu_post; k++) gs_sweep(lv, x, b);
@@ -497,8 +504,8 @@ void* orc_create(int64_t n, const int32_t* i, const int32_t* j, const uint8_t* k
     return o;
 }
 
-// cycle index gamma of P:187-189 (1 = V, 2 = W); default 1
-void orc_set_gamma(void* h, int gamma) { ((Oracle*)h)->gamma = gamma < 1 ? 1 : gamma; }
+// cycle type: gamma of P:187-189 (1 = V, 2 = W) or 3 = F-cycle; default 1
+void orc_set_gamma(void* h, int gamma) { ((Oracle*)h)->gamma = (gamma < 1 || gamma > 3) ? 1 : gamma; }
 
 int orc_num_levels(void* h) { return ((Oracle*)h)->L; }
 int64_t orc_level_n(void* h, int s) { return ((Oracle*)h)->lev[s].n; }
@@ -587,7 +594,7 @@ void orc_restrict_coeff(void* h, int s, const double* vfine, double* vcoarse) {
 void orc_coarse_solve(void* h, const double* b, double* x) {
     Oracle* o = (Oracle*)h; lu_solve(o->lu, o->piv, o->lev[o->L - 1].n, b, x);
 }
-void orc_cycle(void* h, int s, double* x, const double* b) { mg_cycle(*(Oracle*)h, s, x, b); }
+void orc_cycle(void* h, int s, double* x, const double* b) { mg_cycle(*(Oracle*)h, s, x, b, ((Oracle*)h)->gamma); }
 
 // fGMRES(m) — Saad's flexible GMRES ([12],[29]), rules K1-K5; stop on Eq. 23.
 // Vectors f, x0, x in USER order.  precond: 0 = one V-cycle from zero (G16), 1 = identity,
@@ -628,7 +635,7 @@ int orc_solve_ex(void* h, const double* f_user, const double* x0_user, double* x
         std::fill(H.begin(), H.end(), 0.0);
         int jdone = 0; bool breakdown = false;
         for (int j = 0; j < m && iters < o->max_iters; j++) {
-            if (precond == 0) { std::fill(Z[j].begin(), Z[j].end(), 0.0); mg_cycle(*o, 0, Z[j].data(), V[j].data()); }
+            if (precond == 0) { std::fill(Z[j].begin(), Z[j].end(), 0.0); mg_cycle(*o, 0, Z[j].data(), V[j].data(), o->gamma); }
             else if (precond == 1) Z[j] = V[j];
             else lu_solve(o->lu0, o->piv0, n, V[j].data(), Z[j].data());
             apply(lv, Z[j].data(), w.data());

@@ -45,7 +45,7 @@ struct mg_handle_s {
     HostHierarchy hh;
     int L = 0;
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
-    int gamma = 1;                        // cycle index: 1 V-cycle, 2 W-cycle
+    int gamma = 1;                        // cycle type: 1 V-cycle, 2 W-cycle, 3 F-cycle
     bool full_cgs2 = false;               // MG_SETUP_FULL_CGS2
     int64_t n = 0;
     std::vector<LevelDev> lev;
@@ -122,8 +122,17 @@ VecRef enqueue_smooth(const Launch& L, const LevelDev& lv, VecRef cur, VecRef ot
     return cur;
 }
 
+// Types of the visits a cycle of type `kind` (1 V, 2 W, 3 F) pays to the next coarser level: V: one V;
+// W: two W; F: one F, then one V (the F-cycle of the paper's ref. [33], named at P:258; G24).
+int cycle_visits(int kind, int out[2]) {
+    if (kind == 2) { out[0] = out[1] = 2; return 2; }
+    if (kind == 3) { out[0] = 3; out[1] = 1; return 2; }
+    out[0] = 1;
+    return 1;
+}
+
 // The same schedule as enqueue_cycle below, written as a program for the fused small-level kernel.
-void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailProgram& P) {
+void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailProgram& P, int kind) {
     auto push = [&](TailOp op) { if (P.nops < TAIL_MAX_OPS) P.op[P.nops] = op; P.nops++; };
     const LevelDev& lv = h->lev[s];
     if (s == h->L - 1) { TailOp op{}; op.type = TAIL_COARSE; op.level = (unsigned char)s; op.ntiles = 1; op.a = b; op.b = x; push(op); return; }
@@ -136,21 +145,24 @@ void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailPr
     const bool fuse_dr = !h->no_fused_dr;
     for (int nu = h->nu_pre; nu > 0;) { const int k = nu >= 2 ? 2 : 1; gs(k, (fuse_dr && nu == k) ? 2 : 0, x_is_zero, nullptr); x_is_zero = false; nu -= k; }
     if (!fuse_dr) { TailOp op{}; op.type = TAIL_DR; op.level = (unsigned char)s; op.ntiles = h->lev[s + 1].ntiles; op.a = cur; op.b = h->buf[s + 1].b; op.c = b; push(op); }
-    for (int g = 0; g < h->gamma; g++) build_tail(h, s + 1, h->buf[s + 1].x, h->buf[s + 1].b, g == 0, P);
+    int vk[2];
+    const int nvis = cycle_visits(kind, vk);
+    for (int g = 0; g < nvis; g++) build_tail(h, s + 1, h->buf[s + 1].x, h->buf[s + 1].b, g == 0, P, vk[g]);
     int nu = h->nu_post;
     { const int k = nu >= 2 ? 2 : 1; gs(k, 1, false, h->buf[s + 1].x); nu -= k; }
     while (nu > 0) { const int k = nu >= 2 ? 2 : 1; gs(k, 0, false, nullptr); nu -= k; }
     if (cur != x) { TailOp op{}; op.type = TAIL_COPY; op.level = (unsigned char)s; op.a = cur; op.b = x; op.n = lv.nslots; push(op); }
 }
 
-// mg_cycle of PAPER.md:171-195 with gamma = 1, enqueued on L.stream.  x_is_zero: the initial guess is
+// mg_cycle of PAPER.md:171-195 (cycle type `kind`, 0 = the handle's), enqueued on L.stream.  x_is_zero: the initial guess is
 // the zero vector and x need not be read (nor zeroed beforehand).  w_out: also produce w_out = A x for the
 // result (fused into the last smoothing launch); returns whether it was written.
-bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero, double* w_out = nullptr) {
+bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero, double* w_out = nullptr, int kind = 0) {
     const LevelDev& lv = h->lev[s];
+    if (kind == 0) kind = h->gamma;
     if (s >= h->tail_s0) {                                            // small levels: one cooperative kernel
         TailProgram P; P.nops = 0;
-        build_tail(h, s, TAIL_TOPX, TAIL_TOPB, x_is_zero, P);
+        build_tail(h, s, TAIL_TOPX, TAIL_TOPB, x_is_zero, P, kind);
         if (P.nops <= TAIL_MAX_OPS) {
             int grid = 1;
             for (int i = 0; i < P.nops; i++) grid = std::max(grid, P.op[i].type == TAIL_COPY ? 8 : P.op[i].ntiles);
@@ -172,8 +184,10 @@ bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
                                 fuse_dr ? &h->lev[s + 1] : nullptr, h->buf[s + 1].b);
     VecRef other = (cur.base == x.base) ? tmp : x;
     if (!fuse_dr) launch_defect_restrict(L, lv, h->lev[s + 1], cur, b, h->buf[s + 1].b);  // P:183-184  R (A x - b)
-    for (int g = 0; g < h->gamma; g++)                                                    // e0 = 0, gamma visits
-        enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), g == 0);
+    int vk[2];
+    const int nvis = cycle_visits(kind, vk);
+    for (int g = 0; g < nvis; g++)                                                        // e0 = 0, gamma visits
+        enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), g == 0, nullptr, vk[g]);
     VecRef fin;
     bool wrote_w = false;
     if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass
@@ -274,7 +288,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 2 || (o.flags & ~7) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }

@@ -452,3 +452,23 @@ def test_selective_second_gram_schmidt_update(gpu, oracle_mod, cfg, n):
     (xa, ia, ra, na), (xb, ib, rb, nb) = res
     assert nb == ib and 0 <= na <= ia              # full: every step; selective: a subset
     assert ia == ib and rel(xa, xb) <= 1e-10 and ra == pytest.approx(rb, rel=1e-6)
+
+
+def test_f_cycle_gamma3(gpu, oracle_mod):
+    """F-cycle (mg_options.gamma = 3): cycle and solve parity with the oracle, also through the
+    cooperative small-level kernel."""
+    pl = W.make_plane(3, 129)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, gamma=3)
+    o.update(pl.lam, pl.c)
+    rng = np.random.default_rng(9)
+    n = o.level_n(0)
+    x, b = rng.standard_normal(n), rng.standard_normal(n)
+    ref = o.cycle(0, x, b)
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    for tail in (False, True):
+        s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, gamma=3, fused_tail=tail)
+        s.update_coeffs(dev(pl.lam), dev(pl.c))
+        assert rel(host(s.vcycle(0, dev(x), dev(b))), ref) <= 1e-12
+        xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+        assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
+        s.close()

@@ -232,3 +232,37 @@ def test_w_cycle_gamma2(oracle_mod):
     assert np.linalg.norm(ew) <= 1.05 * np.linalg.norm(ev)
     rv, rw = ov.solve(pl.f, pl.x0, 1e-10), ow.solve(pl.f, pl.x0, 1e-10)
     assert rw["status"] == 0 and rw["iters"] <= rv["iters"]
+
+
+def test_f_cycle(oracle_mod):
+    """F-cycle (via its ref. [33]): the next coarser level is visited by an F-cycle, then by a V-cycle.
+    With two levels it equals the V-cycle, with three levels the W-cycle (below the top level both pay two visits to the
+    exact coarsest solve).  With four levels the level-1 sub-cycles are a W-cycle (three levels: F = W) followed by a
+    V-cycle, so the F-cycle can be composed from the separately pinned V- and W-cycle oracles.  Its contraction lies
+    between theirs."""
+    pl = H.small_annulus(129, 4)
+    rng = np.random.default_rng(4)
+    ov, ow, of = (H.make_oracle(oracle_mod, pl, levels=4, gamma=g) for g in (1, 2, 3))
+    n = ov.level_n(0)
+    x, b = rng.standard_normal(n), rng.standard_normal(n)
+    xs = ov.smooth(0, x, b, 2)
+    dc = ov.restrict(0, ov.apply(0, xs) - b)
+    e = ow.cycle(1, np.zeros(ov.level_n(1)), dc)          # F-cycle on levels 1-3 = W-cycle
+    e = ov.cycle(1, e, dc)                                # then a V-cycle, e carried over
+    ref = ov.smooth(0, ov.prolong_correct(0, e, xs), b, 2)
+    got = of.cycle(0, x, b)
+    assert np.linalg.norm(got - ref) <= 1e-12 * np.linalg.norm(ref)
+    assert np.linalg.norm(got - ov.cycle(0, x, b)) > 1e-6 * np.linalg.norm(ref)      # and it is not the V-cycle
+    assert np.linalg.norm(got - ow.cycle(0, x, b)) > 1e-9 * np.linalg.norm(ref)      # nor the W-cycle
+    for lv, other in ((2, 1), (3, 2)):
+        pls = H.small_annulus(65, lv)
+        oa, ob = H.make_oracle(oracle_mod, pls, levels=lv, gamma=3), H.make_oracle(oracle_mod, pls, levels=lv, gamma=other)
+        xx, bb = rng.standard_normal(oa.level_n(0)), rng.standard_normal(oa.level_n(0))
+        assert np.linalg.norm(oa.cycle(0, xx, bb) - ob.cycle(0, xx, bb)) <= 1e-12 * np.linalg.norm(xx)
+    zero = np.zeros(n)
+    ev, ew, ef = x.copy(), x.copy(), x.copy()
+    for _ in range(6):
+        ev, ew, ef = ov.cycle(0, ev, zero), ow.cycle(0, ew, zero), of.cycle(0, ef, zero)
+    assert np.linalg.norm(ew) <= 1.05 * np.linalg.norm(ef) <= 1.05 * 1.05 * np.linalg.norm(ev)
+    rf = of.solve(pl.f, pl.x0, 1e-10)
+    assert rf["status"] == 0 and rf["iters"] <= ov.solve(pl.f, pl.x0, 1e-10)["iters"]
