@@ -201,13 +201,13 @@ def run_ours(args):
     def step_device(k):
         lam, c, f = d_in[k if warm else 0]
         s.update_coeffs(lam, c)
-        _, iters, relres, rc = s.solve(f, d_x if (warm and k > 0) else d_x0, RTOL, x=d_x)   # d_x may alias d_x0
+        _, iters, relres, rc = s.solve(f, d_x if (warm and k > 0) else d_x0, args.rtol, x=d_x)   # d_x may alias d_x0
         return iters, relres, rc
 
     def step_host(k):
         lam, c, f = h_in[k if warm else 0]
         s.update_coeffs_host(lam, c)
-        _, iters, relres, rc = s.solve_host(f, h_x if (warm and k > 0) else h_x0, RTOL, x=h_x)
+        _, iters, relres, rc = s.solve_host(f, h_x if (warm and k > 0) else h_x0, args.rtol, x=h_x)
         return iters, relres, rc
 
     def timed(step, first, steps):
@@ -280,7 +280,7 @@ def run_ours(args):
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config] + (f" [geometry on a {args.lattice}^2 lattice]" if args.lattice else ""),
-                           "unknowns_per_plane": pl.n, "planes": world, "rtol": RTOL,
+                           "unknowns_per_plane": pl.n, "planes": world, "rtol": args.rtol,
                            "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels,
                            "step": "mg_update_coeffs + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
                            "l2_policy": "inputs larger than L2 (no flush)" if pl.n * 8 * 8 > 126e6 else "working set fits L2 (small config)"},
@@ -433,6 +433,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--ref-iters", type=int, default=8, help="iteration cap of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--rtol", type=float, default=RTOL, help="stop tolerance of Eq. 23 (scaling runs beyond the BASELINE sizes; default 1e-10)")
     ap.add_argument("--full-cgs2", action="store_true", help="always run the second Gram-Schmidt update (MG_SETUP_FULL_CGS2)")
     ap.add_argument("--roofline-only", action="store_true", help="launch only the roofline kernel (for ncu captures)")
     ap.add_argument("--lattice", type=int, default=None, help="same geometry on an n x n lattice (2^k + 1; O(N) scaling runs)")

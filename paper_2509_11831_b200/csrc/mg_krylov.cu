@@ -7,7 +7,8 @@
 // Orthogonalisation: classical Gram-Schmidt applied twice (CGS2).  Same Krylov iterates as the oracle's modified
 // Gram-Schmidt (also applied twice) up to rounding.  For restart lengths m <= 32 the two projections take
 // THREE passes over the basis (k_multidot_tma, k_update_dot_tma, k_final_v: see the block comment further down),
-// the first two staged through shared memory by TMA bulk copies; longer restarts use the plain four-pass
+// the first two staged through shared memory by TMA bulk copies, the third skipped in the steps whose measured
+// orthogonality defect is already below REORTH_TOL (k_scale_v instead); longer restarts use the plain four-pass
 // form (k_multidot, k_update_w twice, k_givens, k_next_v).  Grid reductions: per-block partials +
 // last-block-done ticket, summed in a fixed order (deterministic run to run).
 #include <cstdlib>
@@ -200,7 +201,9 @@ __global__ void k_givens(GmresState* st) {
 //                           block then forms h = h1 + h2, h_{j+1,j} = sqrt(||w'||^2 - sum h2^2) (exact for
 //                           orthonormal V; h2 = O(eps) after the first projection so nothing cancels) and runs
 //                           the Givens step, so no separate norm pass and no separate Givens launch
-//   pass 3  k_final_v       v_{j+1} = (w' - V h2) / h_{j+1,j}, written straight into the basis
+//   pass 3  k_final_v       v_{j+1} = (w' - V h2) / h_{j+1,j}, written straight into the basis; where
+//                           ||h2|| <= REORTH_TOL ||w'|| (decided in pass 2's last block) the step keeps h = h1,
+//                           h_{j+1,j} = ||w'|| and k_scale_v writes v_{j+1} = w' / ||w'|| without reading the basis
 // Traffic at column j: 8(j+2) + (16 + 8(j+1)) + (16 + 8(j+1)) = 24 j + 64 B/pt against 32 j + 96.
 constexpr int FUSED_NV = 32;
 constexpr double REORTH_TOL = 1e-13;   // second update skipped when ||V^T w'|| <= REORTH_TOL ||w'|| (G23)
