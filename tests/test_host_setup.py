@@ -35,6 +35,13 @@ def test_error_codes_without_device():
     # compute calls on a host-only handle fail loudly (no CPU fallback)
     assert L.mg_update_coeffs(s._h, C.c_void_p(8), C.c_void_p(8), None) == -5
     assert L.mg_apply(s._h, 0, C.c_void_p(8), C.c_void_p(8), None) == -5
+    # diagnostics before the first solve; option range (gamma 0..3, flag bits 0..2)
+    assert s.last_reorth == -1 and len(s.last_history()[0]) == 0
+    assert L.mg_last_history(None, None, None, 4) == -1 and L.mg_last_reorth(None) == -1
+    for g in (0, 1, 2, 3):
+        B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=1, host_only=True, gamma=g, full_cgs2=True).close()
+    with pytest.raises(B.MgError):
+        B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=1, host_only=True, gamma=4)
     with pytest.raises(B.MgError):
         B.Solver(pl.i, pl.j, pl.kind, -1.0, host_only=True)
     with pytest.raises(B.MgError):
