@@ -34,6 +34,7 @@ typedef struct mg_handle_s* mg_handle;
 #define MG_SETUP_HOST_ONLY 1
 #define MG_SETUP_FUSED_TAIL 2
 #define MG_SETUP_FULL_CGS2 4
+#define MG_NU_NONE (-1) /* mg_options.nu_post: no post-smoothing (0 means "default") */
 
 enum {
     MG_OK = 0,
@@ -67,7 +68,7 @@ typedef struct {
 typedef struct {
     int levels;    /* N_sigma; 0 = auto: coarsen while the bounding lattice > 9x9 and |Inner| >= 16 (M8) */
     int nu_pre;    /* nsmooth_pre, default 2; must be >= 1 (rule T2)                     */
-    int nu_post;   /* nsmooth_post, default 2                                             */
+    int nu_post;   /* nsmooth_post, default 2; MG_NU_NONE = no post-smoothing, V(nu_pre,0)      */
     int restart_m; /* fGMRES restart length m, default 30, max 64                                        */
     int max_iters; /* cap on preconditioner applications, default 200                                    */
     int flags;     /* bit 0 (MG_SETUP_HOST_ONLY): build the host hierarchy only, touch no device; only the

@@ -112,9 +112,12 @@ class Solver:
         j = np.ascontiguousarray(j, dtype=np.int32)
         kind = np.ascontiguousarray(kind, dtype=np.uint8)
         self.n = int(i.shape[0])
+        if int(nu_pre) < 1 or int(nu_post) < 0:
+            raise ValueError("nu_pre must be >= 1 (rule T2) and nu_post >= 0")
         mesh = _Mesh(self.n, i.ctypes.data, j.ctypes.data, float(h))
         bc = _Bc(kind.ctypes.data)
-        opt = _Options(int(levels), int(nu_pre), int(nu_post), int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma))
+        opt = _Options(int(levels), int(nu_pre), int(nu_post) if int(nu_post) != 0 else -1,   # 0 sweeps = MG_NU_NONE
+                        int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma))
         hd = C.c_void_p()
         rc = L.mg_setup(C.byref(mesh), C.byref(bc), C.byref(opt), None if host_only else _stream_ptr(stream), C.byref(hd))
         if rc:

@@ -288,14 +288,14 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < 0 || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < MG_NU_NONE || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
     mg_handle h = new (std::nothrow) mg_handle_s();
     if (!h) return MG_ENOMEM;
     h->nu_pre = o.nu_pre ? o.nu_pre : 2;
-    h->nu_post = o.nu_post ? o.nu_post : 2;
+    h->nu_post = o.nu_post == 0 ? 2 : (o.nu_post == MG_NU_NONE ? 0 : o.nu_post);
     h->m = o.restart_m ? o.restart_m : 30;
     h->max_iters = o.max_iters ? o.max_iters : 200;
     h->gamma = o.gamma > 1 ? o.gamma : 1;

@@ -472,3 +472,50 @@ def test_f_cycle_gamma3(gpu, oracle_mod):
         xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
         assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
         s.close()
+
+
+@pytest.mark.parametrize("seed", list(range(200, 216)))
+def test_random_mesh_and_options(gpu, oracle_mod, seed):
+    """Seeded sweep over ragged random domains x solver options: lattice size, V(nu1,nu2) including no post-smoothing
+    (MG_NU_NONE), V/W/F cycle, restart length (fused and unfused Gram-Schmidt paths), cooperative small-level kernel,
+    selective / full second Gram-Schmidt update.  Cycle parity 1e-12, solve parity as in test_solve."""
+    rng = np.random.default_rng(seed)
+    n = int(rng.choice([65, 97, 129, 161, 257]))
+    nu1, nu2 = max(1, int(rng.integers(0, 4))), int(rng.integers(0, 4))
+    gamma, m = int(rng.choice([1, 1, 2, 3])), int(rng.choice([3, 10, 30, 40]))
+    tail, full = bool(rng.integers(0, 2)), bool(rng.integers(0, 2))
+    pl = H.random_blob_plane(seed, n)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=nu1, nu_post=nu2, m=m, gamma=gamma, max_iters=120)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=nu1, nu_post=nu2, restart_m=m, gamma=gamma, max_iters=120,
+                   fused_tail=tail, full_cgs2=full)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    n0 = o.level_n(0)
+    x, b = rng.standard_normal(n0), rng.standard_normal(n0)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    s.close()
+    assert rc == ro["status"] and abs(iters - ro["iters"]) <= 1
+    if rc == 0:
+        assert rel(host(xg), ro["x"]) <= TOL_SOLVE
+
+
+def test_no_post_smoothing(gpu, oracle_mod):
+    """V(2,0): nu_post = 0 in the binding = MG_NU_NONE in the C ABI (0 there means "default"); the correction is then
+    applied by the stand-alone prolongation kernel and w = A z by the stand-alone operator kernel."""
+    pl = W.make_plane(3, 129)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=2, nu_post=0)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=2, nu_post=0)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    rng = np.random.default_rng(12)
+    n = o.level_n(0)
+    x, b = rng.standard_normal(n), rng.standard_normal(n)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
+    with pytest.raises(ValueError):
+        gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=0)
+    s.close()
