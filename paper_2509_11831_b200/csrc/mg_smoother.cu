@@ -33,7 +33,8 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
 // Levels of at most SUB_MAX_TILES tiles are latency bound (7-25 us per launch whatever the tile count,
 // profiles/r01c_small_levels.md): they run with one CTA per SBX x SBY block, 8 CTAs per tile.
 constexpr int SUB_MAX_TILES = 40, SBX = 16, SBY = 16;      // 8 CTAs per tile
-constexpr int MID_MAX_TILES = 148, MBX = 32, MBY = 16;     // 4 CTAs per tile
+constexpr int MID_MAX_TILES = 74, MBX = 32, MBY = 16;      // 4 CTAs per tile: at most 296 CTAs = one wave at 2 CTAs per SM
+constexpr int HALF_MAX_TILES = 148, HBX = 64, HBY = 16;    // 2 CTAs per tile: one wave up to 148 tiles
 
 template <int NS, bool PC, int EPI, int BX, int BY>
 void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
@@ -55,6 +56,7 @@ void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, Vec
     static const bool no_sub = getenv("MG_B200_NO_SUBBLOCKS") != nullptr;
     if (lv.ntiles <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else if (lv.ntiles <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else if (lv.ntiles <= HALF_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, HBX, HBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else launch_blk<NS, PC, EPI, TX, TY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
 }
 
