@@ -61,6 +61,7 @@ struct Level {
     std::vector<double> parent_w;             // 4n
     std::vector<uint8_t> ptype;               // 0 coincident, 1 R-edge, 2 Z-edge, 3 centre
     std::vector<double> lam, c;
+    std::vector<double> xi;                   // the paper's third field (Eq. 3, Eq. 10); 1 unless orc_update3 set it
     Lookup lut;
 };
 
@@ -250,7 +251,8 @@ static void build_transfers(Level& f, const Level& c) {
 // Dirichlet: Eq. 11; Neumann: Eq. 16 with phi^N of rule D3.
 static inline double row_apply(const Level& lv, int64_t l, const double* x) {
     if (lv.kind[l] == INNER) {
-        const double kappa = 1.0 / (2.0 * lv.h * lv.h);
+        // Eq. 10: the bracket carries xi_{i,j}/2 of the ROW's own point; 1/h^2 restored (reading G1)
+        const double kappa = 1.0 / (2.0 * lv.h * lv.h) * lv.xi[l];
         const int32_t* nb = &lv.nbr[4 * l];
         const double cl = lv.c[l];
         const double aW = kappa * (cl + lv.c[nb[0]]);
@@ -278,10 +280,11 @@ static void apply(const Level& lv, const double* x, double* y) {
 
 // One group of gauss_seidel_rbb: group 0 red inner, 1 black inner, 2 boundary.
 static void gs_group(const Level& lv, double* x, const double* b, int group) {
-    const double kappa = 1.0 / (2.0 * lv.h * lv.h);
+    const double kappa0 = 1.0 / (2.0 * lv.h * lv.h);
     for (int64_t l = 0; l < lv.n; l++) {
         if (lv.colour[l] != group) continue;
         if (lv.kind[l] == INNER) {
+            const double kappa = kappa0 * lv.xi[l];                  // xi_{i,j}/2 of Eq. 10
             const int32_t* nb = &lv.nbr[4 * l];
             const double cl = lv.c[l];
             const double aW = kappa * (cl + lv.c[nb[0]]);
@@ -500,7 +503,7 @@ void* orc_create(int64_t n, const int32_t* i, const int32_t* j, const uint8_t* k
         build_transfers(o->lev[o->lev.size() - 2], o->lev.back());
     }
     o->L = (int)o->lev.size();
-    for (auto& lv : o->lev) { lv.lam.assign(lv.n, 0.0); lv.c.assign(lv.n, 0.0); }
+    for (auto& lv : o->lev) { lv.lam.assign(lv.n, 0.0); lv.c.assign(lv.n, 0.0); lv.xi.assign(lv.n, 1.0); }
     return o;
 }
 
@@ -549,25 +552,38 @@ void orc_transfer_tables(void* h, int s, int32_t* fine9, int32_t* parent, double
 // "update": coefficients in USER order on all points; T4 to all coarser levels;
 // LU-factorise the coarsest operator.  Returns 0, or -1 if a coefficient is not admissible (c <= 0 or non-finite),
 // -2 if the coarsest matrix is singular.
-int orc_update(void* h, const double* lam, const double* c) {
+// xi == NULL: the two-field form of BASELINE.json (paper xi = 1).  Otherwise xi is the paper's third field
+// (Eq. 3; Eq. 10), grid-transferred like lambda and c ("lambda, xi, c") and required > 0.
+int orc_update3(void* h, const double* lam, const double* xi, const double* c) {
     Oracle* o = (Oracle*)h;
     Level& l0 = o->lev[0];
     for (int64_t k = 0; k < l0.n; k++) {
         // c > 0 is required; lambda >= 0 is only the paper's sufficient condition for positive definiteness and its own
         // verification case has lambda = r sin(theta) of both signs (Eq. 21), so lambda is only required to be finite
         if (!(c[k] > 0.0) || !std::isfinite(c[k]) || !std::isfinite(lam[k])) { g_err = "need c>0 and finite lambda"; return -1; }
+        if (xi && (!(xi[k] > 0.0) || !std::isfinite(xi[k]))) { g_err = "need xi>0"; return -1; }
         l0.lam[o->user2canon[k]] = lam[k];
         l0.c[o->user2canon[k]] = c[k];
+        l0.xi[o->user2canon[k]] = xi ? xi[k] : 1.0;
     }
     for (int s = 0; s + 1 < o->L; s++) {
         restrict_coeff(o->lev[s], o->lev[s + 1], o->lev[s].lam.data(), o->lev[s + 1].lam.data());
         restrict_coeff(o->lev[s], o->lev[s + 1], o->lev[s].c.data(), o->lev[s + 1].c.data());
+        if (xi) restrict_coeff(o->lev[s], o->lev[s + 1], o->lev[s].xi.data(), o->lev[s + 1].xi.data());
+        else o->lev[s + 1].xi.assign(o->lev[s + 1].n, 1.0);
     }
     assemble_dense(o->lev[o->L - 1], o->lu);
     if (!lu_factor(o->lu, o->piv, o->lev[o->L - 1].n)) { g_err = "singular coarsest operator"; return -2; }
     o->have_coeffs = true;
     o->lu0.clear();
     return 0;
+}
+
+int orc_update(void* h, const double* lam, const double* c) { return orc_update3(h, lam, nullptr, c); }
+
+void orc_level_xi(void* h, int s, double* xi) {
+    Level& lv = ((Oracle*)h)->lev[s];
+    std::memcpy(xi, lv.xi.data(), 8 * lv.n);
 }
 
 void orc_level_coeffs(void* h, int s, double* lam, double* c) {

@@ -40,7 +40,7 @@ def lib():
         _lib.orc_level_n.restype = C.c_int64
         _lib.orc_level_h.restype = C.c_double
         for name in ("orc_destroy", "orc_num_levels", "orc_level_n", "orc_level_h", "orc_user_perm",
-                     "orc_level_arrays", "orc_transfer_tables", "orc_update", "orc_level_coeffs",
+                     "orc_level_arrays", "orc_transfer_tables", "orc_update", "orc_update3", "orc_level_xi", "orc_level_coeffs",
                      "orc_apply", "orc_smooth", "orc_smooth_group", "orc_restrict", "orc_prolong_correct",
                      "orc_restrict_coeff", "orc_coarse_solve", "orc_cycle", "orc_solve_ex"):
             getattr(_lib, name).argtypes = None
@@ -121,6 +121,19 @@ class Oracle:
         rc = lib().orc_update(self._h, C.c_void_p(lam.ctypes.data), C.c_void_p(c.ctypes.data))
         if rc != 0:
             raise ValueError("oracle update: " + lib().orc_last_error().decode())
+
+    def update3(self, lam, xi, c):
+        """Three-field form lambda*phi - xi*div(c grad phi) = rho (Eq. 3, Eq. 10)."""
+        lam, xi, c = _d(lam), _d(xi), _d(c)
+        assert lam.shape[0] == self.n and c.shape[0] == self.n and xi.shape[0] == self.n
+        rc = lib().orc_update3(self._h, C.c_void_p(lam.ctypes.data), C.c_void_p(xi.ctypes.data), C.c_void_p(c.ctypes.data))
+        if rc != 0:
+            raise ValueError("oracle update: " + lib().orc_last_error().decode())
+
+    def level_xi(self, s):
+        xi = np.empty(self.level_n(s))
+        lib().orc_level_xi(self._h, int(s), C.c_void_p(xi.ctypes.data))
+        return xi
 
     def apply(self, s, x):
         x = _d(x); y = np.empty_like(x)
