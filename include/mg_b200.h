@@ -100,6 +100,14 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
  * operator (rule C) on the device.  Asynchronous on `stream`. */
 int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream);
 
+/* update for the paper's three-field form  lambda phi - xi div(c grad phi) = rho  (Eq. 3; the row of
+ * point (i,j) carries xi_{i,j}/2, Eq. 10).  d_xi: DEVICE, length n, user order, > 0 on inner points
+ * (guard rows, Eq. 11 / 16, do not see it); it is transferred to the coarser levels like lambda and c
+ * (PAPER.md:153, 207).  d_xi == NULL is mg_update_coeffs (xi = 1).  The handle keeps the form of the
+ * last update; switching forms re-captures the iteration graph at the next solve.  The stop test of mg_solve is
+ * on the residual of the three-field rows.  Costs 8 B per point and smoothing launch more than the two-field form. */
+int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, const double* d_c, void* stream);
+
 /* solve: fGMRES(m) with one V-cycle as right preconditioner (rules K1-K5), stopping
  * on ||A x - f|| / ||f|| < rtol (Eq. 23).  d_f, d_x0, d_x: DEVICE, length n, user order;
  * d_x may alias d_x0.  iters (HOST, may be NULL) receives the number of preconditioner applications,
@@ -111,6 +119,7 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
 /* Same two calls with HOST buffers (pageable or pinned): the library stages them through device
  * buffers it owns; copies run on `stream` (PAPER.md:217 describes exactly this transfer pattern). */
 int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c, void* stream);
+int mg_update_coeffs3_host(mg_handle h, const double* h_lambda, const double* h_xi, const double* h_c, void* stream);
 int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_x, double rtol, int* iters,
                   double* final_relres, void* stream);
 
@@ -133,6 +142,8 @@ int mg_level_info(mg_handle h, int level, int32_t* I, int32_t* J, uint8_t* kind,
 int mg_transfer_info(mg_handle h, int level, int32_t* fine9, int32_t* parent, uint8_t* ptype);
 /* Current coefficients of a level (DEVICE -> HOST copy, canonical order). */
 int mg_level_coeffs(mg_handle h, int level, double* h_lambda, double* h_c, void* stream);
+/* xi of a level (DEVICE -> HOST copy, canonical order; all 1 in the two-field form). */
+int mg_level_xi(mg_handle h, int level, double* h_xi, void* stream);
 
 /* ---- single steps, for parity tests.  DEVICE level vectors in canonical order ------------------ */
 int mg_apply(mg_handle h, int level, const double* d_x, double* d_y, void* stream);            /* y = A x (D1-D3) */

@@ -40,7 +40,7 @@ class _Options(C.Structure):
                 ("max_iters", C.c_int), ("flags", C.c_int), ("gamma", C.c_int)]
 
 
-EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_solve", "mg_update_coeffs_host",
+EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_update_coeffs3", "mg_update_coeffs3_host", "mg_level_xi", "mg_solve", "mg_update_coeffs_host",
            "mg_solve_host", "mg_destroy", "mg_num_levels", "mg_level_n", "mg_level_info", "mg_transfer_info",
            "mg_level_coeffs", "mg_apply", "mg_smooth", "mg_restrict", "mg_smooth_restrict", "mg_prolong_correct", "mg_coarse_solve",
            "mg_vcycle", "mg_kernel_launches", "mg_last_solve_ms", "mg_last_update_ms", "mg_last_step_ms", "mg_last_reorth", "mg_last_history", "mg_strerror",
@@ -142,6 +142,26 @@ class Solver:
         rc = lib().mg_update_coeffs(self._h, _dptr(lam), _dptr(c), _stream_ptr(stream))
         if rc:
             raise MgError(rc, "mg_update_coeffs")
+
+    def update_coeffs3(self, lam, xi, c, stream=None):
+        """Three-field form lambda phi - xi div(c grad phi) = rho (Eq. 3); xi=None is update_coeffs."""
+        rc = lib().mg_update_coeffs3(self._h, _dptr(lam), _dptr(xi) if xi is not None else None, _dptr(c), _stream_ptr(stream))
+        if rc:
+            raise MgError(rc, "mg_update_coeffs3")
+
+    def update_coeffs3_host(self, lam, xi, c, stream=None):
+        lam, xi, c = (np.ascontiguousarray(a, dtype=np.float64) for a in (lam, xi, c))
+        rc = lib().mg_update_coeffs3_host(self._h, C.c_void_p(lam.ctypes.data), C.c_void_p(xi.ctypes.data),
+                                          C.c_void_p(c.ctypes.data), _stream_ptr(stream))
+        if rc:
+            raise MgError(rc, "mg_update_coeffs3_host")
+
+    def level_xi(self, s, stream=None):
+        xi = np.empty(self.level_n(s))
+        rc = lib().mg_level_xi(self._h, int(s), C.c_void_p(xi.ctypes.data), _stream_ptr(stream))
+        if rc:
+            raise MgError(rc, "mg_level_xi")
+        return xi
 
     def solve(self, f, x0, rtol, x=None, stream=None):
         import torch

@@ -34,6 +34,7 @@ struct LevelBuf {           // device arrays owned per level
     uint16_t* code = nullptr;
     uint8_t* tflag = nullptr;
     int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
+    double *xi = nullptr, *rxi = nullptr;   // three-field form only: allocated by the first mg_update_coeffs3 with xi
     double *lam = nullptr, *c = nullptr, *rd = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
     double* tb = nullptr;   // right-hand side of the single-step entry points.  The cycle's own b of a coarse level is written ONLY by
                             // the restriction kernels: slots of coarse points under no fine tile are never written and must stay 0.
@@ -67,6 +68,8 @@ struct mg_handle_s {
     double *cwork = nullptr, *Ainv = nullptr;
     // host-buffer staging
     double* stage[3] = {nullptr, nullptr, nullptr};
+    double* stage_xi = nullptr;
+    bool three_field = false;             // the level structs carry xi / rxi (Eq. 3)
     bool have_coeffs = false;
     bool no_fused_dr = false;             // debugging: separate defect + restriction kernel
     cudaError_t tail_err = cudaSuccess;
@@ -345,6 +348,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         d.nslots = hl.nslots();
         d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
         d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c; d.rd = b.rd; d.tflag = b.tflag;
+        d.xi = nullptr; d.rxi = nullptr;
     }
     TRY(dev_alloc(h, (void**)&h->d_lev, sizeof(LevelDev) * h->L, s));
     CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
@@ -383,14 +387,40 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
 // ============================================================================ update / solve
 extern "C" {
 
-int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream) {
+// Switch the level structs between the two-field (xi, rxi null) and the three-field form.  The structs are kernel
+// arguments baked into the captured iteration graph and copied to the device for the fused small-level kernel, so
+// both are refreshed.
+static int set_three_field(mg_handle h, bool on, cudaStream_t s) {
+    if (h->three_field == on) return MG_OK;
+    for (int l = 0; l < h->L; l++) {
+        LevelBuf& b = h->buf[l];
+        if (on && !b.xi) {
+            const size_t vb = (size_t)h->hh.lev[l].nslots() * sizeof(double);
+            int rc = dev_alloc(h, (void**)&b.xi, vb, s); if (rc) return rc;
+            rc = dev_alloc(h, (void**)&b.rxi, vb, s); if (rc) return rc;
+        }
+        h->lev[l].xi = on ? b.xi : nullptr;
+        h->lev[l].rxi = on ? b.rxi : nullptr;
+    }
+    CU(cudaStreamSynchronize(s));         // h->lev is pageable host memory: the copy below must not overlap a later change
+    CU(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));
+    if (h->iter_graph) { cudaGraphExecDestroy(h->iter_graph); h->iter_graph = nullptr; }
+    h->three_field = on;
+    return MG_OK;
+}
+
+int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, const double* d_c, void* stream) {
     if (!h || !d_lambda || !d_c) return MG_EINVAL;
     if (h->host_only) return MG_ECUDA;
     cudaStream_t s = (cudaStream_t)stream;
+    int rc = set_three_field(h, d_xi != nullptr, s);
+    if (rc) return rc;
     Launch L = LZ(h, s);
     CU(cudaEventRecord(h->ev[2], s));
     launch_gather(L, d_lambda, h->user2slot, h->buf[0].lam, h->n);
     launch_gather(L, d_c, h->user2slot, h->buf[0].c, h->n);
+    if (d_xi) launch_gather(L, d_xi, h->user2slot, h->buf[0].xi, h->n);
     for (int l = 0; l + 1 < h->L; l++) launch_restrict_coeff(L, h->lev[l], h->lev[l + 1]);     // rule T4
     for (int l = 0; l < h->L; l++) launch_diag(L, h->lev[l]);                                   // U2: 1 / a_ll for the smoother
     launch_coarse_factor(L, h->lev[h->L - 1], h->cslot, h->slot2row, h->nL, h->cwork, h->Ainv);   // rule C
@@ -399,6 +429,10 @@ int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, voi
     h->have_coeffs = true;
     h->update_timed = true;
     return MG_OK;
+}
+
+int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream) {
+    return mg_update_coeffs3(h, d_lambda, nullptr, d_c, stream);
 }
 
 int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, double rtol, int* iters,
@@ -467,6 +501,19 @@ int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c
     CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
     CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
     return mg_update_coeffs(h, h->stage[0], h->stage[1], stream);
+}
+
+int mg_update_coeffs3_host(mg_handle h, const double* h_lambda, const double* h_xi, const double* h_c, void* stream) {
+    if (!h || !h_lambda || !h_c) return MG_EINVAL;
+    if (!h_xi) return mg_update_coeffs_host(h, h_lambda, h_c, stream);
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_stage(h, s);
+    if (rc) return rc;
+    if (!h->stage_xi) { rc = dev_alloc(h, (void**)&h->stage_xi, sizeof(double) * (size_t)h->n, s); if (rc) return rc; }
+    CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage_xi, h_xi, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    return mg_update_coeffs3(h, h->stage[0], h->stage_xi, h->stage[1], stream);
 }
 
 int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_x, double rtol, int* iters,
@@ -619,6 +666,19 @@ int mg_level_coeffs(mg_handle h, int level, double* h_lambda, double* h_c, void*
         CU(cudaStreamSynchronize(s));
         for (int64_t q = 0; q < lv.n; q++) out[q] = tmp[lv.canon2slot[q]];
     }
+    return MG_OK;
+}
+
+int mg_level_xi(mg_handle h, int level, double* h_xi, void* stream) {
+    if (!h || level < 0 || level >= h->L || !h_xi) return MG_EINVAL;
+    if (!h->have_coeffs) return MG_ENOTREADY;
+    cudaStream_t s = (cudaStream_t)stream;
+    const HostLevel& lv = h->hh.lev[level];
+    if (!h->three_field) { for (int64_t q = 0; q < lv.n; q++) h_xi[q] = 1.0; return MG_OK; }
+    std::vector<double> tmp((size_t)lv.nslots());
+    CU(cudaMemcpyAsync(tmp.data(), h->buf[level].xi, tmp.size() * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    for (int64_t q = 0; q < lv.n; q++) h_xi[q] = tmp[lv.canon2slot[q]];
     return MG_OK;
 }
 

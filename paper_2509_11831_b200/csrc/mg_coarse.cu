@@ -38,7 +38,8 @@ __global__ void k_coarse_assemble(LevelDev lv, const int32_t* __restrict__ cslot
         const double cl = lv.c[s];
         double all = lv.lam[s];
         double a[4];
-        for (int d = 0; d < 4; d++) { a[d] = lv.kappa * (cl + lv.c[sn[d]]); }
+        const double kap = lv.xi ? lv.kappa * lv.xi[s] : lv.kappa;           // xi_{i,j} / (2 h^2), Eq. 10
+        for (int d = 0; d < 4; d++) { a[d] = kap * (cl + lv.c[sn[d]]); }
         all = lv.lam[s] + a[0] + a[1] + a[2] + a[3];
         row[r] = all;
         for (int d = 0; d < 4; d++) row[slot2row[sn[d]]] = -a[d];

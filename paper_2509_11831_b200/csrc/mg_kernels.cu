@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev c
     for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
         const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
         const int64_t s = (int64_t)t * TS + ly * TX + lx;
-        double sl = 0.0, sc = 0.0, sw = 0.0;
+        double sl = 0.0, sc = 0.0, sw = 0.0, sx = 0.0;
         if ((coarse.code[s] & 3) != C_ABSENT) {
 #pragma unroll
             for (int dy = -1; dy <= 1; dy++)
@@ -118,12 +118,16 @@ __global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev c
                 for (int dx = -1; dx <= 1; dx++) {
                     const int64_t fs = fine_slot(ct, 2 * lx + dx, 2 * ly + dy);
                     const double w = (dx == 0 ? 2.0 : 1.0) * (dy == 0 ? 2.0 : 1.0) * 0.0625;
-                    if ((fine.code[fs] & 3) != C_ABSENT) { sl += w * fine.lam[fs]; sc += w * fine.c[fs]; sw += w; }
+                    if ((fine.code[fs] & 3) != C_ABSENT) {
+                        sl += w * fine.lam[fs]; sc += w * fine.c[fs]; sw += w;
+                        if (fine.xi) sx += w * fine.xi[fs];
+                    }
                 }
-            sl /= sw; sc /= sw;
+            sl /= sw; sc /= sw; sx /= sw;
         }
         coarse.lam[s] = sl;
         coarse.c[s] = sc;
+        if (fine.xi) coarse.xi[s] = sx;
     }
 }
 
@@ -141,14 +145,18 @@ __global__ void __launch_bounds__(NT) k_diag(LevelDev lv) {
     for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
         const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
         const int64_t s = (int64_t)t * TS + ly * TX + lx;
-        double r = 0.0;
+        double r = 0.0, rx = 1.0;
         if ((lv.code[s] & 3) == C_INNER) {
             const double cl = lv.c[s];
-            const double aW = lv.kappa * (cl + lv.c[nslot(tn, lx - 1, ly)]), aE = lv.kappa * (cl + lv.c[nslot(tn, lx + 1, ly)]);
-            const double aS = lv.kappa * (cl + lv.c[nslot(tn, lx, ly - 1)]), aN = lv.kappa * (cl + lv.c[nslot(tn, lx, ly + 1)]);
-            r = 1.0 / (lv.lam[s] + aW + aE + aS + aN);
+            const double xi = lv.xi ? lv.xi[s] : 1.0;
+            const double kap = lv.xi ? lv.kappa * xi : lv.kappa;                 // xi_{i,j} / (2 h^2), Eq. 10
+            const double aW = kap * (cl + lv.c[nslot(tn, lx - 1, ly)]), aE = kap * (cl + lv.c[nslot(tn, lx + 1, ly)]);
+            const double aS = kap * (cl + lv.c[nslot(tn, lx, ly - 1)]), aN = kap * (cl + lv.c[nslot(tn, lx, ly + 1)]);
+            r = xi / (lv.lam[s] + aW + aE + aS + aN);                            // the smoother's row is divided by xi
+            rx = 1.0 / xi;
         }
         lv.rd[s] = r;
+        if (lv.rxi) lv.rxi[s] = rx;
     }
 }
 

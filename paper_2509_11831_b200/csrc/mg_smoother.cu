@@ -12,7 +12,7 @@ namespace {
 // EPI = 1: additionally d_c = R (A x_out - b) on the next coarser level (ccode = its point codes, dc = d_c).
 // EPI = 2: additionally w = A x_out (dc = w).
 // BX x BY < tile: several CTAs per tile (blockIdx = tile * blocks-per-tile + block).
-template <int NS, bool PC, int EPI, int BX, int BY>
+template <int NS, bool PC, int EPI, int BX, int BY, int XIM>
 __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
                                               int xin_zero, const uint16_t* __restrict__ ccode, double* __restrict__ dc,
                                               const int* __restrict__ stop) {
@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
     if (stop != nullptr && *stop) return;
     constexpr int NBX = TX / BX, NSUB = NBX * (TY / BY);
     const int t = blockIdx.x / NSUB, sub = blockIdx.x - t * NSUB;
-    gs_tile<NS, PC, false, EPI, BX, BY>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
+    gs_tile<NS, PC, false, EPI, BX, BY, XIM>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
                                        (sub % NBX) * BX, (sub / NBX) * BY);
 }
 
@@ -36,18 +36,26 @@ constexpr int SUB_MAX_TILES = 40, SBX = 16, SBY = 16;      // 8 CTAs per tile
 constexpr int MID_MAX_TILES = 74, MBX = 32, MBY = 16;      // 4 CTAs per tile: at most 296 CTAs = one wave at 2 CTAs per SM
 constexpr int HALF_MAX_TILES = 148, HBX = 64, HBY = 16;    // 2 CTAs per tile: one wave up to 148 tiles
 
-template <int NS, bool PC, int EPI, int BX, int BY>
-void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
-                const uint16_t* ccode, double* dc) {
+template <int NS, bool PC, int EPI, int BX, int BY, int XIM>
+void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
+                  const uint16_t* ccode, double* dc) {
     constexpr size_t smem = Geo<NS, PC, EPI, BX, BY>::SMEM;
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_gs<NS, PC, EPI, BX, BY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(k_gs<NS, PC, EPI, BX, BY, XIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = true;
     }
     const int grid = lv.ntiles * (TX / BX) * (TY / BY);
-    k_gs<NS, PC, EPI, BX, BY><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
+    k_gs<NS, PC, EPI, BX, BY, XIM><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
     if (L.counter) *L.counter += 1;
+}
+
+// two-field form (xi = 1): kernels compiled without xi; three-field form (Eq. 3): with it
+template <int NS, bool PC, int EPI, int BX, int BY>
+void launch_blk(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
+                const uint16_t* ccode, double* dc) {
+    if (lv.xi != nullptr) launch_blk_x<NS, PC, EPI, BX, BY, 1>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else launch_blk_x<NS, PC, EPI, BX, BY, 0>(L, lv, xin, xout, b, ec, zero, ccode, dc);
 }
 
 template <int NS, bool PC, int EPI = 0>

@@ -35,6 +35,12 @@ __device__ __forceinline__ double ldv(const double* p) { return COH ? __ldca(p) 
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// XIM: how the tile code learns whether the level carries the paper's third field xi (Eq. 3):
+// 0 two-field form, 1 three-field form (both compile-time, so the two-field kernels carry no trace of xi),
+// 2 decided at run time from lv.xi (fused small-level kernel, latency bound).
+template <int XIM>
+__device__ __forceinline__ bool has_xi(const LevelDev& lv) { return XIM == 2 ? (lv.xi != nullptr) : (XIM == 1); }
+
 constexpr int GT = 512;     // threads per CTA
 constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
@@ -126,7 +132,7 @@ __device__ __forceinline__ int64_t parent_slot9(const int* pt, int cx, int cy) {
 // thread forms d = A x - b (difference form of rule D1) for its own inner cells of the tile and of the one-cell
 // ring around it, parks it in the (no longer needed) c array, and the 32 x 16 coarse points under the tile
 // gather their 3 x 3 full-weighting stencils; coarse guard rows get 0.  `breg` still holds b.
-template <class G, bool GENERAL>
+template <class G, bool GENERAL, int XIM>
 __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int* tn, const int* pt, const int* odd, const double* sx,
                                                   double* sc, const uint16_t* scode, double (&breg)[2][G::ROUNDS], double kappa,
                                                   const uint16_t* __restrict__ ccode, double* __restrict__ dc, int bx0, int by0) {
@@ -146,12 +152,17 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
                 const int own = col * NC + q, ob = (1 - col) * NC + q;
                 const bool inner = GENERAL ? ((scode[own] & 3) == C_INNER) : true;
                 if (inner && min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry)) >= H - 1) {
-                    const double lam = __ldg(lv.lam + region_slot<H>(tn, rx + bx0, ry + by0));
+                    const int64_t gs = region_slot<H>(tn, rx + bx0, ry + by0);
+                    const double lam = __ldg(lv.lam + gs);
+                    const bool hx = has_xi<XIM>(lv);
+                    const double xi = hx ? __ldg(lv.xi + gs) : 1.0;                  // breg holds b / xi (three-field form)
+                    // __dmul_rn: never contracted into the sums below, so the run-time and compile-time xi variants agree bit for bit
+                    const double kap = hx ? __dmul_rn(kappa, xi) : kappa, bl = hx ? __dmul_rn(breg[col][r], xi) : breg[col][r];
                     const double cl = sc[own], xl = sx[own];
-                    const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
-                    const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
+                    const double aW = kap * (cl + sc[ob + tpar - 1]), aE = kap * (cl + sc[ob + tpar]);
+                    const double aS = kap * (cl + sc[ob - RWC]), aN = kap * (cl + sc[ob + RWC]);
                     d = lam * xl + aW * (xl - sx[ob + tpar - 1]) + aE * (xl - sx[ob + tpar]) + aS * (xl - sx[ob - RWC]) +
-                        aN * (xl - sx[ob + RWC]) - breg[col][r];
+                        aN * (xl - sx[ob + RWC]) - bl;
                 }
             }
             breg[col][r] = d;
@@ -189,7 +200,7 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
 // Fused operator apply (rules D1-D3, the same rows as k_apply): every thread forms (A x) for its own cells of the tile
 // from the smoothed x in shared memory (lambda is the only extra load), parks it in the no longer needed c array,
 // and the tile is written out coalesced.  `breg` is reused as scratch.
-template <class G, bool GENERAL>
+template <class G, bool GENERAL, int XIM>
 __device__ __forceinline__ void apply_epilogue(const LevelDev& lv, int t, const int* tn, const double* sx, double* sc, const uint16_t* scode,
                                                double (&breg)[2][G::ROUNDS], double kappa, double* __restrict__ wout, int bx0, int by0) {
     constexpr int H = G::H, RW = G::RW, RH = G::RH, RWC = G::RWC, NC = G::NC, ROUNDS = G::ROUNDS, BX = G::BW, BY = G::BH;
@@ -207,10 +218,12 @@ __device__ __forceinline__ void apply_epilogue(const LevelDev& lv, int t, const 
                     const uint16_t code = GENERAL ? scode[own] : (uint16_t)C_INNER;
                     const int kind = code & 3;
                     if (kind == C_INNER) {
-                        const double lam = __ldg(lv.lam + region_slot<H>(tn, rx + bx0, ry + by0));
+                        const int64_t gs = region_slot<H>(tn, rx + bx0, ry + by0);
+                        const double lam = __ldg(lv.lam + gs);
+                        const double kap = has_xi<XIM>(lv) ? __dmul_rn(kappa, __ldg(lv.xi + gs)) : kappa;     // xi_{i,j} / (2 h^2), Eq. 10
                         const double cl = sc[own], xl = sx[own];
-                        const double aW = kappa * (cl + sc[ob + tpar - 1]), aE = kappa * (cl + sc[ob + tpar]);
-                        const double aS = kappa * (cl + sc[ob - RWC]), aN = kappa * (cl + sc[ob + RWC]);
+                        const double aW = kap * (cl + sc[ob + tpar - 1]), aE = kap * (cl + sc[ob + tpar]);
+                        const double aS = kap * (cl + sc[ob - RWC]), aN = kap * (cl + sc[ob + RWC]);
                         v = lam * xl + aW * (xl - sx[ob + tpar - 1]) + aE * (xl - sx[ob + tpar]) + aS * (xl - sx[ob - RWC]) +
                             aN * (xl - sx[ob + RWC]);
                     } else if (kind == C_DIR) v = sx[own];
@@ -256,7 +269,7 @@ __device__ __forceinline__ double prolong_e(const int* pt, int odd0, int odd1, i
 }
 
 // x_out = S^NS (x_in - [PC] P e_c);  zero: x_in is the zero vector and is not read.
-template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY>
+template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY, int XIM = 2>
 __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                            const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                            unsigned char* smem_raw, const int* meta = nullptr,
@@ -309,6 +322,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                 xv[r] = (!PC && xin_zero) ? 0.0 : ldv<COH>(xin + s);
                 cv[r] = __ldg(lv.c + s);
                 breg[col][r] = ldv<COH>(b + s);
+                if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));             // 1 on guards: their b is untouched
                 rd[col][r] = __ldg(lv.rd + s);
                 ev[r] = PC ? prolong_e<COH>(pt, odd[0], odd[1], rx - H + bx0, ry - H + by0, ec) : 0.0;
             }
@@ -434,7 +448,10 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
                     const int base = 1 + col + (PC ? 1 : 0);
                     const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
-                    if (nsw > 0) { breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s); }
+                    if (nsw > 0) {
+                        breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s);
+                        if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));
+                    }
                     if ((DR && marg >= H - 1) || (AP && marg >= H)) prefetch_l2(lv.lam + s);     // read by the restriction epilogue
                     act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
                 } else if (kind != C_ABSENT) {
@@ -513,12 +530,12 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
         const int ly = idx / BX, lx = idx - ly * BX;
         xout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sx[cidx<G>(lx + H, ly + H)];
     }
-    if (DR) restrict_epilogue<G, true>(lv, tn, pt, odd, sx, sc, scode, breg, kappa, ccode, dc, bx0, by0);
-    if (AP) apply_epilogue<G, true>(lv, t, tn, sx, sc, scode, breg, kappa, dc, bx0, by0);
+    if (DR) restrict_epilogue<G, true, XIM>(lv, tn, pt, odd, sx, sc, scode, breg, kappa, ccode, dc, bx0, by0);
+    if (AP) apply_epilogue<G, true, XIM>(lv, t, tn, sx, sc, scode, breg, kappa, dc, bx0, by0);
 }
 
 // Interior tile: all cells of the region are inner points.
-template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY>
+template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY, int XIM = 2>
 __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                         unsigned char* smem_raw, const int* meta = nullptr,
@@ -563,6 +580,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 xv[r] = xin_zero ? 0.0 : ldv<COH>(xin + s);
                 cv[r] = __ldg(lv.c + s);
                 breg[col][r] = ldv<COH>(b + s);
+                if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));
                 rd[col][r] = __ldg(lv.rd + s);
                 if (PC) xv[r] -= prolong_e<COH>(pt, odd[0], odd[1], rx - H + bx0, ry - H + by0, ec);   // x <- x - P e_c
             }
@@ -602,7 +620,10 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 const int marg = min(min(rx, RW - 1 - rx), min(ry, RH - 1 - ry));
                 const int base = 1 + col;
                 const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
-                if (nsw > 0) { breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s); }
+                if (nsw > 0) {
+                    breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s);
+                    if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));
+                }
                 if ((DR && marg >= H - 1) || (AP && marg >= H)) prefetch_l2(lv.lam + s);         // read by the restriction epilogue
                 act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
             }
@@ -655,11 +676,11 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
         const int ly = idx / BX, lx = idx - ly * BX;
         xout[(int64_t)t * TS + (by0 + ly) * TX + bx0 + lx] = sx[cidx<G>(lx + H, ly + H)];
     }
-    if (DR) restrict_epilogue<G, false>(lv, tn, pt, odd, sx, sc, nullptr, breg, kappa, ccode, dc, bx0, by0);
-    if (AP) apply_epilogue<G, false>(lv, t, tn, sx, sc, nullptr, breg, kappa, dc, bx0, by0);
+    if (DR) restrict_epilogue<G, false, XIM>(lv, tn, pt, odd, sx, sc, nullptr, breg, kappa, ccode, dc, bx0, by0);
+    if (AP) apply_epilogue<G, false, XIM>(lv, t, tn, sx, sc, nullptr, breg, kappa, dc, bx0, by0);
 }
 
-template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY>
+template <int NS, bool PC, bool COH, int EPI = 0, int BX = TX, int BY = TY, int XIM = 2>
 __device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double* __restrict__ xin, double* __restrict__ xout,
                                         const double* __restrict__ b, const double* __restrict__ ec, int xin_zero,
                                         unsigned char* smem_raw, const int* meta = nullptr,
@@ -667,8 +688,8 @@ __device__ __forceinline__ void gs_tile(const LevelDev& lv, int t, const double*
                                            int bx0 = 0, int by0 = 0) {
     const int flag = meta != nullptr ? meta[META_FLAG] : lv.tflag[t];
     constexpr int need = 1 << (NS - 1 + (EPI ? 1 : 0));         // interior halo 2 NS (+ 1 or 2, rounded up to the next flag)
-    if (flag & need) gs_fast<NS, PC, COH, EPI, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
-    else gs_general<NS, PC, COH, EPI, BX, BY>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
+    if (flag & need) gs_fast<NS, PC, COH, EPI, BX, BY, XIM>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
+    else gs_general<NS, PC, COH, EPI, BX, BY, XIM>(lv, t, xin, xout, b, ec, xin_zero, smem_raw, meta, ccode, dc, bx0, by0);
 }
 
 }  // namespace

@@ -69,8 +69,9 @@ __device__ __forceinline__ double inner_row(const LevelDev& lv, const Nb4 nb, in
     const int64_t sS = (ly > 0) ? s - TX : eS;
     const int64_t sN = (ly < TY - 1) ? s + TX : eN;
     const double cl = __ldg(lv.c + s);
-    const double aW = lv.kappa * (cl + __ldg(lv.c + sW)), aE = lv.kappa * (cl + __ldg(lv.c + sE));
-    const double aS = lv.kappa * (cl + __ldg(lv.c + sS)), aN = lv.kappa * (cl + __ldg(lv.c + sN));
+    const double kap = lv.xi ? lv.kappa * __ldg(lv.xi + s) : lv.kappa;     // xi_{i,j} / (2 h^2), Eq. 10
+    const double aW = kap * (cl + __ldg(lv.c + sW)), aE = kap * (cl + __ldg(lv.c + sE));
+    const double aS = kap * (cl + __ldg(lv.c + sS)), aN = kap * (cl + __ldg(lv.c + sN));
     const double xl = ldv<COH>(x + s);                                     // difference form (rule D1)
     return __ldg(lv.lam + s) * xl + aW * (xl - ldv<COH>(x + sW)) + aE * (xl - ldv<COH>(x + sE)) + aS * (xl - ldv<COH>(x + sS)) +
            aN * (xl - ldv<COH>(x + sN));

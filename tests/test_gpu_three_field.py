@@ -1,0 +1,177 @@
+"""GPU parity (-m gpu) of the paper's three-field form lambda phi - xi div(c grad phi) = rho (Eq. 3,
+PAPER.md:82 Eq. 10) through mg_update_coeffs3: every step and whole solves against the oracle (pinned by
+tests/test_oracle_three_field.py), same tolerances as tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_2509_11831_b200 import workloads as W
+from tests import helpers as H
+from tests.test_gpu_parity import TOL_SOLVE, TOL_STEP, dev, gpu, host, rel  # noqa: F401  (gpu is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def xi_field(pl, seed):
+    """Seeded xi > 0 in user order: a smooth factor in (x, y) times rough per-point noise, contrast about 30."""
+    rng = np.random.default_rng(seed)
+    x, y = pl.i * pl.h, pl.j * pl.h
+    return np.exp(0.8 * np.sin(3.0 * x + 1.0) * np.cos(2.0 * y - 0.5) + 0.4 * rng.standard_normal(pl.n))
+
+
+CASES = {
+    "cfg1_square65": lambda: W.make_plane(1),
+    "cfg2_annulus257_shuffled": lambda: W.make_plane(2, 257, order="shuffle"),
+    "cfg3_dshape257": lambda: W.make_plane(3, 257),
+    "cfg4_dshape513": lambda: W.make_plane(4, 513),
+    "random_blob_103": lambda: H.random_blob_plane(103),
+    "random_blob_106_193": lambda: H.random_blob_plane(106, 193),
+}
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def pair3(request, gpu, oracle_mod):
+    import torch
+    pl = CASES[request.param]()
+    xi = xi_field(pl, 17)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    o.update3(pl.lam, xi, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+    torch.cuda.synchronize()
+    yield pl, xi, o, s
+    s.close()
+
+
+def test_coefficients(pair3):
+    pl, xi, o, s = pair3
+    for lv in range(o.levels):
+        lo, co = o.level_coeffs(lv)
+        lg, cg = s.level_coeffs(lv)
+        assert rel(lg, lo) <= TOL_STEP and rel(cg, co) <= TOL_STEP
+        assert rel(s.level_xi(lv), o.level_xi(lv)) <= TOL_STEP                  # xi transferred by rule T4 too
+    assert np.array_equal(s.level_xi(0), o.level_xi(0))
+
+
+def test_apply_smooth_transfer_steps(pair3):
+    pl, xi, o, s = pair3
+    rng = np.random.default_rng(21)
+    for lv in range(o.levels):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        assert rel(host(s.apply(lv, dev(x))), o.apply(lv, x)) <= TOL_STEP
+        for sweeps in (1, 2, 3):
+            xo = o.smooth(lv, x, b, sweeps)
+            assert rel(host(s.smooth(lv, dev(x), dev(b), sweeps)), xo) <= TOL_STEP
+            if lv + 1 < o.levels:
+                do = o.restrict(lv, o.apply(lv, xo) - b)
+                xg, dg = s.smooth_restrict(lv, dev(x), dev(b), sweeps)
+                assert rel(host(xg), xo) <= TOL_STEP
+                scale = np.linalg.norm(o.restrict(lv, np.abs(o.apply(lv, xo)) + np.abs(b)))
+                assert np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
+
+
+def test_coarse_solve_and_vcycle(pair3):
+    pl, xi, o, s = pair3
+    rng = np.random.default_rng(22)
+    b = rng.standard_normal(o.level_n(o.levels - 1))
+    assert rel(host(s.coarse_solve(dev(b))), o.coarse_solve(b)) <= 1e-11
+    for lv in (0, max(0, o.levels - 2)):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        assert rel(host(s.vcycle(lv, dev(x), dev(b))), o.cycle(lv, x, b)) <= 1e-12
+
+
+def test_solve(pair3):
+    pl, xi, o, s = pair3
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    x, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert rc == 0 and ro["status"] == 0
+    assert abs(iters - ro["iters"]) <= 1
+    assert rel(host(x), ro["x"]) <= TOL_SOLVE
+    xc = H.canon(o, host(x)); fc = H.canon(o, pl.f)
+    true = np.linalg.norm(fc - o.apply(0, xc)) / np.linalg.norm(fc)              # residual of the three-field rows (Eq. 23)
+    assert true < 1.05e-10 and relres == pytest.approx(true, rel=1e-3)
+    s.update_coeffs3_host(pl.lam, xi, pl.c)
+    xh, it2, rr2, rc2 = s.solve_host(pl.f, pl.x0, 1e-10)
+    assert rc2 == 0 and it2 == iters and rel(xh, host(x)) <= 1e-12
+
+
+def test_switching_forms_on_one_handle(gpu, oracle_mod):
+    """two-field -> three-field -> two-field on the same handle (the iteration graph is re-captured): every solve equals
+    the one of a fresh handle bit for bit, and xi = 1 through mg_update_coeffs3 is the two-field result bit for bit."""
+    pl = W.make_plane(3, 257)
+    xi = xi_field(pl, 5)
+    f, x0 = dev(pl.f), dev(pl.x0)
+
+    def fresh(three):
+        s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+        if three:
+            s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+        else:
+            s.update_coeffs(dev(pl.lam), dev(pl.c))
+        x, it, _, rc = s.solve(f, x0, 1e-10)
+        s.close()
+        assert rc == 0
+        return host(x), it
+
+    x2, it2_ = fresh(False)
+    x3, it3_ = fresh(True)
+    assert not np.array_equal(x2, x3)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    for three in (False, True, False, True):
+        if three:
+            s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+        else:
+            s.update_coeffs(dev(pl.lam), dev(pl.c))
+        x, it, _, rc = s.solve(f, x0, 1e-10)
+        assert rc == 0 and it == (it3_ if three else it2_)
+        assert np.array_equal(host(x), x3 if three else x2)
+        assert (s.level_xi(0) != 1.0).any() == three
+    s.update_coeffs3(dev(pl.lam), dev(np.ones(pl.n)), dev(pl.c))
+    x, it, _, rc = s.solve(f, x0, 1e-10)
+    assert rc == 0 and it == it2_ and np.array_equal(host(x), x2)
+    s.update_coeffs3(dev(pl.lam), None, dev(pl.c))
+    x, it, _, rc = s.solve(f, x0, 1e-10)
+    assert rc == 0 and it == it2_ and np.array_equal(host(x), x2)
+    s.close()
+
+
+@pytest.mark.parametrize("nu", [(2, 2), (3, 1)])
+def test_fused_small_levels_bit_identical(gpu, nu):
+    pl = W.make_plane(2, 513)
+    xi = xi_field(pl, 9)
+    out = []
+    for fused in (True, False):
+        s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=nu[0], nu_post=nu[1], fused_tail=fused)
+        s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+        rng = np.random.default_rng(11)
+        res = []
+        for lv in range(s.levels):
+            n = s.level_n(lv)
+            x, b = rng.standard_normal(n), rng.standard_normal(n)
+            res.append(host(s.vcycle(lv, dev(x), dev(b))))
+        xs, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+        res.append(host(xs)); res.append(np.array([iters, rc]))
+        out.append(res)
+        s.close()
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
+
+
+def test_manufactured_solution_on_the_gpu(gpu):
+    """The oracle's MMS pin (test_P11_manufactured_solution_order) repeated on the CUDA path at 257^2 and 513^2:
+    u = sin(pi x) sin(pi y), lambda = c = 1, xi = 1 + x + y/2: error ratio 4 (O(h^2))."""
+    errs = []
+    for n in (257, 513):
+        pl = W.make_plane(1, n)
+        xi = 1.0 + pl.x + 0.5 * pl.y
+        u = np.sin(np.pi * pl.x) * np.sin(np.pi * pl.y)
+        u[pl.kind != 0] = 0.0
+        f = np.where(pl.kind == 0, (1.0 + 2.0 * np.pi ** 2 * xi) * u, 0.0)
+        s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+        s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+        x, it, rr, rc = s.solve(dev(f), dev(np.zeros(pl.n)), 1e-11)
+        s.close()
+        assert rc == 0
+        errs.append(np.linalg.norm(host(x) - u) / np.linalg.norm(u))
+    assert errs[0] / errs[1] == pytest.approx(4.0, abs=0.1)
