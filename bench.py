@@ -92,12 +92,15 @@ class ClockSampler:
         return out
 
 
-def oracle_sample(pl, max_iters):
+def oracle_sample(pl, max_iters, xi=None):
     """The oracle as it stands, 1 thread, on the same plane, capped at max_iters iterations."""
     from oracle import oracle as om
     o = om.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, max_iters=max_iters)
     t0 = time.perf_counter()
-    o.update(pl.lam, pl.c)
+    if xi is None:
+        o.update(pl.lam, pl.c)
+    else:
+        o.update3(pl.lam, xi, pl.c)
     r = o.solve(pl.f, pl.x0, RTOL)
     dt = time.perf_counter() - t0
     return dt, r["iters"], o
@@ -189,6 +192,9 @@ def run_ours(args):
     s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, full_cgs2=args.full_cgs2)
     d_in = [(dev(q.lam), dev(q.c), dev(q.f)) for q in uniq]          # resident in HBM before the timed region
     h_in = [(pin(q.lam).numpy(), pin(q.c).numpy(), pin(q.f).numpy()) for q in uniq]
+    # --three-field: the paper's lambda phi - xi div(c grad phi) = rho (Eq. 3) with a seeded xi, the same every step
+    xi = W.xi_field(pl) if args.three_field else None
+    d_xi, h_xi = (dev(xi), pin(xi).numpy()) if args.three_field else (None, None)
     d_x0, d_x = dev(pl.x0), torch.empty(pl.n, dtype=torch.float64, device="cuda")
     h_x0, h_x = pin(pl.x0).numpy(), torch.empty(pl.n, dtype=torch.float64).pin_memory().numpy()
 
@@ -200,13 +206,16 @@ def run_ours(args):
 
     def step_device(k):
         lam, c, f = d_in[k if warm else 0]
-        s.update_coeffs(lam, c)
+        s.update_coeffs3(lam, d_xi, c)
         _, iters, relres, rc = s.solve(f, d_x if (warm and k > 0) else d_x0, args.rtol, x=d_x)   # d_x may alias d_x0
         return iters, relres, rc
 
     def step_host(k):
         lam, c, f = h_in[k if warm else 0]
-        s.update_coeffs_host(lam, c)
+        if h_xi is None:
+            s.update_coeffs_host(lam, c)
+        else:
+            s.update_coeffs3_host(lam, h_xi, c)
         _, iters, relres, rc = s.solve_host(f, h_x if (warm and k > 0) else h_x0, args.rtol, x=h_x)
         return iters, relres, rc
 
@@ -224,7 +233,7 @@ def run_ours(args):
         return ev0.elapsed_time(ev1), outs, s.kernel_launches - l0, solve_ms, update_ms
 
     if args.roofline_only:                 # profiling aid: only the roofline kernel (after one update), nothing timed
-        s.update_coeffs(*d_in[0][:2])
+        s.update_coeffs3(d_in[0][0], d_xi, d_in[0][1])
         n0 = s.level_n(0)
         xs, bs = torch.randn(n0, dtype=torch.float64, device="cuda"), torch.randn(n0, dtype=torch.float64, device="cuda")
         for _ in range(4):
@@ -260,7 +269,7 @@ def run_ours(args):
         per_launch_ms = float(np.median(t[2:]))
         alg = ROOF_BYTES_PER_POINT * n0
         achieved = alg / (per_launch_ms * 1e-3) / 1e9
-        traffic = ROOF_TRAFFIC_PER_LAUNCH.get(args.config) if args.lattice is None else None
+        traffic = ROOF_TRAFFIC_PER_LAUNCH.get(args.config) if (args.lattice is None and not args.three_field) else None
         roof = {"bound": "hbm", "kernel": "k_gs<2,false,true> level 0: two fused RB-B Gauss-Seidel sweeps + defect + FW restriction per launch",
                 "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "algorithmic_bytes_per_launch": alg, "ms_per_launch": per_launch_ms,
@@ -271,7 +280,7 @@ def run_ours(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        dt, it_o, _ = oracle_sample(pl, args.ref_iters)
+        dt, it_o, _ = oracle_sample(pl, args.ref_iters, xi)
         cpu = {"value": pl.n * it_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"update + first {it_o} fGMRES iterations of the same plane, 1 thread, {dt:.1f} s"}
 
@@ -282,14 +291,15 @@ def run_ours(args):
                 "config": {"workload": WORKLOADS[args.config] + (f" [geometry on a {args.lattice}^2 lattice]" if args.lattice else ""),
                            "unknowns_per_plane": pl.n, "planes": world, "rtol": args.rtol,
                            "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels,
-                           "step": "mg_update_coeffs + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
+                           "form": "three-field (lambda, xi, c), PAPER.md Eq. 3" if args.three_field else "two-field (lambda, c), xi = 1",
+                           "step": ("mg_update_coeffs3" if args.three_field else "mg_update_coeffs") + " + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
                            "l2_policy": "inputs larger than L2 (no flush)" if pl.n * 8 * 8 > 126e6 else "working set fits L2 (small config)"},
                 "iters": iters_all[-1], "iters_per_step": iters_all, "final_relres": outs[-1][1], "status": outs[-1][2],
                 "second_gs_updates": reorth,      # Arnoldi steps of the last solve whose second update ran (G23)
                 "solve_ms": float(np.median(solve_ms)), "update_ms": float(np.median(update_ms)),
                 "solve_ms_per_plane": float(np.median(solve_ms)),
                 "clocks": clocks, "gpu_launches": launches,
-                "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": 4 * pl.n * 8, "d2h_bytes_per_step": pl.n * 8,
+                "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": (5 if args.three_field else 4) * pl.n * 8, "d2h_bytes_per_step": pl.n * 8,
                         "ms_per_step": ms_e2e / args.steps, "iters": outs_e[-1][0]},
                 "roofline": roof, "cpu_baseline": cpu}
         print(json.dumps(line))
@@ -439,6 +449,7 @@ def main():
     ap.add_argument("--lattice", type=int, default=None, help="same geometry on an n x n lattice (2^k + 1; O(N) scaling runs)")
     ap.add_argument("--paper-mms", type=int, default=0, metavar="R",
                     help="run the paper's annulus MMS scaling experiment over R refinements (6 reaches its 24 M points) instead")
+    ap.add_argument("--three-field", action="store_true", help="secondary line: the paper's three-field form with a seeded xi (mg_update_coeffs3)")
     ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved concurrently (secondary line, SURVEY.md 8(f) NEXT-1)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -11,11 +11,7 @@ from tests.test_gpu_parity import TOL_SOLVE, TOL_STEP, dev, gpu, host, rel  # no
 pytestmark = pytest.mark.gpu
 
 
-def xi_field(pl, seed):
-    """Seeded xi > 0 in user order: a smooth factor in (x, y) times rough per-point noise, contrast about 30."""
-    rng = np.random.default_rng(seed)
-    x, y = pl.i * pl.h, pl.j * pl.h
-    return np.exp(0.8 * np.sin(3.0 * x + 1.0) * np.cos(2.0 * y - 0.5) + 0.4 * rng.standard_normal(pl.n))
+xi_field = W.xi_field
 
 
 CASES = {
@@ -159,7 +155,7 @@ def test_fused_small_levels_bit_identical(gpu, nu):
 
 
 def test_manufactured_solution_on_the_gpu(gpu):
-    """The oracle's MMS pin (test_P11_manufactured_solution_order) repeated on the CUDA path at 257^2 and 513^2:
+    """The oracle's MMS pin (test_P12_manufactured_solution_order) repeated on the CUDA path at 257^2 and 513^2:
     u = sin(pi x) sin(pi y), lambda = c = 1, xi = 1 + x + y/2: error ratio 4 (O(h^2))."""
     errs = []
     for n in (257, 513):

@@ -1,4 +1,4 @@
-"""Pins P11 for the oracle's three-field form lambda*phi - xi*div(c grad phi) = rho (Eq. 3,
+"""Pins P12 for the oracle's three-field form lambda*phi - xi*div(c grad phi) = rho (Eq. 3,
 PAPER.md:82 Eq. 10: the bracket of row (i,j) carries xi_{i,j}/2).  Checked against closed forms, the
 absorption property the paper states, a dense direct solve and a manufactured solution;
 never against the oracle's own formulae."""
@@ -19,7 +19,7 @@ def _xi_field(pl, seed=2):
     return np.exp(0.6 * rng.standard_normal(pl.n))
 
 
-def test_P11_eigenpairs_constant_xi(oracle_mod):
+def test_P12_eigenpairs_constant_xi(oracle_mod):
     """Square, c = 1, constant lambda and xi, zero guards: sin sin is an eigenvector with eigenvalue
     lam + xi (4/h^2)(sin^2(k pi h/2) + sin^2(l pi h/2)): xi scales the difference part and not lambda."""
     n, lam0, xi0 = 33, 0.7, 2.5
@@ -39,7 +39,7 @@ def test_P11_eigenpairs_constant_xi(oracle_mod):
 
 
 @pytest.mark.parametrize("geom", ["annulus", "dshape"])
-def test_P11_row_scaling_structure(oracle_mod, geom):
+def test_P12_row_scaling_structure(oracle_mod, geom):
     """Eq. 10: A3 = Lambda + diag(xi) (A2 - Lambda) on inner rows, with the xi of the ROW's point (so A3 is not
     symmetric for variable xi); Dirichlet and Neumann rows (Eq. 11, 16) do not see xi.  Every level."""
     pl = H.small_annulus(33, 3) if geom == "annulus" else H.small_dshape(33, 3)
@@ -63,7 +63,7 @@ def test_P11_row_scaling_structure(oracle_mod, geom):
             assert np.abs(A3 - A3.T).max() > 1e-3 * scale       # row scaling, not a symmetric scaling
 
 
-def test_P11_xi_is_grid_transferred_like_lambda(oracle_mod):
+def test_P12_xi_is_grid_transferred_like_lambda(oracle_mod):
     """P:153 / P:207: lambda, xi and c are all transferred to the coarser levels by the same rule (T4)."""
     pl = H.small_dshape(65, 4)
     xi = _xi_field(pl)
@@ -78,7 +78,7 @@ def test_P11_xi_is_grid_transferred_like_lambda(oracle_mod):
 
 
 @pytest.mark.parametrize("geom", ["annulus", "dshape"])
-def test_P11_absorption_and_dense_solve(oracle_mod, geom):
+def test_P12_absorption_and_dense_solve(oracle_mod, geom):
     """xi "can be absorbed into lambda and rho".  The multi-level three-field solve must equal the dense
     direct solve of the TWO-field operator with lambda/xi and rho/xi on the inner rows (guard rows unchanged)."""
     pl = H.small_annulus(33, 3) if geom == "annulus" else H.small_dshape(33, 3)
@@ -102,7 +102,7 @@ def test_P11_absorption_and_dense_solve(oracle_mod, geom):
     assert r["relres"] == pytest.approx(true, rel=1e-3) and true < 1e-8
 
 
-def test_P11_manufactured_solution_order(oracle_mod):
+def test_P12_manufactured_solution_order(oracle_mod):
     """u = sin(pi x) sin(pi y), lambda = c = 1, xi = 1 + x + y/2 on the unit square:
     rho = (1 + 2 pi^2 xi) u.  Error vs the continuous solution falls by 4 per halving (O(h^2))."""
     errs, its = [], []
@@ -122,7 +122,7 @@ def test_P11_manufactured_solution_order(oracle_mod):
     assert max(its) <= min(its) + 2                              # h-independent iteration count
 
 
-def test_P11_smoother_solves_its_rows(oracle_mod):
+def test_P12_smoother_solves_its_rows(oracle_mod):
     """Gauss-Seidel with xi: after the loop over a group the residual of the three-field rows of that group is zero."""
     pl = H.small_dshape(65, 2)
     o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
@@ -138,7 +138,7 @@ def test_P11_smoother_solves_its_rows(oracle_mod):
             assert np.abs(r[rows]).max() <= 1e-13 * (np.abs(b).max() + np.abs(o.apply(s, np.abs(x))).max())
 
 
-def test_P11_unit_xi_is_the_two_field_form_bit_for_bit(oracle_mod):
+def test_P12_unit_xi_is_the_two_field_form_bit_for_bit(oracle_mod):
     pl = H.small_annulus(65, 3)
     o2 = H.make_oracle(oracle_mod, pl)
     o3 = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
