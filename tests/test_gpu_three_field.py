@@ -171,3 +171,34 @@ def test_manufactured_solution_on_the_gpu(gpu):
         assert rc == 0
         errs.append(np.linalg.norm(host(x) - u) / np.linalg.norm(u))
     assert errs[0] / errs[1] == pytest.approx(4.0, abs=0.1)
+
+
+@pytest.mark.parametrize("seed", list(range(300, 312)))
+def test_random_mesh_and_options(gpu, oracle_mod, seed):
+    """The seeded sweep of tests/test_gpu_parity.py (ragged random domains x V(nu1,nu2) x V/W/F x restart length x
+    cooperative small-level kernel x full / selective second Gram-Schmidt update) in the three-field form; odd seeds
+    also alternate forms on the handle before the compared solve."""
+    rng = np.random.default_rng(seed)
+    n = int(rng.choice([65, 97, 129, 161, 257]))
+    nu1, nu2 = max(1, int(rng.integers(0, 4))), int(rng.integers(0, 4))
+    gamma, m = int(rng.choice([1, 1, 2, 3])), int(rng.choice([3, 10, 30, 40]))
+    tail, full = bool(rng.integers(0, 2)), bool(rng.integers(0, 2))
+    pl = H.random_blob_plane(seed, n)
+    xi = xi_field(pl, seed)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=nu1, nu_post=nu2, m=m, gamma=gamma, max_iters=120)
+    o.update3(pl.lam, xi, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=nu1, nu_post=nu2, restart_m=m, gamma=gamma, max_iters=120,
+                   fused_tail=tail, full_cgs2=full)
+    if seed % 2:
+        s.update_coeffs(dev(pl.lam), dev(pl.c))
+        s.solve(dev(pl.f), dev(pl.x0), 1e-6)
+    s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+    n0 = o.level_n(0)
+    x, b = rng.standard_normal(n0), rng.standard_normal(n0)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    xg, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    s.close()
+    assert rc == ro["status"] and abs(iters - ro["iters"]) <= 1
+    if rc == 0:
+        assert rel(host(xg), ro["x"]) <= TOL_SOLVE
