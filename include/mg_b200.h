@@ -43,7 +43,8 @@ enum {
     MG_EINVAL = -1,       /* null pointer, n <= 0, h <= 0, bad option, bad level                         */
     MG_EMESH = -2,        /* duplicate (i,j); inner point lacking a neighbour; guard without an inner
                              4-neighbour (rule M2); coarsest level too large for the dense solve */
-    MG_ECOEFF = -3,       /* reserved (coefficient check)                                   */
+    MG_ECOEFF = -3,       /* mg_solve: the last update's fields were not admissible: c <= 0,
+                             xi <= 0, or a non-finite value (tested on the device during the update)      */
     MG_ENOTREADY = -4,    /* solve / cycle before the first mg_update_coeffs                             */
     MG_ECUDA = -5,        /* CUDA runtime error or no device                                             */
     MG_ENOMEM = -6
@@ -97,7 +98,8 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
 
 /* update: new coefficients lambda, c (= BASELINE "xi") on ALL n points, DEVICE
  * pointers, user order.  Restricts them to all coarser levels (rule T4) and factorises the coarsest
- * operator (rule C) on the device.  Asynchronous on `stream`. */
+ * operator (rule C) on the device.  Asynchronous on `stream`.  Admissibility (c > 0; finite lambda) is
+ * tested on the device during the call; a violation is reported by the next mg_solve as MG_ECOEFF. */
 int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream);
 
 /* update for the paper's three-field form  lambda phi - xi div(c grad phi) = rho  (Eq. 3; the row of

@@ -60,7 +60,9 @@ struct mg_handle_s {
     double *V = nullptr, *Z = nullptr, *w = nullptr, *r = nullptr, *xs = nullptr, *bs = nullptr;
     GmresState* st = nullptr;
     double* partial = nullptr;
-    int* h_hdr = nullptr;                 // pinned copy of the first 8 ints of the state
+    int* h_hdr = nullptr;                 // pinned copy of the first 8 ints of the state (two slots) + [16] the coefficient flag
+    int* coeff_bad = nullptr;             // device flag of the last update: bit 0 lambda not finite, bit 1 c, bit 2 xi not finite or <= 0
+    bool coeffs_unchecked = false;        // the flag of the last update has not been read yet (first solve / cycle after it)
     GmresState* h_state = nullptr;        // pinned full copy (read at the end of a solve)
     // coarsest level
     int nL = 0;
@@ -317,7 +319,9 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     CUF(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     for (auto& e : h->ev) CUF(cudaEventCreate(&e));
     for (auto& e : h->hev) CUF(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    CUF(cudaMallocHost((void**)&h->h_hdr, 64));
+    CUF(cudaMallocHost((void**)&h->h_hdr, 128));
+    h->h_hdr[16] = 0;
+    TRY(dev_alloc(h, (void**)&h->coeff_bad, sizeof(int), s));
     CUF(cudaMallocHost((void**)&h->h_state, sizeof(GmresState)));
     h->lev.resize(h->L); h->buf.resize(h->L);
     for (int l = 0; l < h->L; l++) {
@@ -418,9 +422,13 @@ int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, c
     if (rc) return rc;
     Launch L = LZ(h, s);
     CU(cudaEventRecord(h->ev[2], s));
-    launch_gather(L, d_lambda, h->user2slot, h->buf[0].lam, h->n);
-    launch_gather(L, d_c, h->user2slot, h->buf[0].c, h->n);
-    if (d_xi) launch_gather(L, d_xi, h->user2slot, h->buf[0].xi, h->n);
+    // admissibility (c > 0; lambda only finite since Eq. 21 P:241 has both signs; xi > 0, G25) is tested on the device while
+    // the fields are gathered; the first mg_solve after the update reads the flag and returns MG_ECOEFF
+    CU(cudaMemsetAsync(h->coeff_bad, 0, sizeof(int), s));
+    launch_gather_check(L, d_lambda, h->user2slot, h->buf[0].lam, h->n, 1, 1, h->coeff_bad);
+    launch_gather_check(L, d_c, h->user2slot, h->buf[0].c, h->n, 2, 2, h->coeff_bad);
+    if (d_xi) launch_gather_check(L, d_xi, h->user2slot, h->buf[0].xi, h->n, 2, 4, h->coeff_bad);
+    h->coeffs_unchecked = true;
     for (int l = 0; l + 1 < h->L; l++) launch_restrict_coeff(L, h->lev[l], h->lev[l + 1]);     // rule T4
     for (int l = 0; l < h->L; l++) launch_diag(L, h->lev[l]);                                   // U2: 1 / a_ll for the smoother
     launch_coarse_factor(L, h->lev[h->L - 1], h->cslot, h->slot2row, h->nL, h->cwork, h->Ainv);   // rule C
@@ -455,7 +463,15 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
         launch_norm2(L, h->r, ns, h->st, h->partial, 1);
         launch_start_cycle(L, h->st, h->r, h->V, ns);
         CU(cudaMemcpyAsync(h->h_hdr, h->st, 32, cudaMemcpyDeviceToHost, s));
+        if (h->coeffs_unchecked) CU(cudaMemcpyAsync(h->h_hdr + 16, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
+        h->coeffs_unchecked = false;
+        if (h->h_hdr[16]) {                                           // the last update's fields were not admissible
+            const int b = h->h_hdr[16];
+            g_last_error = std::string("inadmissible coefficients in the last update:") + ((b & 1) ? " lambda not finite;" : "") +
+                           ((b & 2) ? " c not finite or <= 0 (PAPER.md:51);" : "") + ((b & 4) ? " xi not finite or <= 0;" : "");
+            return MG_ECOEFF;
+        }
         status = h->h_hdr[2];
         if (h->h_hdr[3]) break;                                       // cycle_end set by start: finished
         // One graph launch per Arnoldi step.  The host stays one step ahead: step `it` is enqueued before

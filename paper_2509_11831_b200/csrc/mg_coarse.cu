@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict_
             double b = redv[0]; int i = redi[0];
             for (int w = 1; w < CT / 32; w++)
                 if (redv[w] > b || (redv[w] == b && redi[w] < i)) { b = redv[w]; i = redi[w]; }
-            piv = i;
+            piv = i < n ? i : k;        // a column of NaNs (inadmissible coefficients, MG_ECOEFF) has no maximum: stay in bounds
         }
         __syncthreads();
         const int p = piv;
@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(CIT) k_coarse_invert_coop(int n, int cpb, cons
             double b = redv[0]; int i = redi[0];
             for (int w = 1; w < CIT / 32; w++)
                 if (redv[w] > b || (redv[w] == b && redi[w] < i)) { b = redv[w]; i = redi[w]; }
-            pivbuf[k & 1] = i;
+            pivbuf[k & 1] = i < n ? i : k;   // as above
         }
         for (int r = tid; r < n; r += CIT) colbuf[(size_t)(k & 1) * n + r] = col[r];
         __syncthreads();

@@ -102,6 +102,7 @@ void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev
 void launch_diag(const Launch& L, const LevelDev& lv);   // U2: rd = 1 / a_ll from lambda, c
 void launch_zero(const Launch& L, VecRef x, int64_t n);
 void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n);   // dst[slot[k]] = src[k]
+void launch_gather_check(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n, int mode, int bit, int* bad);
 void launch_scatter(const Launch& L, const double* src_tiled, const int32_t* slot, double* dst, int64_t n);  // dst[k] = src[slot[k]]
 
 // ---- fused small levels (mg_tail.cu): the cycle steps of all levels >= s0 as a program run by one

@@ -228,6 +228,18 @@ __global__ void k_zero(VecRef xr, int64_t n) {
 __global__ void k_gather(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n) {
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[slot[k]] = src[k];
 }
+// gather of a coefficient field with the admissibility test of PAPER.md:51: mode 1: finite; mode 2: finite and > 0.
+// A violation sets *bad (bit 0 lambda, bit 1 c, bit 2 xi, given by `bit`); the values are copied regardless.
+__global__ void k_gather_check(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n,
+                               int mode, int bit, int* __restrict__ bad) {
+    bool any = false;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
+        const double v = src[k];
+        dst[slot[k]] = v;
+        any |= !isfinite(v) || (mode == 2 && !(v > 0.0));
+    }
+    if (any) atomicOr(bad, bit);
+}
 __global__ void k_scatter(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n) {
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[k] = src[slot[k]];
 }
@@ -283,6 +295,10 @@ void launch_zero(const Launch& L, VecRef x, int64_t n) {
 }
 void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n) {
     k_gather<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n);
+    count(L);
+}
+void launch_gather_check(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n, int mode, int bit, int* bad) {
+    k_gather_check<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n, mode, bit, bad);
     count(L);
 }
 void launch_scatter(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n) {

@@ -202,3 +202,35 @@ def test_random_mesh_and_options(gpu, oracle_mod, seed):
     assert rc == ro["status"] and abs(iters - ro["iters"]) <= 1
     if rc == 0:
         assert rel(host(xg), ro["x"]) <= TOL_SOLVE
+
+
+def test_inadmissible_coefficients(gpu, oracle_mod):
+    """c <= 0, xi <= 0 or a non-finite value in an update: the oracle refuses the update; the CUDA path tests
+    the fields on the device while gathering them and the next mg_solve returns MG_ECOEFF (-3) until a valid update."""
+    pl = W.make_plane(2, 129)
+    xi = xi_field(pl, 3)
+    f, x0 = dev(pl.f), dev(pl.x0)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    k = pl.n // 3
+    bad = []
+    c = pl.c.copy(); c[k] = 0.0; bad.append((pl.lam, None, c, "c not finite or <= 0"))
+    c = pl.c.copy(); c[k] = np.nan; bad.append((pl.lam, xi, c, "c not finite or <= 0"))
+    lam = pl.lam.copy(); lam[k] = np.inf; bad.append((lam, None, pl.c, "lambda not finite"))
+    x = xi.copy(); x[k] = -1.0; bad.append((pl.lam, x, pl.c, "xi not finite or <= 0"))
+    for lam, x, c, msg in bad:
+        with pytest.raises(ValueError):
+            o.update3(lam, x if x is not None else np.ones(pl.n), c)
+        s.update_coeffs3(dev(lam), dev(x) if x is not None else None, dev(c))
+        for _ in range(2):                                          # sticky until the next update
+            with pytest.raises(gpu.MgError) as e:
+                s.solve(f, x0, 1e-10)
+            assert e.value.code == -3 and msg in str(e.value)
+        s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))           # a valid update clears it
+        xs, it, rr, rc = s.solve(f, x0, 1e-10)
+        assert rc == 0 and rr < 1e-10
+    # negative lambda is admissible (Eq. 21, PAPER.md:241)
+    s.update_coeffs(dev(pl.lam - 0.3), dev(pl.c))
+    xs, it, rr, rc = s.solve(f, x0, 1e-10)
+    assert rc >= 0
+    s.close()
