@@ -107,7 +107,7 @@ int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, voi
  * (guard rows, Eq. 11 / 16, do not see it); it is transferred to the coarser levels like lambda and c
  * (PAPER.md:153, 207).  d_xi == NULL is mg_update_coeffs (xi = 1).  The handle keeps the form of the
  * last update; switching forms re-captures the iteration graph at the next solve.  The stop test of mg_solve is
- * on the residual of the three-field rows.  Costs 8 B per point and smoothing launch more than the two-field form. */
+ * on the residual of the three-field rows.  Costs 8 B per point and smoothing launch (and one fp64 division per point) more than the two-field form. */
 int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, const double* d_c, void* stream);
 
 /* solve: fGMRES(m) with one V-cycle as right preconditioner (rules K1-K5), stopping

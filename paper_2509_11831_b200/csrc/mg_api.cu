@@ -34,7 +34,7 @@ struct LevelBuf {           // device arrays owned per level
     uint16_t* code = nullptr;
     uint8_t* tflag = nullptr;
     int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
-    double *xi = nullptr, *rxi = nullptr;   // three-field form only: allocated by the first mg_update_coeffs3 with xi
+    double* xi = nullptr;   // three-field form only: allocated by the first mg_update_coeffs3 with xi
     double *lam = nullptr, *c = nullptr, *rd = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
     double* tb = nullptr;   // right-hand side of the single-step entry points.  The cycle's own b of a coarse level is written ONLY by
                             // the restriction kernels: slots of coarse points under no fine tile are never written and must stay 0.
@@ -71,7 +71,7 @@ struct mg_handle_s {
     // host-buffer staging
     double* stage[3] = {nullptr, nullptr, nullptr};
     double* stage_xi = nullptr;
-    bool three_field = false;             // the level structs carry xi / rxi (Eq. 3)
+    bool three_field = false;             // the level structs carry xi (Eq. 3)
     bool have_coeffs = false;
     bool no_fused_dr = false;             // debugging: separate defect + restriction kernel
     cudaError_t tail_err = cudaSuccess;
@@ -352,7 +352,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         d.nslots = hl.nslots();
         d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
         d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c; d.rd = b.rd; d.tflag = b.tflag;
-        d.xi = nullptr; d.rxi = nullptr;
+        d.xi = nullptr;
     }
     TRY(dev_alloc(h, (void**)&h->d_lev, sizeof(LevelDev) * h->L, s));
     CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
@@ -391,7 +391,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
 // ============================================================================ update / solve
 extern "C" {
 
-// Switch the level structs between the two-field (xi, rxi null) and the three-field form.  The structs are kernel
+// Switch the level structs between the two-field (xi null) and the three-field form.  The structs are kernel
 // arguments baked into the captured iteration graph and copied to the device for the fused small-level kernel, so
 // both are refreshed.
 static int set_three_field(mg_handle h, bool on, cudaStream_t s) {
@@ -401,10 +401,8 @@ static int set_three_field(mg_handle h, bool on, cudaStream_t s) {
         if (on && !b.xi) {
             const size_t vb = (size_t)h->hh.lev[l].nslots() * sizeof(double);
             int rc = dev_alloc(h, (void**)&b.xi, vb, s); if (rc) return rc;
-            rc = dev_alloc(h, (void**)&b.rxi, vb, s); if (rc) return rc;
         }
         h->lev[l].xi = on ? b.xi : nullptr;
-        h->lev[l].rxi = on ? b.rxi : nullptr;
     }
     CU(cudaStreamSynchronize(s));         // h->lev is pageable host memory: the copy below must not overlap a later change
     CU(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));

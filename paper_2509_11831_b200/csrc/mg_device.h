@@ -29,10 +29,9 @@ struct LevelDev {
     double* c;
     double* rd;              // 1 / a_ll on inner points (rule D1), 0 elsewhere; derived at every update (U2)
     // Three-field form lambda phi - xi div(c grad phi) = rho (Eq. 3; Eq. 10 PAPER.md:82 carries xi_{i,j}/2
-    // of the row's own point).  Both null in the two-field form (xi = 1).  With xi the smoother works on
-    // the row divided by xi: it reads b * rxi and rd holds xi / a_ll, so its sweeps are unchanged.
+    // of the row's own point).  Null in the two-field form (xi = 1).  With xi the smoother works on
+    // the row divided by xi: it holds b / xi in registers and rd holds xi / a_ll, so its sweeps are unchanged.
     double* xi;              // xi on every present point (grid-transferred like lambda and c)
-    double* rxi;             // 1 / xi on inner points, 1 elsewhere; derived at every update
 };
 
 // A vector that may be one column of a Krylov basis selected on the device:

@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(NT) k_diag(LevelDev lv) {
     for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
         const int ly = threadIdx.x / TX + p * ROWS_PER_PASS;
         const int64_t s = (int64_t)t * TS + ly * TX + lx;
-        double r = 0.0, rx = 1.0;
+        double r = 0.0;
         if ((lv.code[s] & 3) == C_INNER) {
             const double cl = lv.c[s];
             const double xi = lv.xi ? lv.xi[s] : 1.0;
@@ -153,10 +153,8 @@ __global__ void __launch_bounds__(NT) k_diag(LevelDev lv) {
             const double aW = kap * (cl + lv.c[nslot(tn, lx - 1, ly)]), aE = kap * (cl + lv.c[nslot(tn, lx + 1, ly)]);
             const double aS = kap * (cl + lv.c[nslot(tn, lx, ly - 1)]), aN = kap * (cl + lv.c[nslot(tn, lx, ly + 1)]);
             r = xi / (lv.lam[s] + aW + aE + aS + aN);                            // the smoother's row is divided by xi
-            rx = 1.0 / xi;
         }
         lv.rd[s] = r;
-        if (lv.rxi) lv.rxi[s] = rx;
     }
 }
 

@@ -312,7 +312,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
     #pragma unroll
         for (int col = 0; col < 2; col++) {
             uint16_t codes[ROUNDS];
-            double xv[ROUNDS], cv[ROUNDS], ev[ROUNDS];
+            double xv[ROUNDS], cv[ROUNDS], ev[ROUNDS], xiv[ROUNDS];
     #pragma unroll
             for (int r = 0; r < ROUNDS; r++) {
                 const int q = min(tid + r * GT, NC - 1);
@@ -322,7 +322,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                 xv[r] = (!PC && xin_zero) ? 0.0 : ldv<COH>(xin + s);
                 cv[r] = __ldg(lv.c + s);
                 breg[col][r] = ldv<COH>(b + s);
-                if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));             // 1 on guards: their b is untouched
+                xiv[r] = has_xi<XIM>(lv) ? __ldg(lv.xi + s) : 1.0;
                 rd[col][r] = __ldg(lv.rd + s);
                 ev[r] = PC ? prolong_e<COH>(pt, odd[0], odd[1], rx - H + bx0, ry - H + by0, ec) : 0.0;
             }
@@ -342,6 +342,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     const int base = 1 + col + (PC ? 1 : 0);
                     const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
                     act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
+                    if (has_xi<XIM>(lv)) breg[col][r] = __ddiv_rn(breg[col][r], xiv[r]);    // the smoother's row is divided by xi
                 } else if (kind != C_ABSENT) {
                     const int pos = atomicAdd(&gcount, 1);
                     if (pos < GCAP) { glist[pos] = (uint16_t)(ry * RW + rx); gb[pos] = breg[col][r]; }
@@ -450,7 +451,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     const int nsw = marg >= base ? min(NS, (marg - base) / 3 + 1) : 0;
                     if (nsw > 0) {
                         breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s);
-                        if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));
+                        if (has_xi<XIM>(lv)) breg[col][r] = __ddiv_rn(breg[col][r], __ldg(lv.xi + s));
                     }
                     if ((DR && marg >= H - 1) || (AP && marg >= H)) prefetch_l2(lv.lam + s);     // read by the restriction epilogue
                     act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
@@ -580,7 +581,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 xv[r] = xin_zero ? 0.0 : ldv<COH>(xin + s);
                 cv[r] = __ldg(lv.c + s);
                 breg[col][r] = ldv<COH>(b + s);
-                if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));
+                if (has_xi<XIM>(lv)) breg[col][r] = __ddiv_rn(breg[col][r], __ldg(lv.xi + s));
                 rd[col][r] = __ldg(lv.rd + s);
                 if (PC) xv[r] -= prolong_e<COH>(pt, odd[0], odd[1], rx - H + bx0, ry - H + by0, ec);   // x <- x - P e_c
             }
@@ -622,7 +623,7 @@ __device__ __forceinline__ void gs_fast(const LevelDev& lv, int t, const double*
                 const int nsw = marg >= base ? min(NS, (marg - base) / 2 + 1) : 0;
                 if (nsw > 0) {
                     breg[col][r] = ldv<COH>(b + s); rd[col][r] = __ldg(lv.rd + s);
-                    if (has_xi<XIM>(lv)) breg[col][r] = __dmul_rn(breg[col][r], __ldg(lv.rxi + s));
+                    if (has_xi<XIM>(lv)) breg[col][r] = __ddiv_rn(breg[col][r], __ldg(lv.xi + s));
                 }
                 if ((DR && marg >= H - 1) || (AP && marg >= H)) prefetch_l2(lv.lam + s);         // read by the restriction epilogue
                 act |= (unsigned)(nsw | (tpar << 2)) << (4 * (col * ROUNDS + r));
