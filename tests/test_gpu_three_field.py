@@ -234,3 +234,36 @@ def test_inadmissible_coefficients(gpu, oracle_mod):
     xs, it, rr, rc = s.solve(f, x0, 1e-10)
     assert rc >= 0
     s.close()
+
+
+def test_time_stepping_three_fields(gpu, oracle_mod):
+    """BASELINE.json configs[4] at reduced size in the three-field form: lambda, c and the right-hand side perturbed every
+    step by the workload's rule, xi multiplied by a seeded 5 % perturbation every step, warm start, output aliasing the
+    guess; device- and host-buffer entry points alternate."""
+    pl = W.make_plane(5, 257)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    xi = xi_field(pl, 23)
+    xo, xg, cur = pl.x0.copy(), dev(pl.x0), pl
+    rng = np.random.default_rng(99)
+    for k in range(4):
+        o.update3(cur.lam, xi, cur.c)
+        ro = o.solve(cur.f, xo, 1e-10)
+        if k % 2 == 0:
+            s.update_coeffs3(dev(cur.lam), dev(xi), dev(cur.c))
+        else:
+            s.update_coeffs3_host(cur.lam, xi, cur.c)
+        for lv in range(o.levels):
+            assert rel(s.level_xi(lv), o.level_xi(lv)) <= TOL_STEP
+            assert rel(s.level_coeffs(lv)[0], o.level_coeffs(lv)[0]) <= TOL_STEP
+        _, iters, relres, rc = s.solve(dev(cur.f), xg, 1e-10, x=xg)
+        assert rc == 0 and ro["status"] == 0 and abs(iters - ro["iters"]) <= 1
+        assert rel(host(xg), ro["x"]) <= TOL_SOLVE and relres < 1e-10
+        if k == 0:
+            first_iters = iters
+        else:
+            assert iters < first_iters
+        xo = ro["x"]
+        cur = W.next_step(cur, k)
+        xi = xi * (1.0 + 0.05 * rng.uniform(-1.0, 1.0, pl.n))
+    s.close()
