@@ -267,3 +267,32 @@ def test_time_stepping_three_fields(gpu, oracle_mod):
         cur = W.next_step(cur, k)
         xi = xi * (1.0 + 0.05 * rng.uniform(-1.0, 1.0, pl.n))
     s.close()
+
+
+@pytest.mark.parametrize("neumann", [False, True])
+def test_paper_annulus_mms_v55_three_fields_as_printed(gpu, oracle_mod, neumann):
+    """The paper's verification case with lambda, xi, c as Eq. 21 prints them (xi not absorbed), V(5,5):
+    parity with the oracle, and the discretisation error against Eq. 22."""
+    from tests.test_oracle_paper_mms import discrete_offsets
+    h, levels = 2e-3, 5
+    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=False)
+    xi = pl.meta["xi"]
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
+    f = pl.f
+    if neumann:
+        oR, oZ = discrete_offsets(o.level_arrays(0), pl.n)
+        f = W.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
+    o.update3(pl.lam, xi, pl.c)
+    ro = o.solve(f, pl.x0, 1e-10)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
+    s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+    rng = np.random.default_rng(9)
+    n0 = o.level_n(0)
+    x, b = rng.standard_normal(n0), rng.standard_normal(n0)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    xg, iters, relres, rc = s.solve(dev(f), dev(pl.x0), 1e-10)
+    assert rc == 0 and ro["status"] == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xg), ro["x"]) <= TOL_SOLVE
+    m = pl.kind == 0
+    err = np.linalg.norm(host(xg)[m] - pl.meta["phi"][m]) / np.linalg.norm(pl.meta["phi"][m])
+    assert err < (1.2e-2 if neumann else 1e-4)              # O(h) / O(h^2) at h = 2e-3 (PAPER.md:274)
+    s.close()

@@ -25,15 +25,18 @@ def discrete_offsets(lv, n):
     return W.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
 
 
-def solve_case(om, h, levels, neumann):
-    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann)
+def solve_case(om, h, levels, neumann, three_field=False):
+    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=not three_field)
     o = om.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=int(GOLD["nu_pre"]), nu_post=int(GOLD["nu_post"]))
     f = pl.f
     if neumann:
         lv = o.level_arrays(0)
         oR, oZ = discrete_offsets(lv, pl.n)
         f = W.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
-    o.update(pl.lam, pl.c)
+    if three_field:
+        o.update3(pl.lam, pl.meta["xi"], pl.c)
+    else:
+        o.update(pl.lam, pl.c)
     r = o.solve(f, pl.x0, GOLD["rtol"])
     assert r["status"] == 0
     m = pl.kind == 0
@@ -62,3 +65,17 @@ def test_P10_convergence_order_and_iteration_band(oracle_mod, neumann, order):
         assert order - 0.5 < np.log2(a / b) < order + 0.7, (e2, einf)
     # 11 iterations at the coarsest resolution, 17 at the finest of six; slow growth
     assert all(GOLD["iters_first"] - 5 <= k <= GOLD["iters_last"] + 5 for k in its) and its[-1] - its[0] <= 5, its
+
+
+@pytest.mark.parametrize("neumann,order", [(False, GOLD["order_dirichlet"]), (True, GOLD["order_neumann_inner"])])
+def test_P10_three_fields_as_printed(oracle_mod, neumann, order):
+    """The same case with lambda, xi, c handed over as Eq. 21 prints them (orc_update3, xi = R sqrt(r)(2 + cos theta) not
+    absorbed): the discrete solution is the one of the absorbed system (row scaling), so the errors against Eq. 22 are
+    the same to solver tolerance and the orders are the printed ones; the stop test now sees the unscaled residual."""
+    res3 = [solve_case(oracle_mod, H0 / 2 ** k, int(GOLD["levels_first"]) + k, neumann, three_field=True) for k in range(2)]
+    res2 = [solve_case(oracle_mod, H0 / 2 ** k, int(GOLD["levels_first"]) + k, neumann) for k in range(2)]
+    for a, b in zip(res3, res2):
+        assert a[2] == pytest.approx(b[2], rel=1e-3)                 # same discretisation error
+        assert abs(a[1] - b[1]) <= 3                                  # and about the same iteration count
+    assert order - 0.35 < np.log2(res3[0][2] / res3[1][2]) < order + 0.6
+    assert all(GOLD["iters_first"] - 5 <= r[1] <= GOLD["iters_last"] + 5 for r in res3)
