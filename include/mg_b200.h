@@ -103,8 +103,8 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
 int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream);
 
 /* update for the paper's three-field form  lambda phi - xi div(c grad phi) = rho  (Eq. 3; the row of
- * point (i,j) carries xi_{i,j}/2, Eq. 10).  d_xi: DEVICE, length n, user order, > 0 on inner points
- * (guard rows, Eq. 11 / 16, do not see it); it is transferred to the coarser levels like lambda and c
+ * point (i,j) carries xi_{i,j}/2, Eq. 10).  d_xi: DEVICE, length n, user order, > 0 on ALL points
+ * (guard rows, Eq. 11 / 16, do not contain it, but the coarser levels average over guards too); it is transferred to the coarser levels like lambda and c
  * (PAPER.md:153, 207).  d_xi == NULL is mg_update_coeffs (xi = 1).  The handle keeps the form of the
  * last update; switching forms re-captures the iteration graph at the next solve.  The stop test of mg_solve is
  * on the residual of the three-field rows.  Costs 8 B per point and smoothing launch (and one fp64 division per point) more than the two-field form. */
