@@ -198,3 +198,81 @@ def test_P7_ordering_independence(oracle_mod):
     ra, rb = oa.solve(a.f, a.x0, 1e-10), ob.solve(b.f, b.x0, 1e-10)
     assert ra["iters"] == rb["iters"]
     assert np.array_equal(H.canon(oa, ra["x"]), H.canon(ob, rb["x"]))
+
+
+def _geoms():
+    return [H.small_annulus(65, 3), H.small_dshape(129, 4), H.random_blob_plane(3), H.random_blob_plane(4)]
+
+
+def test_P6_set_bnds_hom_and_prolongation_brute_force(oracle_mod):
+    """Rule T3 on ragged meshes with Neumann guards, every level.  The correction e = P e_c must (i) equal the
+    bilinear interpolation of P:153 / Fig. 3 on fine inner points, parents absent from the coarse mesh counting 0
+    (written here from the weights 1 / (1/2, 1/2) / (1/4 x 4) with a dict on (I, J)); (ii) vanish on Dirichlet guards
+    (homogeneous Eq. 11); (iii) satisfy the HOMOGENEOUS Neumann row on Neumann guards: (A e)_l = 0
+    (Eq. 16, with Gamma = 0; set_bnds_hom) — fallback guards included.  Dropping the 1/(1 - w_self)
+    of half-integer normals, or leaving Neumann guards at 0, fails (iii)."""
+    rng = np.random.default_rng(11)
+    n_neu = n_fb = n_half = 0
+    for pl in _geoms():
+        o = H.make_oracle(oracle_mod, pl)
+        for s in range(o.levels - 1):
+            fa, ca = o.level_arrays(s), o.level_arrays(s + 1)
+            nf, nc = o.level_n(s), o.level_n(s + 1)
+            ec = rng.standard_normal(nc)
+            e = -o.prolong_correct(s, ec, np.zeros(nf))
+            cmap = {(int(i), int(j)): k for k, (i, j) in enumerate(zip(ca["I"], ca["J"]))}
+            val = lambda ci, cj: ec[cmap[(ci, cj)]] if (ci, cj) in cmap else 0.0
+            exp = np.zeros(nf)
+            for l in np.nonzero(fa["kind"] == 0)[0]:
+                I, J = int(fa["I"][l]), int(fa["J"][l])
+                Il, Jl = I // 2, J // 2                             # Python floor division: lower coarse index
+                if I % 2 == 0 and J % 2 == 0:
+                    exp[l] = val(Il, Jl)
+                elif J % 2 == 0:
+                    exp[l] = 0.5 * val(Il, Jl) + 0.5 * val(Il + 1, Jl)
+                elif I % 2 == 0:
+                    exp[l] = 0.5 * val(Il, Jl) + 0.5 * val(Il, Jl + 1)
+                else:
+                    exp[l] = 0.25 * (val(Il, Jl) + val(Il + 1, Jl) + val(Il, Jl + 1) + val(Il + 1, Jl + 1))
+            inner, dirich, neum = fa["kind"] == 0, fa["kind"] == 1, fa["kind"] == 2
+            assert np.abs(e[inner] - exp[inner]).max() <= 1e-15 * np.abs(ec).max()
+            assert np.array_equal(e[dirich], np.zeros(dirich.sum()))
+            Ae = o.apply(s, e)
+            h = o.level_h(s)
+            assert np.abs(Ae[neum]).max(initial=0.0) <= 4e-16 * np.abs(ec).max() / h
+            if neum.any():                                       # the guards really carry the interpolated values
+                assert np.abs(e[neum]).max() > 0.0
+            n_neu += int(neum.sum())
+            n_fb += int((neum & (fa["ns_fallback"] == 1)).sum())
+            n_half += int((neum & (fa["ns_fallback"] == 0) & ((np.abs(fa["ns_tn"]) % 2).sum(axis=1) > 0)).sum())
+    assert n_neu > 500 and n_fb > 0 and n_half > 50              # every branch of set_bnds_hom was exercised
+
+
+def test_P6_restriction_brute_force_ragged(oracle_mod):
+    """Rule T2 next to ragged boundaries, every level: d_c(I, J) = 1/16 [1 2 1; 2 4 2; 1 2 1] over the fine INNER
+    points (2I+dx, 2J+dy) present (fine guards and absent points contribute 0) on coarse inner rows; coarse
+    guard rows are 0.  Written here with dicts on (I, J), independent of the oracle's fine9 tables."""
+    rng = np.random.default_rng(12)
+    near = 0
+    for pl in _geoms():
+        o = H.make_oracle(oracle_mod, pl)
+        for s in range(o.levels - 1):
+            fa, ca = o.level_arrays(s), o.level_arrays(s + 1)
+            d = rng.standard_normal(o.level_n(s))
+            got = o.restrict(s, d)
+            fmap = {(int(i), int(j)): k for k, (i, j) in enumerate(zip(fa["I"], fa["J"]))}
+            exp = np.zeros(o.level_n(s + 1))
+            for q in np.nonzero(ca["kind"] == 0)[0]:
+                I, J = int(ca["I"][q]), int(ca["J"][q])
+                acc = 0.0
+                for dy in (-1, 0, 1):
+                    for dx in (-1, 0, 1):
+                        l = fmap.get((2 * I + dx, 2 * J + dy), -1)
+                        if l >= 0 and fa["kind"][l] == 0:
+                            acc += (2 - abs(dx)) * (2 - abs(dy)) / 16.0 * d[l]
+                        else:
+                            near += 1
+                exp[q] = acc
+            assert np.abs(got - exp).max() <= 2e-16 * 4
+            assert np.array_equal(got[ca["kind"] != 0], np.zeros((ca["kind"] != 0).sum()))
+    assert near > 1000                                             # stencils with missing / guard fine points were hit

@@ -142,12 +142,10 @@ def test_P9_krylov_invariants(oracle_mod):
     V, Z, Hh, k = r["V"], r["Z"], r["H"], r["ncols"]
     assert k >= 5 and r["status"] == 0
     Vk = V[:k]                                                     # v_{k+1} is not formed on exit
-    # modified Gram-Schmidt: orthogonal to rounding while the residual is still large; the loss grows
-    # like eps*cond/residual near convergence (Paige-Rozloznik-Strakos), so bound it by that product
+    # modified Gram-Schmidt applied TWICE (rule K2, reading G22): the basis is orthonormal to working precision in
+    # every column, also near convergence where a single pass loses orthogonality like eps*cond/residual
     G = np.abs(Vk @ Vk.T - np.eye(k))
-    assert G[:6, :6].max() <= 1e-11
-    for j in range(2, k):
-        assert G[:j + 1, :j + 1].max() * r["hist"][j - 1] <= 1e-10
+    assert G.max() <= 1e-13
     # Arnoldi relation A Z_k = V_{k+1} H_k (flexible GMRES, Saad [29]) on the first k-1 columns
     lhs = A @ Z[:k - 1].T
     rhs = V[:k].T @ Hh[:k, :k - 1]
