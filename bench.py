@@ -399,6 +399,7 @@ def run_paper_mms(args):
     events), error against the manufactured solution.  Context for BASELINE.md, not the headline metric."""
     import torch
     from paper_2509_11831_b200 import binding as B
+    from tests import cases as TC      # the paper-case generator is test material (sympy); only this option needs it
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
@@ -407,13 +408,13 @@ def run_paper_mms(args):
     for k in range(args.paper_mms):
         h, levels = 4e-3 / 2 ** k, 4 + k
         for neumann in (False, True):
-            pl = W.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=not args.three_field)
+            pl = TC.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=not args.three_field)
             s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
             f = pl.f
             if neumann:
                 lv = s.level_info(0)
-                oR, oZ = W.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
-                f = W.neumann_gamma(pl, oR[lv["user2canon"]], oZ[lv["user2canon"]])
+                oR, oZ = TC.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
+                f = TC.neumann_gamma(pl, oR[lv["user2canon"]], oZ[lv["user2canon"]])
             d_lam, d_c, d_f, d_x0 = dev(pl.lam), dev(pl.c), dev(f), dev(pl.x0)
             d_xi = dev(pl.meta["xi"]) if args.three_field else None      # Eq. 21's xi as printed, not absorbed
             sol, upd = [], []

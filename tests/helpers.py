@@ -3,6 +3,7 @@ dicts; shares nothing with oracle/ or the CUDA package)."""
 import numpy as np
 
 from paper_2509_11831_b200 import workloads as W
+from tests import cases as TC
 
 
 def make_oracle(om, pl, **kw):
@@ -23,7 +24,7 @@ def square_plane(n, levels, lam=1.0, c=1.0):
     inner = W.square_mask(n)
     h = 1.0 / (n - 1)
     neu = np.zeros((n, n), bool)
-    return W.mask_plane(inner, neu, h, lam_f=np.full((n, n), lam), c_f=np.full((n, n), c), levels=levels)
+    return TC.mask_plane(inner, neu, h, lam_f=np.full((n, n), lam), c_f=np.full((n, n), c), levels=levels)
 
 
 def small_annulus(n=33, levels=2, seed=5, neumann_inner=True, i0=0, j0=0, order="rowmajor"):
@@ -36,7 +37,7 @@ def small_annulus(n=33, levels=2, seed=5, neumann_inner=True, i0=0, j0=0, order=
     lam = 0.5 + rng.uniform(0, 1, (n, n))
     c = np.exp(0.5 * rng.standard_normal((n, n)))
     f = rng.standard_normal((n, n))
-    return W.mask_plane(inner, neu, h, lam, c, f, levels=levels, i0=i0, j0=j0, order=order, seed=seed)
+    return TC.mask_plane(inner, neu, h, lam, c, f, levels=levels, i0=i0, j0=j0, order=order, seed=seed)
 
 
 def small_dshape(n=33, levels=2, seed=7, order="rowmajor"):
@@ -49,7 +50,7 @@ def small_dshape(n=33, levels=2, seed=7, order="rowmajor"):
     lam = 0.01 + rng.uniform(0, 1, (n, n))
     c = np.exp(rng.standard_normal((n, n)) + np.log(10.0) * closed)
     f = rng.standard_normal((n, n))
-    return W.mask_plane(inner, neu, h, lam, c, f, levels=levels, order=order, seed=seed)
+    return TC.mask_plane(inner, neu, h, lam, c, f, levels=levels, order=order, seed=seed)
 
 
 def random_blob_plane(seed, n=97):
@@ -66,7 +67,7 @@ def random_blob_plane(seed, n=97):
     lam = 0.2 + rng.uniform(0, 1, (n, n))
     c = np.exp(0.7 * W.gaussian_field(rng, n, 0.1, h))
     f = rng.standard_normal((n, n))
-    return W.mask_plane(inner, neu, h, lam, c, f, levels=0, i0=-41 - seed, j0=-13 + 2 * seed, seed=seed,
+    return TC.mask_plane(inner, neu, h, lam, c, f, levels=0, i0=-41 - seed, j0=-13 + 2 * seed, seed=seed,
                         order="shuffle" if seed % 2 else "rowmajor")
 
 

@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 from paper_2509_11831_b200 import workloads as W
+from tests import cases as TC
 from tests import helpers as H
 
 pytestmark = pytest.mark.gpu
@@ -357,7 +358,7 @@ def test_guard_list_overflow_path(gpu, oracle_mod):
     lam = 0.5 + rng.uniform(0, 1, (n, n))
     c = np.exp(0.3 * rng.standard_normal((n, n)))
     f = rng.standard_normal((n, n))
-    pl = W.mask_plane(inner, neu, 1.0 / (n - 1), lam, c, f, levels=7)
+    pl = TC.mask_plane(inner, neu, 1.0 / (n - 1), lam, c, f, levels=7)
     assert (pl.kind != 0).sum() > 300000
     o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=7)
     o.update(pl.lam, pl.c)
@@ -387,12 +388,12 @@ def test_paper_annulus_mms_v55(gpu, oracle_mod, neumann):
     parity with the oracle, and the discretisation error against the manufactured solution is the oracle's."""
     from tests.test_oracle_paper_mms import discrete_offsets
     h, levels = 2e-3, 5
-    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann)
+    pl = TC.make_paper_annulus(h, levels, neumann_inner=neumann)
     o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
     f = pl.f
     if neumann:
         oR, oZ = discrete_offsets(o.level_arrays(0), pl.n)
-        f = W.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
+        f = TC.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
     o.update(pl.lam, pl.c)
     ro = o.solve(f, pl.x0, 1e-10)
     s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)

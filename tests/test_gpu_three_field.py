@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 from paper_2509_11831_b200 import workloads as W
+from tests import cases as TC
 from tests import helpers as H
 from tests.test_gpu_parity import TOL_SOLVE, TOL_STEP, dev, gpu, host, rel  # noqa: F401  (gpu is a fixture)
 
@@ -275,13 +276,13 @@ def test_paper_annulus_mms_v55_three_fields_as_printed(gpu, oracle_mod, neumann)
     parity with the oracle, and the discretisation error against Eq. 22."""
     from tests.test_oracle_paper_mms import discrete_offsets
     h, levels = 2e-3, 5
-    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=False)
+    pl = TC.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=False)
     xi = pl.meta["xi"]
     o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)
     f = pl.f
     if neumann:
         oR, oZ = discrete_offsets(o.level_arrays(0), pl.n)
-        f = W.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
+        f = TC.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
     o.update3(pl.lam, xi, pl.c)
     ro = o.solve(f, pl.x0, 1e-10)
     s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=5, nu_post=5)

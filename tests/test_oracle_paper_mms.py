@@ -12,6 +12,7 @@ import numpy as np
 import pytest
 
 from paper_2509_11831_b200 import workloads as W
+from tests import cases as TC
 
 GOLD = {}
 for _line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_mms.txt")):
@@ -22,17 +23,17 @@ H0 = GOLD["h_first"]
 
 
 def discrete_offsets(lv, n):
-    return W.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
+    return TC.neumann_offsets(lv["kind"], lv["ns_tn"], lv["ns_fallback"], lv["nbr"])
 
 
 def solve_case(om, h, levels, neumann, three_field=False):
-    pl = W.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=not three_field)
+    pl = TC.make_paper_annulus(h, levels, neumann_inner=neumann, absorb_xi=not three_field)
     o = om.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=levels, nu_pre=int(GOLD["nu_pre"]), nu_post=int(GOLD["nu_post"]))
     f = pl.f
     if neumann:
         lv = o.level_arrays(0)
         oR, oZ = discrete_offsets(lv, pl.n)
-        f = W.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
+        f = TC.neumann_gamma(pl, oR[o.user2canon], oZ[o.user2canon])
     if three_field:
         o.update3(pl.lam, pl.meta["xi"], pl.c)
     else:
@@ -45,7 +46,7 @@ def solve_case(om, h, levels, neumann, three_field=False):
 
 
 def test_point_count_at_the_papers_coarsest_resolution():
-    pl = W.make_paper_annulus(H0, int(GOLD["levels_first"]))
+    pl = TC.make_paper_annulus(H0, int(GOLD["levels_first"]))
     # the paper's N = 25 726 includes its (thicker) guard layer; one 4-adjacent layer gives a few per cent fewer points
     assert 0.93 * GOLD["n_first"] < pl.n < GOLD["n_first"]
     # inner points = lattice points with 0.2 < r < 0.4: pi (0.4^2 - 0.2^2) / h^2 = 23 562 up to the lattice-point discrepancy
