@@ -43,8 +43,13 @@ enum {
     MG_EINVAL = -1,       /* null pointer, n <= 0, h <= 0, bad option, bad level                         */
     MG_EMESH = -2,        /* duplicate (i,j); inner point lacking a neighbour; guard without an inner
                              4-neighbour (rule M2); coarsest level too large for the dense solve */
-    MG_ECOEFF = -3,       /* mg_solve: the last update's fields were not admissible: c <= 0,
-                             xi <= 0, or a non-finite value (tested on the device during the update)      */
+    MG_ECOEFF = -3,       /* mg_solve / single-step calls: the last update's fields were not admissible: c <= 0
+                             (PAPER.md:51), xi <= 0, a non-finite value, or a coarsest-level operator that is
+                             singular (zero / non-finite pivot) — all tested on the device during the update.
+                             Deviations from a synchronous check, both deliberate: the update itself returns
+                             MG_OK and the NEXT call that uses the operators reports the error (the update
+                             is asynchronous, G26); lambda < 0 is accepted (the paper's own test
+                             case has lambda of both signs, Eq. 21)                            */
     MG_ENOTREADY = -4,    /* solve / cycle before the first mg_update_coeffs                             */
     MG_ECUDA = -5,        /* CUDA runtime error or no device                                             */
     MG_ENOMEM = -6
@@ -86,7 +91,8 @@ typedef struct {
 } mg_options;
 
 /* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).
- * alloc returns a device pointer or NULL; both may be NULL to restore cudaMalloc/cudaFree. */
+ * alloc returns a device pointer or NULL; both may be NULL to restore cudaMalloc/cudaFree.  A handle remembers the
+ * pair that was installed when it was created and uses it for all its later allocations and in mg_destroy. */
 typedef void* (*mg_alloc_fn)(uint64_t bytes, void* stream);
 typedef void (*mg_free_fn)(void* ptr);
 int mg_set_allocator(mg_alloc_fn alloc_fn, mg_free_fn free_fn);
@@ -114,7 +120,9 @@ int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, c
  * on ||A x - f|| / ||f|| < rtol (Eq. 23).  d_f, d_x0, d_x: DEVICE, length n, user order;
  * d_x may alias d_x0.  iters (HOST, may be NULL) receives the number of preconditioner applications,
  * final_relres (HOST, may be NULL) the recomputed true relative residual.  Returns after the stream
- * has finished the solve.  Returns MG_OK, MG_NOT_CONVERGED, MG_BREAKDOWN or an error. */
+ * has finished the solve.  Returns MG_OK, MG_NOT_CONVERGED, MG_BREAKDOWN or an error.  On MG_NOT_CONVERGED
+ * mg_last_error() says whether the recurrence residual had passed rtol while the recomputed true residual had not
+ * (rtol below the accuracy attainable in fp64 on this mesh; the method has no stagnation exit). */
 int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, double rtol, int* iters,
              double* final_relres, void* stream);
 

@@ -27,6 +27,11 @@ class MgError(RuntimeError):
         self.code = code
 
 
+def last_error() -> str:
+    """mg_last_error(): the calling thread's last error / diagnostic text."""
+    return lib().mg_last_error().decode()
+
+
 class _Mesh(C.Structure):
     _fields_ = [("n", C.c_int64), ("i", C.c_void_p), ("j", C.c_void_p), ("h", C.c_double)]
 

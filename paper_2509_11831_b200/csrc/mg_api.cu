@@ -33,7 +33,7 @@ mg_free_fn g_free = nullptr;
 struct LevelBuf {           // device arrays owned per level
     uint16_t* code = nullptr;
     uint8_t* tflag = nullptr;
-    int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr;
+    int32_t *tnb = nullptr, *ctab = nullptr, *ptab = nullptr, *tij = nullptr, *canon2slot = nullptr, *tlist[2] = {nullptr, nullptr}, *smeta[2] = {nullptr, nullptr};
     double* xi = nullptr;   // three-field form only: allocated by the first mg_update_coeffs3 with xi
     double *lam = nullptr, *c = nullptr, *rd = nullptr, *x = nullptr, *x2 = nullptr, *b = nullptr, *d = nullptr;
     double* tb = nullptr;   // right-hand side of the single-step entry points.  The cycle's own b of a coarse level is written ONLY by
@@ -80,6 +80,9 @@ struct mg_handle_s {
     cudaGraphExec_t iter_graph = nullptr;
     int64_t iter_graph_kernels = 0;
     int64_t launches = 0;
+    mg_alloc_fn alloc = nullptr;          // allocator installed when the handle was created: used for every later allocation
+    mg_free_fn free_fn = nullptr;         // of this handle and by mg_destroy, whatever mg_set_allocator is called with afterwards
+    int device = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // solve, update, single step
     cudaEvent_t hev[2] = {nullptr, nullptr};   // header copies of the two Arnoldi steps in flight
     bool solve_timed = false, update_timed = false, step_timed = false;
@@ -90,8 +93,8 @@ namespace {
 int dev_alloc(mg_handle h, void** p, size_t bytes, cudaStream_t s) {
     *p = nullptr;
     if (bytes == 0) bytes = 8;
-    if (g_alloc) {
-        *p = g_alloc((uint64_t)bytes, (void*)s);
+    if (h->alloc) {
+        *p = h->alloc((uint64_t)bytes, (void*)s);
         if (!*p) { g_last_error = "allocator returned NULL"; return MG_ENOMEM; }
     } else {
         cudaError_t e = cudaMalloc(p, bytes);
@@ -111,6 +114,24 @@ int upload(mg_handle h, T** dst, const std::vector<T>& src, cudaStream_t s) {
 }
 
 Launch LZ(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }
+
+// The last update's device-side admissibility flag (G26), already copied to h_hdr[16]: MG_ECOEFF with the reason.
+int coeff_error(int b) {
+    g_last_error = std::string("inadmissible coefficients in the last update:") + ((b & 1) ? " lambda not finite;" : "") +
+                   ((b & 2) ? " c not finite or <= 0 (PAPER.md:51);" : "") + ((b & 4) ? " xi not finite or <= 0;" : "") +
+                   ((b & 8) ? " the coarsest-level operator is singular (zero or non-finite pivot);" : "");
+    return MG_ECOEFF;
+}
+
+// Single-step entry points: read the flag of an update that has not been checked yet (one small synchronous copy).
+int check_coeffs(mg_handle h, cudaStream_t s) {
+    if (h->coeffs_unchecked) {
+        CU(cudaMemcpyAsync(h->h_hdr + 16, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        h->coeffs_unchecked = false;
+    }
+    return h->h_hdr[16] ? coeff_error(h->h_hdr[16]) : MG_OK;
+}
 
 // nu Gauss-Seidel sweeps, two per launch where possible, ping-ponging between `cur` and `other`.
 // Returns the buffer that holds the result.
@@ -282,7 +303,7 @@ int mg_destroy(mg_handle h) {
     for (auto& e : h->hev) if (e) cudaEventDestroy(e);
     if (h->h_hdr) cudaFreeHost(h->h_hdr);
     if (h->h_state) cudaFreeHost(h->h_state);
-    for (void* p : h->allocs) { if (g_free) g_free(p); else cudaFree(p); }
+    for (void* p : h->allocs) { if (h->free_fn) h->free_fn(p); else cudaFree(p); }
     delete h;
     return MG_OK;
 }
@@ -306,6 +327,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     h->gamma = o.gamma > 1 ? o.gamma : 1;
     h->full_cgs2 = (o.flags & MG_SETUP_FULL_CGS2) != 0;
     h->n = mesh->n;
+    h->alloc = g_alloc; h->free_fn = g_free;
     int rc = build_hierarchy(mesh->n, mesh->i, mesh->j, bc->kind, mesh->h, o.levels, h->hh);
     if (rc) { g_last_error = h->hh.err; delete h; return rc; }
     h->L = (int)h->hh.lev.size();
@@ -313,6 +335,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (h->nL > 1024) { g_last_error = "coarsest level has more than 1024 points; use more levels"; delete h; return MG_EMESH; }
     if (host_only) { h->host_only = true; *out = h; return MG_OK; }
     cudaStream_t s = (cudaStream_t)stream;
+    cudaGetDevice(&h->device);
     auto fail = [&](int code) { mg_destroy(h); return code; };
 #define TRY(x) do { int rc__ = (x); if (rc__) return fail(rc__); } while (0)
 #define CUF(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { g_last_error = std::string(#call) + ": " + cudaGetErrorString(e__); return fail(MG_ECUDA); } } while (0)
@@ -336,6 +359,16 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         for (int t = 0; t < hl.ntiles; t++) { tij[2 * t] = hl.tI[t]; tij[2 * t + 1] = hl.tJ[t]; }
         TRY(upload(h, &b.tij, tij, s));
         TRY(upload(h, &b.canon2slot, hl.canon2slot, s));
+        for (int k = 0; k < 2; k++) {
+            TRY(upload(h, &b.tlist[k], hl.tlist[k], s));
+            std::vector<int32_t> meta((size_t)24 * hl.nint[k], 0);           // tables of the interior tiles, packed in list order
+            for (int32_t q = 0; q < hl.nint[k]; q++) {
+                const int32_t t = hl.tlist[k][q];
+                for (int e = 0; e < 9; e++) { meta[24 * (size_t)q + e] = hl.tnb[9 * (size_t)t + e]; meta[24 * (size_t)q + 9 + e] = hl.ptab.empty() ? 0 : hl.ptab[9 * (size_t)t + e]; }
+                meta[24 * (size_t)q + 18] = hl.tI[t] & 1; meta[24 * (size_t)q + 19] = hl.tJ[t] & 1; meta[24 * (size_t)q + 20] = t;
+            }
+            TRY(upload(h, &b.smeta[k], meta, s));
+        }
         const size_t vb = (size_t)hl.nslots() * sizeof(double);
         TRY(dev_alloc(h, (void**)&b.lam, vb, s));
         TRY(dev_alloc(h, (void**)&b.c, vb, s));
@@ -353,11 +386,12 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
         d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c; d.rd = b.rd; d.tflag = b.tflag;
         d.xi = nullptr;
+        for (int k = 0; k < 2; k++) { d.tlist[k] = b.tlist[k]; d.nint[k] = hl.nint[k]; d.smeta[k] = b.smeta[k]; }
     }
     TRY(dev_alloc(h, (void**)&h->d_lev, sizeof(LevelDev) * h->L, s));
     CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
     h->no_fused_dr = getenv("MG_B200_NO_FUSED_DR") != nullptr;
-    h->tail_cap = std::min(tail_max_grid(), 2 * 148);
+    h->tail_cap = std::min(tail_max_grid(), 2 * dev_info().sms);
     if (h->tail_cap > 0 && h->nu_pre >= 1 && h->nu_post >= 1 && ((o.flags & MG_SETUP_FUSED_TAIL) || getenv("MG_B200_FUSED_TAIL")))
         for (int l = h->L - 1; l >= 0 && h->lev[l].ntiles <= h->tail_cap; l--) h->tail_s0 = l;
     TRY(upload(h, &h->user2slot, h->hh.user2slot, s));
@@ -369,7 +403,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     TRY(dev_alloc(h, (void**)&h->xs, v0, s));
     TRY(dev_alloc(h, (void**)&h->bs, v0, s));
     TRY(dev_alloc(h, (void**)&h->st, sizeof(GmresState), s));
-    TRY(dev_alloc(h, (void**)&h->partial, sizeof(double) * RED_BLOCKS * (MAX_M + 2), s));
+    TRY(dev_alloc(h, (void**)&h->partial, sizeof(double) * RED_BLOCKS_MAX * (MAX_M + 2), s));
     {   // coarsest level: canonical row -> slot and its inverse
         HostLevel& cl = h->hh.lev.back();
         std::vector<int32_t> s2r((size_t)cl.nslots(), 0);
@@ -429,7 +463,7 @@ int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, c
     h->coeffs_unchecked = true;
     for (int l = 0; l + 1 < h->L; l++) launch_restrict_coeff(L, h->lev[l], h->lev[l + 1]);     // rule T4
     for (int l = 0; l < h->L; l++) launch_diag(L, h->lev[l]);                                   // U2: 1 / a_ll for the smoother
-    launch_coarse_factor(L, h->lev[h->L - 1], h->cslot, h->slot2row, h->nL, h->cwork, h->Ainv);   // rule C
+    launch_coarse_factor(L, h->lev[h->L - 1], h->cslot, h->slot2row, h->nL, h->cwork, h->Ainv, h->coeff_bad);   // rule C
     CU(cudaEventRecord(h->ev[3], s));
     CU(cudaGetLastError());
     h->have_coeffs = true;
@@ -444,6 +478,7 @@ int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, voi
 int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, double rtol, int* iters,
              double* final_relres, void* stream) {
     if (!h || !d_f || !d_x0 || !d_x || !(rtol > 0.0)) return MG_EINVAL;
+    if (h->host_only) return MG_ECUDA;
     if (!h->have_coeffs) return MG_ENOTREADY;
     cudaStream_t s = (cudaStream_t)stream;
     Launch L = LZ(h, s);
@@ -465,10 +500,8 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
         CU(cudaStreamSynchronize(s));
         h->coeffs_unchecked = false;
         if (h->h_hdr[16]) {                                           // the last update's fields were not admissible
-            const int b = h->h_hdr[16];
-            g_last_error = std::string("inadmissible coefficients in the last update:") + ((b & 1) ? " lambda not finite;" : "") +
-                           ((b & 2) ? " c not finite or <= 0 (PAPER.md:51);" : "") + ((b & 4) ? " xi not finite or <= 0;" : "");
-            return MG_ECOEFF;
+            h->solve_timed = false;                                   // ev[0] has no matching end event
+            return coeff_error(h->h_hdr[16]);
         }
         status = h->h_hdr[2];
         if (h->h_hdr[3]) break;                                       // cycle_end set by start: finished
@@ -498,6 +531,21 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
     if (final_relres) *final_relres = h->h_state->relres;
     if (status == 1 || status == 4) return MG_OK;
     if (status == 3) return MG_BREAKDOWN;
+    {   // Not converged.  If the recurrence residual (Eq. 23 inside a cycle, rule K3) went below rtol while the recomputed true
+        // residual (rule K5) did not, the solve sits on the fp64 floor of evaluating b - A x, about eps |A||x| / |b| ~ 1/h^2
+        // (DESIGN.md "Attainable accuracy"); the paper has no stagnation exit, so the call only says so.
+        const GmresState* st = h->h_state;
+        const int k = std::min(st->iters, 512);
+        double best = 1e300;
+        for (int i = 0; i < k; i++) best = std::min(best, st->hist[i]);
+        char buf[320];
+        if (k > 0 && best < rtol)
+            snprintf(buf, sizeof buf, "not converged after %d iterations: the recurrence residual reached %.2e < rtol = %.2e but the true residual "
+                     "|b - A x| / |b| stays at %.2e: rtol is below the accuracy attainable in fp64 on this mesh", st->iters, best, rtol, st->relres);
+        else
+            snprintf(buf, sizeof buf, "not converged after %d iterations: |b - A x| / |b| = %.2e, rtol = %.2e", st->iters, st->relres, rtol);
+        g_last_error = buf;
+    }
     return MG_NOT_CONVERGED;
 }
 
@@ -509,6 +557,7 @@ static int ensure_stage(mg_handle h, cudaStream_t s) {
 
 int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c, void* stream) {
     if (!h || !h_lambda || !h_c) return MG_EINVAL;
+    if (h->host_only) return MG_ECUDA;
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
@@ -520,6 +569,7 @@ int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c
 int mg_update_coeffs3_host(mg_handle h, const double* h_lambda, const double* h_xi, const double* h_c, void* stream) {
     if (!h || !h_lambda || !h_c) return MG_EINVAL;
     if (!h_xi) return mg_update_coeffs_host(h, h_lambda, h_c, stream);
+    if (h->host_only) return MG_ECUDA;
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
@@ -533,6 +583,7 @@ int mg_update_coeffs3_host(mg_handle h, const double* h_lambda, const double* h_
 int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_x, double rtol, int* iters,
                   double* final_relres, void* stream) {
     if (!h || !h_f || !h_x0 || !h_x) return MG_EINVAL;
+    if (h->host_only) return MG_ECUDA;
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
@@ -697,7 +748,8 @@ int mg_level_xi(mg_handle h, int level, double* h_xi, void* stream) {
 }
 
 // ============================================================================ single steps (parity tests)
-#define CHECK_LEVEL(cond) do { if (!h || !(cond)) return MG_EINVAL; if (h->host_only) return MG_ECUDA; if (!h->have_coeffs) return MG_ENOTREADY; } while (0)
+#define CHECK_LEVEL(cond) do { if (!h || !(cond)) return MG_EINVAL; if (h->host_only) return MG_ECUDA; if (!h->have_coeffs) return MG_ENOTREADY; \
+        { int rc__ = check_coeffs(h, (cudaStream_t)stream); if (rc__) return rc__; } } while (0)
 
 int mg_apply(mg_handle h, int level, const double* d_x, double* d_y, void* stream) {
     CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_y);

@@ -73,7 +73,7 @@ __global__ void k_coarse_assemble(LevelDev lv, const int32_t* __restrict__ cslot
 // In-place Gauss-Jordan with partial pivoting (first maximum wins ties) on W = [A | I] -> [I | A^-1].
 // One CTA; when [A | I] fits (n <= ~110) it is worked on in shared memory, so a pivot step costs three
 // barriers instead of three global-memory round trips.
-__global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict__ Wg, double* __restrict__ Ainv, int in_smem) {
+__global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict__ Wg, double* __restrict__ Ainv, int in_smem, int* __restrict__ bad) {
     extern __shared__ __align__(16) double wsm[];
     __shared__ double fac[1024];
     __shared__ double redv[CT / 32];
@@ -105,6 +105,7 @@ __global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict_
             for (int w = 1; w < CT / 32; w++)
                 if (redv[w] > b || (redv[w] == b && redi[w] < i)) { b = redv[w]; i = redi[w]; }
             piv = i < n ? i : k;        // a column of NaNs (inadmissible coefficients, MG_ECOEFF) has no maximum: stay in bounds
+            if (!(b > 0.0) || isinf(b)) atomicOr(bad, 8);      // zero or non-finite pivot: the coarsest operator is singular (the oracle's -2)
         }
         __syncthreads();
         const int p = piv;
@@ -137,7 +138,7 @@ __global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict_
 // step.  Same arithmetic and pivot rule as k_coarse_invert.
 constexpr int CIT = 256;
 __global__ void __launch_bounds__(CIT) k_coarse_invert_coop(int n, int cpb, const double* __restrict__ Wg, double* __restrict__ Ainv,
-                                                            double* colbuf, int* pivbuf) {
+                                                            double* colbuf, int* pivbuf, int* __restrict__ bad) {
     namespace cg = cooperative_groups;
     cg::grid_group grid = cg::this_grid();
     extern __shared__ __align__(16) double csm[];
@@ -167,6 +168,7 @@ __global__ void __launch_bounds__(CIT) k_coarse_invert_coop(int n, int cpb, cons
             for (int w = 1; w < CIT / 32; w++)
                 if (redv[w] > b || (redv[w] == b && redi[w] < i)) { b = redv[w]; i = redi[w]; }
             pivbuf[k & 1] = i < n ? i : k;   // as above
+            if (!(b > 0.0) || isinf(b)) atomicOr(bad, 8);
         }
         for (int r = tid; r < n; r += CIT) colbuf[(size_t)(k & 1) * n + r] = col[r];
         __syncthreads();
@@ -220,22 +222,13 @@ __global__ void __launch_bounds__(CT) k_coarse_solve(const double* __restrict__ 
 }  // namespace
 
 void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
-                          double* work, double* Ainv) {
+                          double* work, double* Ainv, int* bad) {
     k_coarse_assemble<<<(n + 127) / 128, 128, 0, L.stream>>>(lv, cslot, slot2row, n, work);
     const size_t wbytes = (size_t)n * 2 * n * sizeof(double);
     const int in_smem = wbytes <= 200 * 1024;
-    static bool configured = false;
-    static int coop_sms = 0;
-    if (!configured) {
-        cudaFuncSetAttribute(k_coarse_invert, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        cudaFuncSetAttribute(k_coarse_invert_coop, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        int dev = 0, coop = 0, sms = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        coop_sms = coop ? sms : 0;
-        configured = true;
-    }
+    ensure_dyn_smem((const void*)k_coarse_invert, 200 * 1024);
+    ensure_dyn_smem((const void*)k_coarse_invert_coop, 200 * 1024);
+    const int coop_sms = dev_info().coop ? dev_info().sms : 0;
     if (!in_smem && coop_sms > 0) {                           // column slabs over a cooperative grid
         int G = std::min(coop_sms, (2 * n + 3) / 4);
         int cpb = (2 * n + G - 1) / G;
@@ -245,13 +238,13 @@ void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cs
             double* colbuf = work + (size_t)2 * n * n;        // 2 n doubles + 2 ints behind [A | I] (allocated by mg_setup)
             int* pivbuf = reinterpret_cast<int*>(colbuf + 2 * n);
             const double* Wg = work;
-            void* args[] = {(void*)&n, (void*)&cpb, (void*)&Wg, (void*)&Ainv, (void*)&colbuf, (void*)&pivbuf};
+            void* args[] = {(void*)&n, (void*)&cpb, (void*)&Wg, (void*)&Ainv, (void*)&colbuf, (void*)&pivbuf, (void*)&bad};
             cudaLaunchCooperativeKernel((const void*)k_coarse_invert_coop, dim3(G), dim3(CIT), args, smem, L.stream);
             if (L.counter) *L.counter += 2;
             return;
         }
     }
-    k_coarse_invert<<<1, CT, in_smem ? wbytes : 0, L.stream>>>(n, work, Ainv, in_smem);
+    k_coarse_invert<<<1, CT, in_smem ? wbytes : 0, L.stream>>>(n, work, Ainv, in_smem, bad);
     if (L.counter) *L.counter += 2;
 }
 

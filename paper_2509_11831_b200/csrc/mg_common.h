@@ -38,6 +38,8 @@ struct HostLevel {
     std::vector<int32_t> ctab;          // on a COARSE level: 9 * ntiles ids of the FINE tiles (2TJ-1..2TJ+1) x (2TI-1..2TI+1)
     std::vector<int32_t> ptab;          // on a FINE level: 9 * ntiles ids of the COARSE tiles (pTJ-1..pTJ+1) x (pTI-1..pTI+1), pT = floor(T/2)
     std::vector<uint8_t> tflag;         // per tile: bit 0 / 1 / 2 = all cells within 2 / 4 / 6 cells of the tile are inner points
+    std::vector<int32_t> tlist[2];      // tiles sorted into [interior | general] by flag bit 1 (k = 0: halo 4) and bit 2 (k = 1: halo 6)
+    int32_t nint[2] = {0, 0};           // number of interior tiles at the head of tlist[k]
     std::vector<int32_t> canon2slot;    // canonical (J, I) order -> slot
     int64_t n = 0, n_inner = 0;
     int64_t nslots() const { return (int64_t)(ntiles + 1) * TS; }

@@ -9,8 +9,18 @@
 namespace mgb {
 
 constexpr int MAX_M = 64;          // largest fGMRES restart length
-constexpr int RED_BLOCKS = 592;    // 4 x 148 SMs: blocks of the grid-wide reductions
+constexpr int RED_BLOCKS_MAX = 1024;   // capacity of the per-block partial sums of the grid-wide reductions
 constexpr int RED_THREADS = 256;
+
+// Per-device facts, queried once per device (mg_devinfo.cu).
+struct DevInfo {
+    int device;
+    int sms;     // cudaDevAttrMultiProcessorCount (148 on B200)
+    int coop;    // cooperative launch supported
+};
+const DevInfo& dev_info();                                       // of the calling thread's current device
+cudaError_t ensure_dyn_smem(const void* func, size_t bytes);     // opt-in dynamic shared memory, once per (kernel, device)
+inline int red_blocks() { const int b = 4 * dev_info().sms; return b < RED_BLOCKS_MAX ? b : RED_BLOCKS_MAX; }   // blocks of the grid-wide reductions
 
 // One multigrid level on the device (all pointers device memory; vectors have nslots entries).
 struct LevelDev {
@@ -25,6 +35,9 @@ struct LevelDev {
     const int32_t* ptab;     // 9 per tile (this level as the fine side): coarse tiles around the parent tile
     const int32_t* tij;      // 2 per tile: tile coordinates (TI, TJ)
     const uint8_t* tflag;    // per tile: bits 0 / 1 / 2 = every cell within 2 / 4 / 6 cells of the tile is an inner point
+    const int32_t* tlist[2]; // tile ids, [nint[k] interior tiles | the rest], by flag bit 1 (k = 0) / bit 2 (k = 1)
+    int32_t nint[2];
+    const int32_t* smeta[2]; // per interior tile of tlist[k], in list order: 24 ints {tnb[9], ptab[9], TI & 1, TJ & 1, tile id, pad} (mg_strip_gs.cuh)
     double* lam;
     double* c;
     double* rd;              // 1 / a_ll on inner points (rule D1), 0 elsewhere; derived at every update (U2)
@@ -141,7 +154,7 @@ cudaError_t launch_tail(const Launch& L, const LevelDev* d_levs, int s0, int nle
 
 // ---- coarsest level (mg_coarse.cu) ----
 void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
-                          double* work /* n x 2n */, double* Ainv /* n x n */);
+                          double* work /* n x 2n */, double* Ainv /* n x n */, int* bad /* bit 3 set on a zero / non-finite pivot */);
 void launch_coarse_solve(const Launch& L, const double* Ainv, const int32_t* cslot, int n, VecRef b_tiled, VecRef x_tiled);
 
 // ---- fGMRES vector kernels (mg_krylov.cu) ----

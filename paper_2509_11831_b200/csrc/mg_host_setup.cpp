@@ -127,6 +127,13 @@ void build_tile_tables(HostLevel& lv) {
             }
         lv.tflag[t] = (uint8_t)((reach >= 2 ? 1 : 0) | (reach >= 4 ? 2 : 0) | (reach >= 6 ? 4 : 0));
     }
+    // tile lists of the register-tiled smoother (interior tiles) and of the general tile code (the rest)
+    for (int k = 0; k < 2; k++) {
+        lv.tlist[k].clear();
+        for (int32_t t = 0; t < lv.ntiles; t++) if (lv.tflag[t] & (2 << k)) lv.tlist[k].push_back(t);
+        lv.nint[k] = (int32_t)lv.tlist[k].size();
+        for (int32_t t = 0; t < lv.ntiles; t++) if (!(lv.tflag[t] & (2 << k))) lv.tlist[k].push_back(t);
+    }
     // canonical order: ascending (J, I)
     lv.canon2slot.clear(); lv.canon2slot.reserve((size_t)lv.n);
     int32_t t0 = 0;

@@ -242,7 +242,7 @@ __global__ void k_scatter(const double* __restrict__ src, const int32_t* __restr
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[k] = src[slot[k]];
 }
 
-inline int grid1d(int64_t n) { return (int)std::min<int64_t>((n + 255) / 256, 148 * 8); }
+inline int grid1d(int64_t n) { return (int)std::min<int64_t>((n + 255) / 256, dev_info().sms * 8); }
 inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; }
 
 }  // namespace
@@ -260,11 +260,7 @@ void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coar
 }
 
 void launch_defect_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, VecRef x, VecRef b, double* d_coarse) {
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_defect_restrict, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DR_SMEM);
-        configured = true;
-    }
+    ensure_dyn_smem((const void*)k_defect_restrict, DR_SMEM);
     k_defect_restrict<<<coarse.ntiles, NT, DR_SMEM, L.stream>>>(fine, coarse, x, b, d_coarse, L.stop);
     count(L);
 }

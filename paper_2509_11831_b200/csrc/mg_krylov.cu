@@ -208,7 +208,7 @@ __global__ void k_givens(GmresState* st) {
 constexpr int FUSED_NV = 32;
 constexpr double REORTH_TOL = 1e-13;   // second update skipped when ||V^T w'|| <= REORTH_TOL ||w'|| (G23)
 constexpr int UD_THREADS = 128;
-constexpr int UD_BLOCKS = 148 * 2;   // 254 registers x 128 threads: two blocks per SM, one wave
+// register-staged variant: 254 registers x 128 threads, two blocks per SM, one wave
 
 // One grid-stride sweep with NV basis values x EPT elements held in registers per thread.
 template <int NV, int EPT>
@@ -591,48 +591,42 @@ inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; 
 }  // namespace
 
 void launch_norm2(const Launch& L, const double* v, int64_t n, GmresState* st, double* partial, int which) {
-    k_norm2<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(v, n, st, partial, which); count(L);
+    k_norm2<<<red_blocks(), RED_THREADS, 0, L.stream>>>(v, n, st, partial, which); count(L);
 }
 void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double* V0, int64_t n) {
-    k_start_cycle<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
+    k_start_cycle<<<red_blocks(), RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
 }
 void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int m) {
     static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
-    static bool configured = false;
-    if (!no_tma && !configured) {
-        cudaFuncSetAttribute(k_multidot_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UDT_SMEM);
-        configured = true;
-    }
+    if (!no_tma) ensure_dyn_smem((const void*)k_multidot_tma, UDT_SMEM);
+    const int sms = dev_info().sms;
     if (m <= FUSED_NV && !no_tma && n % (UDT_THREADS * 4) == 0)
-        k_multidot_tma<<<148, UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
-    else if (m <= FUSED_NV) k_multidot_t<<<148 * 2, MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
-    else k_multidot<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+        k_multidot_tma<<<sms, UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
+    else if (m <= FUSED_NV) k_multidot_t<<<sms * 2, MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    else k_multidot<<<red_blocks(), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
 }
 void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass) {
-    k_update_w<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
+    k_update_w<<<red_blocks(), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
 }
 void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial) {
     static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
-    static bool configured = false;
-    if (!no_tma && !configured) {
-        cudaFuncSetAttribute(k_update_dot_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UDT_SMEM);
-        configured = true;
-    }
-    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<148, UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
-    else k_update_dot<<<UD_BLOCKS, UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    if (!no_tma) ensure_dyn_smem((const void*)k_update_dot_tma, UDT_SMEM);
+    const int sms = dev_info().sms;
+    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<sms, UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
+    else k_update_dot<<<sms * 2, UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
 }
 void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
-    k_final_v<<<148 * 2, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
-    k_scale_v<<<148 * 8, SV_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_final_v<<<dev_info().sms * 2, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_scale_v<<<dev_info().sms * 8, SV_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
 }
 void launch_givens(const Launch& L, GmresState* st) { k_givens<<<1, 32, 0, L.stream>>>(st); count(L); }
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
-    k_next_v<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_next_v<<<red_blocks(), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
 }
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st) {
-    k_update_x<<<RED_BLOCKS, 256, 0, L.stream>>>(x, Z, stride, n, st); count(L);
+    k_update_x<<<red_blocks(), 256, 0, L.stream>>>(x, Z, stride, n, st); count(L);
 }
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol, bool full_cgs2) {
     static const char* env = getenv("MG_B200_REORTH_TOL");          // experiments only

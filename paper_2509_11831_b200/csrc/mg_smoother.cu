@@ -1,8 +1,9 @@
 // Kernels and launchers of the smoother; the tile-level device code is in mg_tile_gs.cuh (shared with the
 // fused small-level kernel of mg_tail.cu).
+#include <algorithm>
 #include <cstdlib>
 
-#include "mg_tile_gs.cuh"
+#include "mg_strip_gs.cuh"
 
 namespace mgb {
 
@@ -15,11 +16,12 @@ namespace {
 template <int NS, bool PC, int EPI, int BX, int BY, int XIM>
 __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef xout_r, VecRef b_r, const double* __restrict__ ec,
                                               int xin_zero, const uint16_t* __restrict__ ccode, double* __restrict__ dc,
-                                              const int* __restrict__ stop) {
+                                              const int* __restrict__ stop, const int* __restrict__ tlist) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (stop != nullptr && *stop) return;
     constexpr int NBX = TX / BX, NSUB = NBX * (TY / BY);
-    const int t = blockIdx.x / NSUB, sub = blockIdx.x - t * NSUB;
+    const int ti = blockIdx.x / NSUB, sub = blockIdx.x - ti * NSUB;
+    const int t = tlist != nullptr ? tlist[ti] : ti;            // the launch covers a list of tiles, or all of them
     gs_tile<NS, PC, false, EPI, BX, BY, XIM>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
                                        (sub % NBX) * BX, (sub / NBX) * BY);
 }
@@ -32,21 +34,36 @@ __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
 
 // Levels of at most SUB_MAX_TILES tiles are latency bound (7-25 us per launch whatever the tile count,
 // profiles/r01c_small_levels.md): they run with one CTA per SBX x SBY block, 8 CTAs per tile.
-constexpr int SUB_MAX_TILES = 40, SBX = 16, SBY = 16;      // 8 CTAs per tile
-constexpr int MID_MAX_TILES = 74, MBX = 32, MBY = 16;      // 4 CTAs per tile: at most 296 CTAs = one wave at 2 CTAs per SM
-constexpr int HALF_MAX_TILES = 148, HBX = 64, HBY = 16;    // 2 CTAs per tile: one wave up to 148 tiles
+constexpr int SBX = 16, SBY = 16;      // 8 CTAs per tile: levels of at most 40 tiles on 148 SMs (sms * 10 / 37)
+constexpr int MBX = 32, MBY = 16;      // 4 CTAs per tile: at most one wave at 2 CTAs per SM (tiles <= sms / 2)
+constexpr int HBX = 64, HBY = 16;      // 2 CTAs per tile: one wave up to `sms` tiles
+
+inline bool no_strips() { static const bool v = getenv("MG_B200_NO_STRIPS") != nullptr; return v; }
 
 template <int NS, bool PC, int EPI, int BX, int BY, int XIM>
 void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
                   const uint16_t* ccode, double* dc) {
     constexpr size_t smem = Geo<NS, PC, EPI, BX, BY>::SMEM;
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_gs<NS, PC, EPI, BX, BY, XIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = true;
+    ensure_dyn_smem((const void*)k_gs<NS, PC, EPI, BX, BY, XIM>, smem);
+    if (NS == 2 && XIM == 0 && BX == TX && BY == TY && !no_strips()) {
+        // large level, two-field form: interior tiles by the register-tiled kernel, the rest by the general tile code
+        constexpr int K = EPI ? 1 : 0, SH = EPI ? 6 : 4;
+        using SG = SGeo<SH>;
+        const int nint = lv.nint[K], ngen = lv.ntiles - nint;
+        if (ngen > 0) {
+            k_gs<NS, PC, EPI, BX, BY, XIM><<<ngen, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, lv.tlist[K] + nint);
+            if (L.counter) *L.counter += 1;
+        }
+        if (nint > 0) {
+            constexpr size_t ssm = SG::smem(4 + (EPI ? 1 : 0), PC);
+            ensure_dyn_smem((const void*)k_gs_strip<SH, PC, EPI>, ssm);
+            k_gs_strip<SH, PC, EPI><<<std::min(nint, dev_info().sms), SG::NT, ssm, L.stream>>>(lv, lv.smeta[K], nint, xin, xout, b, ec, zero ? 1 : 0, dc, L.stop);
+            if (L.counter) *L.counter += 1;
+        }
+        return;
     }
     const int grid = lv.ntiles * (TX / BX) * (TY / BY);
-    k_gs<NS, PC, EPI, BX, BY, XIM><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
+    k_gs<NS, PC, EPI, BX, BY, XIM><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, nullptr);
     if (L.counter) *L.counter += 1;
 }
 
@@ -62,6 +79,8 @@ template <int NS, bool PC, int EPI = 0>
 void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, VecRef b, const double* ec, bool zero,
                const uint16_t* ccode = nullptr, double* dc = nullptr) {
     static const bool no_sub = getenv("MG_B200_NO_SUBBLOCKS") != nullptr;
+    const int sms = dev_info().sms;
+    const int SUB_MAX_TILES = sms * 10 / 37, MID_MAX_TILES = sms / 2, HALF_MAX_TILES = sms;
     if (lv.ntiles <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else if (lv.ntiles <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else if (lv.ntiles <= HALF_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, HBX, HBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
@@ -98,7 +117,7 @@ void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coar
 }
 
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n) {
-    k_copy<<<(int)std::min<int64_t>((n + 255) / 256, 148 * 8), 256, 0, L.stream>>>(src, dst, n);
+    k_copy<<<(int)std::min<int64_t>((n + 255) / 256, dev_info().sms * 8), 256, 0, L.stream>>>(src, dst, n);
     if (L.counter) *L.counter += 1;
 }
 

@@ -1,0 +1,306 @@
+// S2 (+S3, S4, S1) on INTERIOR tiles of the large levels, register-tiled: the same two fused red-black Gauss-Seidel
+// sweeps (gauss_seidel_rbb; every cell of an interior tile's region is an inner point, so the boundary
+// loop is empty), optionally preceded by the coarse-grid correction x <- x - P e_c and followed by the
+// restricted defect or by w = A x, as gs_fast of mg_tile_gs.cuh — same arithmetic in the same
+// order, so both kernels produce the same bits — but organised around registers instead of shared memory:
+//
+//   * a thread owns a STRIP: one column pair (2p, 2p+1) x R consecutive rows of the region (tile + halo H).  In every
+//     row of a pair exactly one cell is red and one is black, at positions fixed at compile time, so the colour
+//     phases are straight-line code over registers: x, b, 1/a_ll and the face sums (c_l + c_nb) of the strip stay in
+//     registers for the whole kernel (the face sums are sweep-invariant: computed once), the N/S neighbours and one
+//     of the W/E neighbours of every cell are the thread's own registers;
+//   * shared memory only carries what crosses a strip boundary: every updated value is also published to a
+//     colour-split mirror of x (the layout of mg_tile_gs.cuh), from which a thread reads the ONE cross-lane W/E
+//     neighbour of each cell and the rows just above / below its strip.  Per cell update: 1 LDS.64 + 1 STS.64 (+ 2 LDS
+//     per strip and phase) against 9 LDS.64 + 1 STS.64 in gs_fast;
+//   * a warp of "main" strips covers exactly the 32 column pairs of the tile, one warp per block of R rows, so its
+//     global loads and stores are whole 512-byte tile rows (LDG.128 / STG.128).  The H halo column pairs of the row
+//     blocks are packed into a few extra warps (32 / H row blocks per warp);
+//   * no predication: every strip runs every phase; values within p cells of the region edge are wrong after phase p
+//     and never reach the tile (halo H >= 2 NS), as in any temporally blocked sweep;
+//   * the CTA is persistent (one per SM: the register file holds one region) and walks a list of interior tiles.
+//     Loads are decoupled from the arithmetic by asynchronous copies (cp.async, SASS LDGSTS): while tile i is swept in
+//     registers, every thread's strip of tile i + 1 (x, c, b, 1/a_ll, lambda, coarse parents) streams from HBM into
+//     that thread's PRIVATE staging slots in shared memory — private, so no barrier guards the staging buffer and one
+//     buffer suffices: a thread refills its slots right after it has moved them into registers.  The per-tile tables
+//     (neighbour tiles, parent tiles) come from a packed per-list array two tiles ahead.
+#pragma once
+#include "mg_tile_gs.cuh"
+
+namespace mgb {
+namespace {
+
+template <int H>
+struct SGeo {
+    static_assert(H % 2 == 0 && 32 % 1 == 0, "halo must be even: column pairs may not straddle tiles");
+    static constexpr int R = 4;                          // rows per strip
+    static constexpr int RW = TX + 2 * H, RH = TY + 2 * H, RWC = RW / 2;
+    static_assert(RH % R == 0, "region height must be a multiple of the strip height");
+    static constexpr int NRB = RH / R;                   // row blocks = main warps
+    static constexpr int RBL = 32 / H;                   // row blocks of halo pairs per extra warp
+    static constexpr int NLW = (NRB + RBL - 1) / RBL;    // extra warps
+    static constexpr int NW = NRB + NLW, NT = 32 * NW;
+    static constexpr int NCP = (RH + 2) * RWC;           // cells per colour, one padding row below and above the region
+    static constexpr size_t MIRROR = (size_t)4 * NCP * sizeof(double);   // mirrors of x and c (c: later d / w scratch)
+    // + staging: NA arrays x R rows x NT threads of 16-byte pairs, (PC) 6 coarse values per thread, 3 tile-table buffers
+    static constexpr size_t smem(int na, bool pc) { return MIRROR + (size_t)na * R * NT * 16 + (pc ? (size_t)6 * NT * 8 : 0) + 3 * 24 * 4; }
+};
+constexpr int SMETA = 24;   // ints per list entry of LevelDev::smeta: tn[9], pt[9], odd[2], tile id, padding
+
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// x_out = S^2 (x_in - [PC] P e_c) on the nlist interior tiles described by smeta; EPI as in k_gs (1: d_c = R (A x_out - b), 2: w = A x_out).
+template <int H, bool PC, int EPI>
+__global__ void __launch_bounds__(SGeo<H>::NT, 1) k_gs_strip(LevelDev lv, const int* __restrict__ smeta, int nlist, VecRef xin_r, VecRef xout_r,
+                                                             VecRef b_r, const double* __restrict__ ec, int xin_zero,
+                                                             double* __restrict__ dc, const int* __restrict__ stop) {
+    using G = SGeo<H>;
+    constexpr int R = G::R, RWC = G::RWC, NCP = G::NCP, NRB = G::NRB, RBL = G::RBL, NT = G::NT;
+    constexpr bool DR = EPI == 1, AP = EPI == 2;
+    constexpr int NA = 4 + (EPI ? 1 : 0);                   // staged arrays: c, b, 1/a_ll, x, (lambda)
+    static_assert(H >= 4 + (DR ? 2 : (AP ? 1 : 0)), "halo too small for two sweeps and the epilogue");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (stop != nullptr && *stop) return;
+    double* sx = reinterpret_cast<double*>(smem_raw);       // [2][RH + 2][RWC] colour-split mirror of x
+    double* sc = sx + 2 * NCP;                              // same for c; dead after the face sums: scratch of the epilogues
+    double2* stg = reinterpret_cast<double2*>(sc + 2 * NCP);   // [NA][R][NT] private staging slots
+    double* se = reinterpret_cast<double*>(stg + NA * R * NT); // (PC) [6][NT] coarse parents
+    int* M = reinterpret_cast<int*>(se + (PC ? 6 * NT : 0));   // [3][SMETA] tile tables of tiles i, i + 1, i + 2
+    const double* __restrict__ xin = resolve(xin_r);
+    double* __restrict__ xout = resolve(xout_r);
+    const double* __restrict__ b = resolve(b_r);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // ---- the strip of this thread: pair column p, rows ry0 .. ry0 + R - 1 of the region
+    int p, rb;
+    const bool main_w = warp < NRB;
+    if (main_w) { p = H / 2 + lane; rb = warp; }
+    else {
+        int g = lane / H, k = lane - g * H;
+        rb = (warp - NRB) * RBL + g;
+        if (g >= RBL || rb >= NRB) { g = 0; k = 0; rb = (warp - NRB) * RBL; }   // spare lanes duplicate the warp's first strip
+        p = (k < H / 2) ? k : 32 + k;
+    }
+    const int ry0 = rb * R;
+    const int lx0 = 2 * p - H;                              // tile-relative column of the pair's first cell (even)
+    const int ox = (lx0 < 0) ? -1 : (lx0 >= TX ? 1 : 0);
+    const int lxm = lx0 - ox * TX;
+    // colour-split index of cell (pos, row r) of the strip: colour (r + pos) & 1 (ry0, 2p even), row ry0 + r + 1 (padding), column p
+    const int sbase = (ry0 + 1) * RWC + p;
+#define SIDX(pos, r) ((((r) + (pos)) & 1) * NCP + sbase + (r) * RWC)
+    const double kappa = lv.kappa;
+    const int G0 = gridDim.x;
+
+    // asynchronous copies of this thread's strip of the tile described by m[] into its staging slots
+    auto prefetch = [&](const int* m) {
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const int ly = ry0 + r - H;
+            const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
+            const int64_t gs = (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm;
+            cp_async16(&stg[(0 * R + r) * NT + tid], lv.c + gs);
+            cp_async16(&stg[(1 * R + r) * NT + tid], b + gs);
+            cp_async16(&stg[(2 * R + r) * NT + tid], lv.rd + gs);
+            if (!xin_zero) cp_async16(&stg[(3 * R + r) * NT + tid], xin + gs);
+            if (EPI) cp_async16(&stg[(4 * R + r) * NT + tid], lv.lam + gs);
+        }
+        if (PC) {
+            // coarse parents of the strip (bilinear prolongation): columns cx, cx + 1, rows cy0 .. cy0 + 2
+            const int cx = m[18] * (TX / 2) + (lx0 >> 1), cy0 = m[19] * (TY / 2) + ((ry0 - H) >> 1);
+#pragma unroll
+            for (int q = 0; q < 3; q++) {
+                cp_async8(&se[(2 * q) * NT + tid], ec + parent_slot9(m + 9, cx, cy0 + q));
+                cp_async8(&se[(2 * q + 1) * NT + tid], ec + parent_slot9(m + 9, cx + 1, cy0 + q));
+            }
+        }
+        cp_async_commit();
+    };
+
+    if (tid < SMETA) {
+        M[tid] = smeta[(int64_t)blockIdx.x * SMETA + tid];
+        if ((int)blockIdx.x + G0 < nlist) M[SMETA + tid] = smeta[(int64_t)(blockIdx.x + G0) * SMETA + tid];
+    }
+    __syncthreads();
+    prefetch(M);
+    int ib = 0;                                             // buffer of the current tile's tables
+    for (int it = blockIdx.x; it < nlist; it += G0) {
+        const int* m = M + ib * SMETA;
+        const int* pt = m + 9;
+        const int* odd = m + 18;
+        const int t = m[20];
+        const bool more2 = it + 2 * G0 < nlist;
+        int mnext = 0;
+        if (tid < SMETA && more2) mnext = __ldg(smeta + (int64_t)(it + 2 * G0) * SMETA + tid);    // tables two tiles ahead
+        // ---- the strip: staging slots -> registers (pairs)
+        cp_async_wait_all();
+        double x[R][2], c[R][2], br[R][2], rd[R][2];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const double2 cv = stg[(0 * R + r) * NT + tid], bv = stg[(1 * R + r) * NT + tid], dv = stg[(2 * R + r) * NT + tid];
+            c[r][0] = cv.x; c[r][1] = cv.y; br[r][0] = bv.x; br[r][1] = bv.y; rd[r][0] = dv.x; rd[r][1] = dv.y;
+            if (xin_zero) { x[r][0] = 0.0; x[r][1] = 0.0; }
+            else { const double2 xv = stg[(3 * R + r) * NT + tid]; x[r][0] = xv.x; x[r][1] = xv.y; }
+        }
+        double lam[R][2];
+        if (EPI) {
+#pragma unroll
+            for (int r = 0; r < R; r++) { const double2 lv2 = stg[(4 * R + r) * NT + tid]; lam[r][0] = lv2.x; lam[r][1] = lv2.y; }
+        }
+        double e[3][2];
+        if (PC) {
+#pragma unroll
+            for (int q = 0; q < 3; q++) { e[q][0] = se[(2 * q) * NT + tid]; e[q][1] = se[(2 * q + 1) * NT + tid]; }
+        }
+        // the slots are consumed: refill them with the next tile of this CTA while this one is computed
+        if (it + G0 < nlist) prefetch(M + (ib == 2 ? 0 : ib + 1) * SMETA);
+        if (PC) {
+            // x <- x - P e_c (bilinear): weights 1 / (1/2, 1/2) / (1/4 x 4) over the parents
+            // (cx, cy), (cx+1, cy), (cx, cy+1), (cx+1, cy+1); rows r = 0..3 of the strip use coarse rows cy0 .. cy0 + 2
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int q = r >> 1;
+                if ((r & 1) == 0) {
+                    x[r][0] -= e[q][0];
+                    x[r][1] -= 0.5 * e[q][0] + 0.5 * e[q][1];
+                } else {
+                    x[r][0] -= 0.5 * e[q][0] + 0.5 * e[q + 1][0];
+                    x[r][1] -= 0.25 * e[q][0] + 0.25 * e[q][1] + 0.25 * e[q + 1][0] + 0.25 * e[q + 1][1];
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            sx[SIDX(0, r)] = x[r][0]; sx[SIDX(1, r)] = x[r][1];
+            sc[SIDX(0, r)] = c[r][0]; sc[SIDX(1, r)] = c[r][1];
+        }
+        __syncthreads();
+        // ---- face sums c_l + c_nb (sweep-invariant): hW | cell 0 | hM | cell 1 | hE per row, v[r] below row r per column
+        double hW[R], hM[R], hE[R], v[R + 1][2];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            hW[r] = c[r][0] + sc[SIDX(1, r) - 1];            // W of cell 0: cell 1 of pair p - 1 (other colour, same row)
+            hM[r] = c[r][0] + c[r][1];
+            hE[r] = c[r][1] + sc[SIDX(0, r) + 1];            // E of cell 1: cell 0 of pair p + 1
+        }
+#pragma unroll
+        for (int q = 0; q < 2; q++) {
+            v[0][q] = c[0][q] + sc[SIDX(q, -1)];
+#pragma unroll
+            for (int r = 1; r < R; r++) v[r][q] = c[r][q] + c[r - 1][q];
+            v[R][q] = c[R - 1][q] + sc[SIDX(q, R)];
+        }
+        // ---- two sweeps: red (colour 0), black (colour 1); the cell of colour col in row r is at position (r + col) & 1
+#pragma unroll
+        for (int ph = 0; ph < 4; ph++) {
+            const int col = ph & 1;
+            const double xs = sx[SIDX(col, -1)];             // S neighbour of the updated cell of row 0 (position col)
+            const double xn = sx[SIDX(1 - col, R)];          // N neighbour of the updated cell of row R - 1 (R even: position 1 - col)
+            double xc[R];                                    // the cross-lane W / E neighbours
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int pos = (r + col) & 1;
+                xc[r] = pos == 0 ? sx[SIDX(1, r) - 1] : sx[SIDX(0, r) + 1];
+            }
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int pos = (r + col) & 1;
+                const double xW = pos == 0 ? xc[r] : x[r][0], xE = pos == 0 ? x[r][1] : xc[r];
+                const double aW = pos == 0 ? hW[r] : hM[r], aE = pos == 0 ? hM[r] : hE[r];
+                const double xS = r == 0 ? xs : x[r - 1][pos], xN = r == R - 1 ? xn : x[r + 1][pos];
+                double acc = aW * xW;
+                acc = fma(aE, xE, acc);
+                acc = fma(v[r][pos], xS, acc);
+                acc = fma(v[r + 1][pos], xN, acc);
+                x[r][pos] = fma(kappa, acc, br[r][pos]) * rd[r][pos];
+            }
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int pos = (r + col) & 1;
+                sx[SIDX(pos, r)] = x[r][pos];
+            }
+            __syncthreads();
+        }
+        // ---- write the tile rows of the main strips
+        if (main_w) {
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int ly = ry0 + r - H;
+                if (ly >= 0 && ly < TY)
+                    *reinterpret_cast<double2*>(xout + (int64_t)t * TS + ly * TX + 2 * lane) = make_double2(x[r][0], x[r][1]);
+            }
+        }
+        if (DR) {
+            // d = A x - b (difference form of rule D1) on the RED cells of the tile and of the one-cell ring around it: the
+            // black cells were updated last from the current red values, their defect is zero up to rounding
+            const double xs = sx[SIDX(0, -1)], xn = sx[SIDX(1, R)];
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int pos = r & 1, ry = ry0 + r, rx = 2 * p + pos;
+                double d = 0.0;
+                if (min(min(rx, G::RW - 1 - rx), min(ry, G::RH - 1 - ry)) >= H - 1) {
+                    const double xl = x[r][pos];
+                    const double xW = pos == 0 ? sx[SIDX(1, r) - 1] : x[r][0], xE = pos == 0 ? x[r][1] : sx[SIDX(0, r) + 1];
+                    const double xS = r == 0 ? xs : x[r - 1][pos], xN = r == R - 1 ? xn : x[r + 1][pos];
+                    const double aW = kappa * (pos == 0 ? hW[r] : hM[r]), aE = kappa * (pos == 0 ? hM[r] : hE[r]);
+                    const double aS = kappa * v[r][pos], aN = kappa * v[r + 1][pos];
+                    d = lam[r][pos] * xl + aW * (xl - xW) + aE * (xl - xE) + aS * (xl - xS) + aN * (xl - xN) - br[r][pos];
+                }
+                sc[SIDX(pos, r)] = d;
+            }
+            __syncthreads();
+            // the 32 x 16 coarse points under the tile gather their full-weighting stencils (rule T2; only the red
+            // entries are non-zero): coarse point under fine cell 0 of pair p in an even row
+            const int ptile = pt[4];
+            if (main_w && ptile != lv.ntiles_coarse) {
+#pragma unroll
+                for (int r = 0; r < R; r += 2) {
+                    const int ly = ry0 + r - H;
+                    if (ly >= 0 && ly < TY) {
+                        const int i0 = SIDX(0, r);               // red cell (2p, ry); diagonal reds: cells 1 of pairs p - 1, p in rows ry -+ 1
+                        double acc = 0.0;
+                        acc += 0.0625 * sc[i0 - RWC - 1];
+                        acc += 0.0625 * sc[i0 - RWC];
+                        acc += 0.25 * sc[i0];
+                        acc += 0.0625 * sc[i0 + RWC - 1];
+                        acc += 0.0625 * sc[i0 + RWC];
+                        dc[(int64_t)ptile * TS + (odd[1] * (TY / 2) + (ly >> 1)) * TX + odd[0] * (TX / 2) + lane] = acc;
+                    }
+                }
+            }
+        }
+        if (AP) {
+            // w = A x_out on the tile (rule D1, difference form), both colours
+            if (main_w) {
+                const double xs0 = sx[SIDX(0, -1)], xs1 = sx[SIDX(1, -1)], xn0 = sx[SIDX(0, R)], xn1 = sx[SIDX(1, R)];
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    const int ly = ry0 + r - H;
+                    if (ly >= 0 && ly < TY) {
+                        const double x0 = x[r][0], x1 = x[r][1];
+                        const double xW = sx[SIDX(1, r) - 1], xE = sx[SIDX(0, r) + 1];
+                        const double s0 = r == 0 ? xs0 : x[r - 1][0], n0 = r == R - 1 ? xn0 : x[r + 1][0];
+                        const double s1 = r == 0 ? xs1 : x[r - 1][1], n1 = r == R - 1 ? xn1 : x[r + 1][1];
+                        const double w0 = lam[r][0] * x0 + (kappa * hW[r]) * (x0 - xW) + (kappa * hM[r]) * (x0 - x1) + (kappa * v[r][0]) * (x0 - s0) +
+                                          (kappa * v[r + 1][0]) * (x0 - n0);
+                        const double w1 = lam[r][1] * x1 + (kappa * hM[r]) * (x1 - x0) + (kappa * hE[r]) * (x1 - xE) + (kappa * v[r][1]) * (x1 - s1) +
+                                          (kappa * v[r + 1][1]) * (x1 - n1);
+                        *reinterpret_cast<double2*>(dc + (int64_t)t * TS + ly * TX + 2 * lane) = make_double2(w0, w1);
+                    }
+                }
+            }
+        }
+        if (tid < SMETA && more2) M[(ib == 0 ? 2 : ib - 1) * SMETA + tid] = mnext;   // buffer of tile i - 1 = buffer of tile i + 2
+        ib = ib == 2 ? 0 : ib + 1;
+        __syncthreads();                                    // the mirrors are free, the tables of tile i + 2 are visible
+    }
+#undef SIDX
+}
+
+}  // namespace
+}  // namespace mgb

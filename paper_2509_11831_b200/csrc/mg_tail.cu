@@ -131,16 +131,12 @@ size_t tail_smem() {
 }  // namespace
 
 int tail_max_grid() {
-    static int cached = -1;
-    if (cached >= 0) return cached;
+    // per device: the caller (mg_setup) stores the result in the handle
     const size_t smem = tail_smem();
-    if (cudaFuncSetAttribute(k_tail, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return cached = 0; }
-    int per_sm = 0, dev = 0, sms = 0, coop = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tail, GT, smem) != cudaSuccess) { cudaGetLastError(); return cached = 0; }
-    return cached = per_sm * sms;
+    if (ensure_dyn_smem((const void*)k_tail, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int per_sm = 0;
+    if (!dev_info().coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tail, GT, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return per_sm * dev_info().sms;
 }
 
 cudaError_t launch_tail(const Launch& L, const LevelDev* d_levs, int s0, int nlev, const TailProgram& prog, const TailCoarse& cs,

@@ -35,6 +35,13 @@ def test_error_codes_without_device():
     # compute calls on a host-only handle fail loudly (no CPU fallback)
     assert L.mg_update_coeffs(s._h, C.c_void_p(8), C.c_void_p(8), None) == -5
     assert L.mg_apply(s._h, 0, C.c_void_p(8), C.c_void_p(8), None) == -5
+    # ... including the solve and the host-buffer entry points (MG_ECUDA, not an allocation failure)
+    buf = np.zeros(pl.n)
+    p = C.c_void_p(buf.ctypes.data)
+    assert L.mg_solve(s._h, p, p, p, C.c_double(1e-10), None, None, None) == -5
+    assert L.mg_solve_host(s._h, p, p, p, C.c_double(1e-10), None, None, None) == -5
+    assert L.mg_update_coeffs_host(s._h, p, p, None) == -5
+    assert L.mg_update_coeffs3_host(s._h, p, p, p, None) == -5
     # diagnostics before the first solve; option range (gamma 0..3, flag bits 0..2)
     assert s.last_reorth == -1 and len(s.last_history()[0]) == 0
     assert L.mg_last_history(None, None, None, 4) == -1 and L.mg_last_reorth(None) == -1
