@@ -361,8 +361,9 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         TRY(upload(h, &b.canon2slot, hl.canon2slot, s));
         for (int k = 0; k < 2; k++) {
             TRY(upload(h, &b.tlist[k], hl.tlist[k], s));
-            std::vector<int32_t> meta((size_t)24 * hl.nint[k], 0);           // tables of the interior tiles, packed in list order
-            for (int32_t q = 0; q < hl.nint[k]; q++) {
+            const int32_t nmeta = hl.nint[k] + hl.ngen[k];
+            std::vector<int32_t> meta((size_t)24 * nmeta, 0);                // tables of the interior and general tiles, packed in list order
+            for (int32_t q = 0; q < nmeta; q++) {
                 const int32_t t = hl.tlist[k][q];
                 for (int e = 0; e < 9; e++) { meta[24 * (size_t)q + e] = hl.tnb[9 * (size_t)t + e]; meta[24 * (size_t)q + 9 + e] = hl.ptab.empty() ? 0 : hl.ptab[9 * (size_t)t + e]; }
                 meta[24 * (size_t)q + 18] = hl.tI[t] & 1; meta[24 * (size_t)q + 19] = hl.tJ[t] & 1; meta[24 * (size_t)q + 20] = t;
@@ -386,7 +387,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         d.h = hl.h; d.kappa = 1.0 / (2.0 * hl.h * hl.h);
         d.code = b.code; d.tnb = b.tnb; d.ctab = b.ctab; d.ptab = b.ptab; d.tij = b.tij; d.lam = b.lam; d.c = b.c; d.rd = b.rd; d.tflag = b.tflag;
         d.xi = nullptr;
-        for (int k = 0; k < 2; k++) { d.tlist[k] = b.tlist[k]; d.nint[k] = hl.nint[k]; d.smeta[k] = b.smeta[k]; }
+        for (int k = 0; k < 2; k++) { d.tlist[k] = b.tlist[k]; d.nint[k] = hl.nint[k]; d.ngen[k] = hl.ngen[k]; d.smeta[k] = b.smeta[k]; }
     }
     TRY(dev_alloc(h, (void**)&h->d_lev, sizeof(LevelDev) * h->L, s));
     CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));

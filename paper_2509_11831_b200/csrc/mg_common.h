@@ -17,6 +17,7 @@ namespace mgb {
 constexpr int TX = 64;
 constexpr int TY = 32;
 constexpr int TS = TX * TY;
+constexpr int GUARD_CAP = 512;   // capacity of the per-CTA guard list of the smoother kernels
 
 // Per-slot 16-bit code.
 //  bits 0-1 : 0 absent, 1 inner, 2 Dirichlet guard, 3 Neumann guard
@@ -38,8 +39,10 @@ struct HostLevel {
     std::vector<int32_t> ctab;          // on a COARSE level: 9 * ntiles ids of the FINE tiles (2TJ-1..2TJ+1) x (2TI-1..2TI+1)
     std::vector<int32_t> ptab;          // on a FINE level: 9 * ntiles ids of the COARSE tiles (pTJ-1..pTJ+1) x (pTI-1..pTI+1), pT = floor(T/2)
     std::vector<uint8_t> tflag;         // per tile: bit 0 / 1 / 2 = all cells within 2 / 4 / 6 cells of the tile are inner points
-    std::vector<int32_t> tlist[2];      // tiles sorted into [interior | general] by flag bit 1 (k = 0: halo 4) and bit 2 (k = 1: halo 6)
-    int32_t nint[2] = {0, 0};           // number of interior tiles at the head of tlist[k]
+    // tiles sorted into [interior | general | overflow]: interior by flag bit 1 (k = 0: halo 4) / bit 2 (k = 1: halo 6);
+    // overflow = more than GUARD_CAP guard points within 8 cells of the tile (they stay on the shared-memory tile code)
+    std::vector<int32_t> tlist[2];
+    int32_t nint[2] = {0, 0}, ngen[2] = {0, 0};
     std::vector<int32_t> canon2slot;    // canonical (J, I) order -> slot
     int64_t n = 0, n_inner = 0;
     int64_t nslots() const { return (int64_t)(ntiles + 1) * TS; }

@@ -35,9 +35,9 @@ struct LevelDev {
     const int32_t* ptab;     // 9 per tile (this level as the fine side): coarse tiles around the parent tile
     const int32_t* tij;      // 2 per tile: tile coordinates (TI, TJ)
     const uint8_t* tflag;    // per tile: bits 0 / 1 / 2 = every cell within 2 / 4 / 6 cells of the tile is an inner point
-    const int32_t* tlist[2]; // tile ids, [nint[k] interior tiles | the rest], by flag bit 1 (k = 0) / bit 2 (k = 1)
-    int32_t nint[2];
-    const int32_t* smeta[2]; // per interior tile of tlist[k], in list order: 24 ints {tnb[9], ptab[9], TI & 1, TJ & 1, tile id, pad} (mg_strip_gs.cuh)
+    const int32_t* tlist[2]; // tile ids, [nint[k] interior | ngen[k] general | overflow tiles], by flag bit 1 (k = 0) / bit 2 (k = 1)
+    int32_t nint[2], ngen[2];
+    const int32_t* smeta[2]; // per interior and general tile of tlist[k], in list order: 24 ints {tnb[9], ptab[9], TI & 1, TJ & 1, tile id, pad} (mg_strip_gs.cuh)
     double* lam;
     double* c;
     double* rd;              // 1 / a_ll on inner points (rule D1), 0 elsewhere; derived at every update (U2)

@@ -127,12 +127,27 @@ void build_tile_tables(HostLevel& lv) {
             }
         lv.tflag[t] = (uint8_t)((reach >= 2 ? 1 : 0) | (reach >= 4 ? 2 : 0) | (reach >= 6 ? 4 : 0));
     }
-    // tile lists of the register-tiled smoother (interior tiles) and of the general tile code (the rest)
+    // tile lists of the register-tiled smoother: interior tiles, general tiles, and tiles with more guards in reach
+    // than the smoother's guard list holds
+    std::vector<uint8_t> ovf((size_t)lv.ntiles, 0);
+    for (int32_t t = 0; t < lv.ntiles; t++) {
+        if (lv.tflag[t] & 4) continue;
+        int ng = 0;
+        for (int ly = -8; ly < TY + 8; ly++)
+            for (int lx = -8; lx < TX + 8; lx++) {
+                const int ox = lx < 0 ? -1 : (lx >= TX ? 1 : 0), oy = ly < 0 ? -1 : (ly >= TY ? 1 : 0);
+                const int32_t q = lv.tnb[(size_t)9 * t + (oy + 1) * 3 + (ox + 1)];
+                ng += code_kind(lv.code[(size_t)q * TS + (ly - oy * TY) * TX + (lx - ox * TX)]) >= C_DIR;
+            }
+        ovf[t] = ng > GUARD_CAP;
+    }
     for (int k = 0; k < 2; k++) {
         lv.tlist[k].clear();
         for (int32_t t = 0; t < lv.ntiles; t++) if (lv.tflag[t] & (2 << k)) lv.tlist[k].push_back(t);
         lv.nint[k] = (int32_t)lv.tlist[k].size();
-        for (int32_t t = 0; t < lv.ntiles; t++) if (!(lv.tflag[t] & (2 << k))) lv.tlist[k].push_back(t);
+        for (int32_t t = 0; t < lv.ntiles; t++) if (!(lv.tflag[t] & (2 << k)) && !ovf[t]) lv.tlist[k].push_back(t);
+        lv.ngen[k] = (int32_t)lv.tlist[k].size() - lv.nint[k];
+        for (int32_t t = 0; t < lv.ntiles; t++) if (!(lv.tflag[t] & (2 << k)) && ovf[t]) lv.tlist[k].push_back(t);
     }
     // canonical order: ascending (J, I)
     lv.canon2slot.clear(); lv.canon2slot.reserve((size_t)lv.n);

@@ -38,6 +38,7 @@ constexpr int SBX = 16, SBY = 16;      // 8 CTAs per tile: levels of at most 40 
 constexpr int MBX = 32, MBY = 16;      // 4 CTAs per tile: at most one wave at 2 CTAs per SM (tiles <= sms / 2)
 constexpr int HBX = 64, HBY = 16;      // 2 CTAs per tile: one wave up to `sms` tiles
 
+inline double strip_gen_cost() { static const double v = getenv("MG_B200_STRIP_GEN_COST") ? atof(getenv("MG_B200_STRIP_GEN_COST")) : 2.5; return v; }
 inline bool no_strips() { static const bool v = getenv("MG_B200_NO_STRIPS") != nullptr; return v; }
 
 template <int NS, bool PC, int EPI, int BX, int BY, int XIM>
@@ -47,17 +48,28 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
     ensure_dyn_smem((const void*)k_gs<NS, PC, EPI, BX, BY, XIM>, smem);
     if (NS == 2 && XIM == 0 && BX == TX && BY == TY && !no_strips()) {
         // large level, two-field form: interior tiles by the register-tiled kernel, the rest by the general tile code
-        constexpr int K = EPI ? 1 : 0, SH = EPI ? 6 : 4;
-        using SG = SGeo<SH>;
-        const int nint = lv.nint[K], ngen = lv.ntiles - nint;
-        if (ngen > 0) {
-            k_gs<NS, PC, EPI, BX, BY, XIM><<<ngen, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, lv.tlist[K] + nint);
+        constexpr int K = EPI ? 1 : 0, SH = EPI ? 6 : 4, GH = (EPI || PC) ? 8 : 6;
+        const int nint = lv.nint[K], ngen = lv.ngen[K], novf = lv.ntiles - nint - ngen, sms = dev_info().sms;
+        if (novf > 0) {
+            k_gs<NS, PC, EPI, BX, BY, XIM><<<novf, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, lv.tlist[K] + nint + ngen);
             if (L.counter) *L.counter += 1;
         }
-        if (nint > 0) {
-            constexpr size_t ssm = SG::smem(4 + (EPI ? 1 : 0), PC);
-            ensure_dyn_smem((const void*)k_gs_strip<SH, PC, EPI>, ssm);
-            k_gs_strip<SH, PC, EPI><<<std::min(nint, dev_info().sms), SG::NT, ssm, L.stream>>>(lv, lv.smeta[K], nint, xin, xout, b, ec, zero ? 1 : 0, dc, L.stop);
+        if (nint + ngen > 0) {
+            // one launch: the first ggen CTAs walk the general tiles, the rest the interior tiles; a general tile costs
+            // about STRIP_GEN_COST interior ones (wider halo, boundary phases), the SMs are split in that proportion
+            using SI = SGeo<SH>; using SGG = SGeo<GH>;
+            constexpr size_t ssm = std::max(SI::smem(PC, false), SGG::smem(PC, true));
+            constexpr int nthreads = std::max(SI::NT, SGG::NT);
+            const int grid = std::min(sms, nint + ngen);
+            int ggen = 0;
+            if (ngen > 0) {
+                const double wg = ngen * strip_gen_cost();
+                ggen = std::max(1, std::min(ngen, (int)(grid * wg / (wg + nint) + 0.5)));
+                if (nint > 0) ggen = std::min(ggen, grid - 1);
+            }
+            ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI>, ssm);
+            k_gs_strip<SH, GH, PC, EPI><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, xin, xout, b,
+                                                                            ec, zero ? 1 : 0, ccode, dc, L.stop);
             if (L.counter) *L.counter += 1;
         }
         return;

@@ -42,7 +42,7 @@ template <int XIM>
 __device__ __forceinline__ bool has_xi(const LevelDev& lv) { return XIM == 2 ? (lv.xi != nullptr) : (XIM == 1); }
 
 constexpr int GT = 512;     // threads per CTA
-constexpr int GCAP = 512;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
+constexpr int GCAP = GUARD_CAP;   // guard-list capacity per CTA; beyond it the guard phase scans the owned cells
 
 // EPI: epilogue after the sweeps.  1 (DR): the launch also restricts the defect of its result (needs x two cells beyond
 // the tile).  2 (AP): the launch also writes w = A x_out (needs one cell beyond the tile): the operator apply of the

@@ -166,3 +166,35 @@ def test_not_converged_says_why(gpu):
     assert rc == 1 and iters == 60 and relres < 1e-11
     assert "attainable" in gpu.last_error()
     s.close()
+
+
+@pytest.mark.parametrize("seed,lattice", [(301, 1025), (302, 769), (303, 1281)])
+def test_register_tiled_smoother_on_ragged_large_meshes(gpu, oracle_mod, seed, lattice):
+    """Levels of more than one tile per SM run the register-tiled smoother kernels (k_gs_strip): interior tiles and,
+    with guard lists, masks and the boundary phase, general tiles.  Ragged random domains with holes, islands, mixed
+    Dirichlet / Neumann guards, half-integer normals and fallback stencils at a size where level 0 (and 1) take that
+    path: every fused variant against the oracle — plain sweeps, sweeps + restricted defect, correction + sweeps inside
+    the cycle, and correction + sweeps + w = A x inside the solve."""
+    pl = H.random_blob_plane(seed, lattice)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    o.update(pl.lam, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    assert s.levels == o.levels
+    rng = np.random.default_rng(seed)
+    for lv in (0, 1):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        for sweeps in (2, 3, 4):
+            assert rel(host(s.smooth(lv, dev(x), dev(b), sweeps)), o.smooth(lv, x, b, sweeps)) <= TOL_STEP
+        xo = o.smooth(lv, x, b, 2)
+        do = o.restrict(lv, o.apply(lv, xo) - b)
+        xg, dg = s.smooth_restrict(lv, dev(x), dev(b), 2)
+        scale = np.linalg.norm(o.restrict(lv, np.abs(o.apply(lv, xo)) + np.abs(b)))
+        assert rel(host(xg), xo) <= TOL_STEP and np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
+        assert rel(host(s.vcycle(lv, dev(x), dev(b))), o.cycle(lv, x, b)) <= 1e-12
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    xs, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    print(f"blob {seed} {lattice}: n={pl.n} levels={o.levels} iters gpu/oracle={iters}/{ro['iters']} rel.err={rel(host(xs), ro['x']):.2e}")
+    assert rc == ro["status"] == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xs), ro["x"]) <= TOL_SOLVE
+    s.close()
