@@ -88,6 +88,12 @@ typedef struct {
                       Other bits must be 0.                                                              */
     int gamma;     /* cycle index of PAPER.md:187-189, 197: 0 or 1 = V-cycle (default), 2 = W-cycle; 3 = F-cycle
                       (one F-cycle visit, then one V-cycle visit of the next coarser level)   */
+    int planes;    /* P >= 1 (0 = 1): number of planes solved TOGETHER on this mesh (one elliptic solve per
+                      poloidal plane, all planes share the mesh).  The handle keeps the mesh data once and every vector
+                      P times; mg_update_coeffs / mg_solve then take P fields back to back (plane p at offset p * n),
+                      every kernel launch covers all planes (gridDim.y = P), each plane has its own fGMRES state and
+                      stops on its own Eq. 23; results are bit-identical to P separate handles.  The single-step and
+                      inspection calls below work on plane 0.                                                   */
 } mg_options;
 
 /* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).
@@ -103,7 +109,7 @@ int mg_set_allocator(mg_alloc_fn alloc_fn, mg_free_fn free_fn);
 int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* stream, mg_handle* out);
 
 /* update: new coefficients lambda, c (= BASELINE "xi") on ALL n points, DEVICE
- * pointers, user order.  Restricts them to all coarser levels (rule T4) and factorises the coarsest
+ * pointers, user order (P * n values for a handle with P planes).  Restricts them to all coarser levels (rule T4) and factorises the coarsest
  * operator (rule C) on the device.  Asynchronous on `stream`.  Admissibility (c > 0; finite lambda) is
  * tested on the device during the call; a violation is reported by the next mg_solve as MG_ECOEFF. */
 int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, void* stream);
@@ -119,7 +125,9 @@ int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, c
 /* solve: fGMRES(m) with one V-cycle as right preconditioner (rules K1-K5), stopping
  * on ||A x - f|| / ||f|| < rtol (Eq. 23).  d_f, d_x0, d_x: DEVICE, length n, user order;
  * d_x may alias d_x0.  iters (HOST, may be NULL) receives the number of preconditioner applications,
- * final_relres (HOST, may be NULL) the recomputed true relative residual.  Returns after the stream
+ * final_relres (HOST, may be NULL) the recomputed true relative residual.  With P planes (mg_options.planes) the three
+ * vectors hold P * n values (plane p at p * n), iters and final_relres are arrays of P entries, and the return value
+ * is the worst over the planes (MG_BREAKDOWN > MG_NOT_CONVERGED > MG_OK).  Returns after the stream
  * has finished the solve.  Returns MG_OK, MG_NOT_CONVERGED, MG_BREAKDOWN or an error.  On MG_NOT_CONVERGED
  * mg_last_error() says whether the recurrence residual had passed rtol while the recomputed true residual had not
  * (rtol below the accuracy attainable in fp64 on this mesh; the method has no stagnation exit). */

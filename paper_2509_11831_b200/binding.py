@@ -42,7 +42,7 @@ class _Bc(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("levels", C.c_int), ("nu_pre", C.c_int), ("nu_post", C.c_int), ("restart_m", C.c_int),
-                ("max_iters", C.c_int), ("flags", C.c_int), ("gamma", C.c_int)]
+                ("max_iters", C.c_int), ("flags", C.c_int), ("gamma", C.c_int), ("planes", C.c_int)]
 
 
 EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_update_coeffs3", "mg_update_coeffs3_host", "mg_level_xi", "mg_solve", "mg_update_coeffs_host",
@@ -108,7 +108,7 @@ def _dptr(t):
 class Solver:
     """create / update / solve on one mesh."""
 
-    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1, full_cgs2=False):
+    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1, full_cgs2=False, planes=1):
         import torch
         if not host_only and not torch.cuda.is_available():
             raise RuntimeError("paper_2509_11831_b200 needs a CUDA device (no CPU fallback)")
@@ -122,12 +122,13 @@ class Solver:
         mesh = _Mesh(self.n, i.ctypes.data, j.ctypes.data, float(h))
         bc = _Bc(kind.ctypes.data)
         opt = _Options(int(levels), int(nu_pre), int(nu_post) if int(nu_post) != 0 else -1,   # 0 sweeps = MG_NU_NONE
-                        int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma))
+                        int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma), int(planes))
         hd = C.c_void_p()
         rc = L.mg_setup(C.byref(mesh), C.byref(bc), C.byref(opt), None if host_only else _stream_ptr(stream), C.byref(hd))
         if rc:
             raise MgError(rc, "mg_setup")
         self._h = hd
+        self.planes = max(1, int(planes))     # with P > 1 planes: fields are [P, n] tensors, iters / relres arrays of P
         self.levels = L.mg_num_levels(self._h)
         self.device = None if host_only else torch.device("cuda", torch.cuda.current_device())
 
@@ -172,12 +173,15 @@ class Solver:
         import torch
         if x is None:
             x = torch.empty_like(f)
-        iters, relres = C.c_int(0), C.c_double(0.0)
-        rc = lib().mg_solve(self._h, _dptr(f), _dptr(x0), _dptr(x), C.c_double(rtol), C.byref(iters),
-                            C.byref(relres), _stream_ptr(stream))
+        P = self.planes
+        assert f.numel() == P * self.n and x0.numel() == P * self.n and x.numel() == P * self.n
+        iters, relres = (C.c_int * P)(), (C.c_double * P)()
+        rc = lib().mg_solve(self._h, _dptr(f), _dptr(x0), _dptr(x), C.c_double(rtol), iters, relres, _stream_ptr(stream))
         if rc < 0:
             raise MgError(rc, "mg_solve")
-        return x, iters.value, relres.value, rc
+        if P == 1:
+            return x, iters[0], relres[0], rc
+        return x, list(iters), list(relres), rc
 
     def update_coeffs_host(self, lam, c, stream=None):
         lam = np.ascontiguousarray(lam, dtype=np.float64); c = np.ascontiguousarray(c, dtype=np.float64)
@@ -187,14 +191,18 @@ class Solver:
 
     def solve_host(self, f, x0, rtol, x=None, stream=None):
         f = np.ascontiguousarray(f, dtype=np.float64); x0 = np.ascontiguousarray(x0, dtype=np.float64)
+        P = self.planes
         if x is None:
-            x = np.empty(self.n)
-        iters, relres = C.c_int(0), C.c_double(0.0)
+            x = np.empty(f.shape)
+        assert f.size == P * self.n and x0.size == P * self.n and x.size == P * self.n
+        iters, relres = (C.c_int * P)(), (C.c_double * P)()
         rc = lib().mg_solve_host(self._h, C.c_void_p(f.ctypes.data), C.c_void_p(x0.ctypes.data), C.c_void_p(x.ctypes.data),
-                                 C.c_double(rtol), C.byref(iters), C.byref(relres), _stream_ptr(stream))
+                                 C.c_double(rtol), iters, relres, _stream_ptr(stream))
         if rc < 0:
             raise MgError(rc, "mg_solve_host")
-        return x, iters.value, relres.value, rc
+        if P == 1:
+            return x, iters[0], relres[0], rc
+        return x, list(iters), list(relres), rc
 
     # ---- inspection
     def level_n(self, s):

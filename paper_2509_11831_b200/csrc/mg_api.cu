@@ -45,6 +45,7 @@ struct LevelBuf {           // device arrays owned per level
 struct mg_handle_s {
     HostHierarchy hh;
     int L = 0;
+    int P = 1;                            // planes solved together on this mesh; vectors are [plane][slot]
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
     int gamma = 1;                        // cycle type: 1 V-cycle, 2 W-cycle, 3 F-cycle
     bool full_cgs2 = false;               // MG_SETUP_FULL_CGS2
@@ -60,7 +61,8 @@ struct mg_handle_s {
     double *V = nullptr, *Z = nullptr, *w = nullptr, *r = nullptr, *xs = nullptr, *bs = nullptr;
     GmresState* st = nullptr;
     double* partial = nullptr;
-    int* h_hdr = nullptr;                 // pinned copy of the first 8 ints of the state (two slots) + [16] the coefficient flag
+    int* h_hdr = nullptr;                 // pinned copy of the first 8 ints of every plane's state (two slots of P x 8 ints)
+    int* h_flag = nullptr;                // pinned copy of the coefficient flag (behind the headers)
     int* coeff_bad = nullptr;             // device flag of the last update: bit 0 lambda not finite, bit 1 c, bit 2 xi not finite or <= 0
     bool coeffs_unchecked = false;        // the flag of the last update has not been read yet (first solve / cycle after it)
     GmresState* h_state = nullptr;        // pinned full copy (read at the end of a solve)
@@ -113,9 +115,11 @@ int upload(mg_handle h, T** dst, const std::vector<T>& src, cudaStream_t s) {
     return MG_OK;
 }
 
-Launch LZ(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }
+Launch LZ(mg_handle h, cudaStream_t s) { Launch L{s, &h->launches}; L.planes = h->P; return L; }
+Launch LZ1(mg_handle h, cudaStream_t s) { return Launch{s, &h->launches}; }       // plane 0 only (single-step entry points)
+VecRef lvec(mg_handle h, int level, double* p) { return vec(p, h->lev[level].nslots); }   // a level vector of all planes
 
-// The last update's device-side admissibility flag (G26), already copied to h_hdr[16]: MG_ECOEFF with the reason.
+// The last update's device-side admissibility flag (G26), already copied to *h_flag: MG_ECOEFF with the reason.
 int coeff_error(int b) {
     g_last_error = std::string("inadmissible coefficients in the last update:") + ((b & 1) ? " lambda not finite;" : "") +
                    ((b & 2) ? " c not finite or <= 0 (PAPER.md:51);" : "") + ((b & 4) ? " xi not finite or <= 0;" : "") +
@@ -126,11 +130,11 @@ int coeff_error(int b) {
 // Single-step entry points: read the flag of an update that has not been checked yet (one small synchronous copy).
 int check_coeffs(mg_handle h, cudaStream_t s) {
     if (h->coeffs_unchecked) {
-        CU(cudaMemcpyAsync(h->h_hdr + 16, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(h->h_flag, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
         h->coeffs_unchecked = false;
     }
-    return h->h_hdr[16] ? coeff_error(h->h_hdr[16]) : MG_OK;
+    return *h->h_flag ? coeff_error(*h->h_flag) : MG_OK;
 }
 
 // nu Gauss-Seidel sweeps, two per launch where possible, ping-ponging between `cur` and `other`.
@@ -186,7 +190,7 @@ void build_tail(mg_handle h, int s, double* x, double* b, bool x_is_zero, TailPr
 bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool x_is_zero, double* w_out = nullptr, int kind = 0) {
     const LevelDev& lv = h->lev[s];
     if (kind == 0) kind = h->gamma;
-    if (s >= h->tail_s0) {                                            // small levels: one cooperative kernel
+    if (s >= h->tail_s0 && h->P == 1) {                                            // small levels: one cooperative kernel
         TailProgram P; P.nops = 0;
         build_tail(h, s, TAIL_TOPX, TAIL_TOPB, x_is_zero, P, kind);
         if (P.nops <= TAIL_MAX_OPS) {
@@ -203,7 +207,7 @@ bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
         launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, b, x);
         return false;
     }
-    VecRef tmp = vec(h->buf[s].x2);
+    VecRef tmp = lvec(h, s, h->buf[s].x2);
     if (x_is_zero && h->nu_pre == 0) { launch_zero(L, x, lv.nslots); x_is_zero = false; }
     const bool fuse_dr = h->nu_pre > 0 && !h->no_fused_dr;
     VecRef cur = enqueue_smooth(L, lv, x, tmp, b, h->nu_pre, x_is_zero,                   // P:178-181 (+ P:183-184 fused)
@@ -213,7 +217,7 @@ bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
     int vk[2];
     const int nvis = cycle_visits(kind, vk);
     for (int g = 0; g < nvis; g++)                                                        // e0 = 0, gamma visits
-        enqueue_cycle(h, L, s + 1, vec(h->buf[s + 1].x), vec(h->buf[s + 1].b), g == 0, nullptr, vk[g]);
+        enqueue_cycle(h, L, s + 1, lvec(h, s + 1, h->buf[s + 1].x), lvec(h, s + 1, h->buf[s + 1].b), g == 0, nullptr, vk[g]);
     VecRef fin;
     bool wrote_w = false;
     if (h->nu_post > 0) {                                 // P:194-197 fused into the first post-smoothing pass
@@ -232,10 +236,11 @@ bool enqueue_cycle(mg_handle h, const Launch& L, int s, VecRef x, VecRef b, bool
 // One Arnoldi step (rule K2): z_j = MG(v_j), w = A z_j, CGS2, Givens + stop test, v_{j+1}.
 void enqueue_iteration(mg_handle h, const Launch& L) {
     const int64_t ns = h->lev[0].nslots;
-    VecRef zj{h->Z, ns, &h->st->j, 0}, vj{h->V, ns, &h->st->j, 0};
+    const int64_t bps = (int64_t)(h->m + 1) * ns;                    // plane stride of the Krylov bases
+    VecRef zj{h->Z, ns, &h->st->j, 0, bps}, vj{h->V, ns, &h->st->j, 0, bps};
     static const bool no_fused_apply = getenv("MG_B200_NO_FUSED_APPLY") != nullptr;
     if (!enqueue_cycle(h, L, 0, zj, vj, true, no_fused_apply ? nullptr : h->w))          // w = A z_j fused into the cycle's last launch
-        launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w), 0);
+        launch_apply(L, h->lev[0], zj, vec(nullptr), vec(h->w, ns), 0);
     launch_multidot(L, h->w, h->V, ns, ns, h->st, h->partial, h->m);
     if (h->m <= MAX_M_FUSED) {                                     // three passes over the basis
         launch_update_dot(L, h->w, h->V, ns, ns, h->st, h->partial);
@@ -314,7 +319,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < MG_NU_NONE || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < MG_NU_NONE || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0 || o.planes < 0 || o.planes > 4096) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
@@ -325,6 +330,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     h->m = o.restart_m ? o.restart_m : 30;
     h->max_iters = o.max_iters ? o.max_iters : 200;
     h->gamma = o.gamma > 1 ? o.gamma : 1;
+    h->P = o.planes > 1 ? o.planes : 1;
     h->full_cgs2 = (o.flags & MG_SETUP_FULL_CGS2) != 0;
     h->n = mesh->n;
     h->alloc = g_alloc; h->free_fn = g_free;
@@ -342,10 +348,11 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     CUF(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
     for (auto& e : h->ev) CUF(cudaEventCreate(&e));
     for (auto& e : h->hev) CUF(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    CUF(cudaMallocHost((void**)&h->h_hdr, 128));
-    h->h_hdr[16] = 0;
+    CUF(cudaMallocHost((void**)&h->h_hdr, sizeof(int) * (16 * (size_t)h->P + 8)));      // two header slots of 8 ints per plane + the coefficient flag
+    h->h_flag = h->h_hdr + 16 * (size_t)h->P;
+    *h->h_flag = 0;
     TRY(dev_alloc(h, (void**)&h->coeff_bad, sizeof(int), s));
-    CUF(cudaMallocHost((void**)&h->h_state, sizeof(GmresState)));
+    CUF(cudaMallocHost((void**)&h->h_state, sizeof(GmresState) * h->P));
     h->lev.resize(h->L); h->buf.resize(h->L);
     for (int l = 0; l < h->L; l++) {
         HostLevel& hl = h->hh.lev[l];
@@ -370,7 +377,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
             }
             TRY(upload(h, &b.smeta[k], meta, s));
         }
-        const size_t vb = (size_t)hl.nslots() * sizeof(double);
+        const size_t vb1 = (size_t)hl.nslots() * sizeof(double), vb = vb1 * h->P;      // every vector once per plane
         TRY(dev_alloc(h, (void**)&b.lam, vb, s));
         TRY(dev_alloc(h, (void**)&b.c, vb, s));
         TRY(dev_alloc(h, (void**)&b.rd, vb, s));
@@ -378,7 +385,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         TRY(dev_alloc(h, (void**)&b.x2, vb, s));
         TRY(dev_alloc(h, (void**)&b.b, vb, s));
         TRY(dev_alloc(h, (void**)&b.d, vb, s));
-        TRY(dev_alloc(h, (void**)&b.tb, vb, s));
+        TRY(dev_alloc(h, (void**)&b.tb, vb1, s));
         LevelDev& d = h->lev[l];
         d.ntiles = hl.ntiles;
         d.ntiles_fine = l > 0 ? h->hh.lev[l - 1].ntiles : 0;
@@ -393,26 +400,26 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     CUF(cudaMemcpyAsync(h->d_lev, h->lev.data(), sizeof(LevelDev) * h->L, cudaMemcpyHostToDevice, s));
     h->no_fused_dr = getenv("MG_B200_NO_FUSED_DR") != nullptr;
     h->tail_cap = std::min(tail_max_grid(), 2 * dev_info().sms);
-    if (h->tail_cap > 0 && h->nu_pre >= 1 && h->nu_post >= 1 && ((o.flags & MG_SETUP_FUSED_TAIL) || getenv("MG_B200_FUSED_TAIL")))
+    if (h->P == 1 && h->tail_cap > 0 && h->nu_pre >= 1 && h->nu_post >= 1 && ((o.flags & MG_SETUP_FUSED_TAIL) || getenv("MG_B200_FUSED_TAIL")))
         for (int l = h->L - 1; l >= 0 && h->lev[l].ntiles <= h->tail_cap; l--) h->tail_s0 = l;
     TRY(upload(h, &h->user2slot, h->hh.user2slot, s));
-    const size_t v0 = (size_t)h->lev[0].nslots * sizeof(double);
+    const size_t v0 = (size_t)h->lev[0].nslots * sizeof(double) * h->P;
     TRY(dev_alloc(h, (void**)&h->V, v0 * (h->m + 1), s));
     TRY(dev_alloc(h, (void**)&h->Z, v0 * (h->m + 1), s));
     TRY(dev_alloc(h, (void**)&h->w, v0, s));
     TRY(dev_alloc(h, (void**)&h->r, v0, s));
     TRY(dev_alloc(h, (void**)&h->xs, v0, s));
     TRY(dev_alloc(h, (void**)&h->bs, v0, s));
-    TRY(dev_alloc(h, (void**)&h->st, sizeof(GmresState), s));
-    TRY(dev_alloc(h, (void**)&h->partial, sizeof(double) * RED_BLOCKS_MAX * (MAX_M + 2), s));
+    TRY(dev_alloc(h, (void**)&h->st, sizeof(GmresState) * h->P, s));
+    TRY(dev_alloc(h, (void**)&h->partial, sizeof(double) * RED_BLOCKS_MAX * (MAX_M + 2) * h->P, s));
     {   // coarsest level: canonical row -> slot and its inverse
         HostLevel& cl = h->hh.lev.back();
         std::vector<int32_t> s2r((size_t)cl.nslots(), 0);
         for (int r = 0; r < h->nL; r++) s2r[cl.canon2slot[r]] = r;
         h->cslot = h->buf[h->L - 1].canon2slot;
         TRY(upload(h, &h->slot2row, s2r, s));
-        TRY(dev_alloc(h, (void**)&h->cwork, sizeof(double) * (2 * (size_t)h->nL * h->nL + 2 * (size_t)h->nL + 2), s));   // [A | I] + published column (x2) + pivots
-        TRY(dev_alloc(h, (void**)&h->Ainv, sizeof(double) * (size_t)h->nL * h->nL, s));
+        TRY(dev_alloc(h, (void**)&h->cwork, sizeof(double) * coarse_work_doubles(h->nL) * h->P, s));   // [A | I] + published column (x2) + pivots
+        TRY(dev_alloc(h, (void**)&h->Ainv, sizeof(double) * (size_t)h->nL * h->nL * h->P, s));
     }
     CUF(cudaStreamSynchronize(s));
 #undef TRY
@@ -434,7 +441,7 @@ static int set_three_field(mg_handle h, bool on, cudaStream_t s) {
     for (int l = 0; l < h->L; l++) {
         LevelBuf& b = h->buf[l];
         if (on && !b.xi) {
-            const size_t vb = (size_t)h->hh.lev[l].nslots() * sizeof(double);
+            const size_t vb = (size_t)h->hh.lev[l].nslots() * sizeof(double) * h->P;
             int rc = dev_alloc(h, (void**)&b.xi, vb, s); if (rc) return rc;
         }
         h->lev[l].xi = on ? b.xi : nullptr;
@@ -458,9 +465,10 @@ int mg_update_coeffs3(mg_handle h, const double* d_lambda, const double* d_xi, c
     // admissibility (c > 0; lambda only finite since Eq. 21 P:241 has both signs; xi > 0, G25) is tested on the device while
     // the fields are gathered; the first mg_solve after the update reads the flag and returns MG_ECOEFF
     CU(cudaMemsetAsync(h->coeff_bad, 0, sizeof(int), s));
-    launch_gather_check(L, d_lambda, h->user2slot, h->buf[0].lam, h->n, 1, 1, h->coeff_bad);
-    launch_gather_check(L, d_c, h->user2slot, h->buf[0].c, h->n, 2, 2, h->coeff_bad);
-    if (d_xi) launch_gather_check(L, d_xi, h->user2slot, h->buf[0].xi, h->n, 2, 4, h->coeff_bad);
+    const int64_t ns0 = h->lev[0].nslots;
+    launch_gather_check(L, d_lambda, h->user2slot, h->buf[0].lam, h->n, ns0, 1, 1, h->coeff_bad);
+    launch_gather_check(L, d_c, h->user2slot, h->buf[0].c, h->n, ns0, 2, 2, h->coeff_bad);
+    if (d_xi) launch_gather_check(L, d_xi, h->user2slot, h->buf[0].xi, h->n, ns0, 2, 4, h->coeff_bad);
     h->coeffs_unchecked = true;
     for (int l = 0; l + 1 < h->L; l++) launch_restrict_coeff(L, h->lev[l], h->lev[l + 1]);     // rule T4
     for (int l = 0; l < h->L; l++) launch_diag(L, h->lev[l]);                                   // U2: 1 / a_ll for the smoother
@@ -476,6 +484,16 @@ int mg_update_coeffs(mg_handle h, const double* d_lambda, const double* d_c, voi
     return mg_update_coeffs3(h, d_lambda, nullptr, d_c, stream);
 }
 
+// first 8 ints (j, iters, status, cycle_end, ...) of every plane's state -> pinned header slot `slot`
+static int copy_headers(mg_handle h, int slot, cudaStream_t s) {
+    CU(cudaMemcpy2DAsync(h->h_hdr + (size_t)slot * 8 * h->P, 32, h->st, sizeof(GmresState), 32, h->P, cudaMemcpyDeviceToHost, s));
+    return MG_OK;
+}
+static bool all_ended(mg_handle h, int slot) {
+    for (int p = 0; p < h->P; p++) if (!h->h_hdr[((size_t)slot * h->P + p) * 8 + 3]) return false;
+    return true;
+}
+
 int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, double rtol, int* iters,
              double* final_relres, void* stream) {
     if (!h || !d_f || !d_x0 || !d_x || !(rtol > 0.0)) return MG_EINVAL;
@@ -486,73 +504,81 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
     int rc = build_iter_graph(h);
     if (rc) return rc;
     const int64_t ns = h->lev[0].nslots;
+    const int P = h->P;
     CU(cudaEventRecord(h->ev[0], s));
     launch_init_state(L, h->st, h->m, h->max_iters, rtol, h->full_cgs2);
-    launch_gather(L, d_f, h->user2slot, h->bs, h->n);                 // B1: user order -> tile layout
-    launch_gather(L, d_x0, h->user2slot, h->xs, h->n);
+    launch_gather(L, d_f, h->user2slot, h->bs, h->n, ns);             // B1: user order -> tile layout
+    launch_gather(L, d_x0, h->user2slot, h->xs, h->n, ns);
     launch_norm2(L, h->bs, ns, h->st, h->partial, 0);                 // K1: bn = ||b||
-    int status = 0;
+    // All planes run the same launches; each has its own state.  A plane whose restart cycle has ended (converged,
+    // m columns, max_iters, breakdown) makes its CTAs return at once until every plane has ended the cycle; then
+    // x is updated (a plane that did not start the cycle adds nothing) and the next cycle starts where needed.
     for (int cycle = 0; cycle < 1000000; cycle++) {
-        launch_apply(L, h->lev[0], vec(h->xs), vec(h->bs), vec(h->r), 1);      // r = b - A x (rule D4)
+        launch_apply(L, h->lev[0], vec(h->xs, ns), vec(h->bs, ns), vec(h->r, ns), 1);      // r = b - A x (rule D4)
         launch_norm2(L, h->r, ns, h->st, h->partial, 1);
         launch_start_cycle(L, h->st, h->r, h->V, ns);
-        CU(cudaMemcpyAsync(h->h_hdr, h->st, 32, cudaMemcpyDeviceToHost, s));
-        if (h->coeffs_unchecked) CU(cudaMemcpyAsync(h->h_hdr + 16, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
+        rc = copy_headers(h, 0, s);
+        if (rc) return rc;
+        if (h->coeffs_unchecked) CU(cudaMemcpyAsync(h->h_flag, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
         h->coeffs_unchecked = false;
-        if (h->h_hdr[16]) {                                           // the last update's fields were not admissible
+        if (*h->h_flag) {                                             // the last update's fields were not admissible
             h->solve_timed = false;                                   // ev[0] has no matching end event
-            return coeff_error(h->h_hdr[16]);
+            return coeff_error(*h->h_flag);
         }
-        status = h->h_hdr[2];
-        if (h->h_hdr[3]) break;                                       // cycle_end set by start: finished
+        if (all_ended(h, 0)) break;                                   // no plane started a cycle: finished
         // One graph launch per Arnoldi step.  The host stays one step ahead: step `it` is enqueued before
-        // the header of step it-1 is inspected, so the GPU never idles on the round trip; a step enqueued
+        // the headers of step it-1 are inspected, so the GPU never idles on the round trip; a step enqueued
         // after the cycle has ended finds cycle_end set and every kernel in it returns at once.
         for (int it = 0; it < h->m; it++) {
             CU(cudaGraphLaunch(h->iter_graph, s));
             h->launches += h->iter_graph_kernels;
-            CU(cudaMemcpyAsync(h->h_hdr + 8 * (it & 1), h->st, 32, cudaMemcpyDeviceToHost, s));
+            rc = copy_headers(h, it & 1, s);
+            if (rc) return rc;
             CU(cudaEventRecord(h->hev[it & 1], s));
             if (it >= 1) {
                 CU(cudaEventSynchronize(h->hev[(it - 1) & 1]));
-                if (h->h_hdr[8 * ((it - 1) & 1) + 3]) break;
+                if (all_ended(h, (it - 1) & 1)) break;
             }
         }
         launch_update_x(L, h->xs, h->Z, ns, ns, h->st);               // K4
     }
-    if (status == 4) launch_zero(L, vec(h->xs), ns);                  // K1: zero right-hand side
-    launch_scatter(L, h->xs, h->user2slot, d_x, h->n);                // B1: tile layout -> user order
+    launch_zero_rhs_planes(L, h->xs, ns, h->st);                      // K1: zero right-hand side -> x = 0
+    launch_scatter(L, h->xs, h->user2slot, d_x, h->n, ns);            // B1: tile layout -> user order
     CU(cudaEventRecord(h->ev[1], s));
-    CU(cudaMemcpyAsync(h->h_state, h->st, sizeof(GmresState), cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(h->h_state, h->st, sizeof(GmresState) * P, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     CU(cudaGetLastError());
     h->solve_timed = true;
-    if (iters) *iters = h->h_state->iters;
-    if (final_relres) *final_relres = h->h_state->relres;
-    if (status == 1 || status == 4) return MG_OK;
-    if (status == 3) return MG_BREAKDOWN;
-    {   // Not converged.  If the recurrence residual (Eq. 23 inside a cycle, rule K3) went below rtol while the recomputed true
-        // residual (rule K5) did not, the solve sits on the fp64 floor of evaluating b - A x, about eps |A||x| / |b| ~ 1/h^2
-        // (DESIGN.md "Attainable accuracy"); the paper has no stagnation exit, so the call only says so.
-        const GmresState* st = h->h_state;
-        const int k = std::min(st->iters, 512);
-        double best = 1e300;
-        for (int i = 0; i < k; i++) best = std::min(best, st->hist[i]);
-        char buf[320];
-        if (k > 0 && best < rtol)
-            snprintf(buf, sizeof buf, "not converged after %d iterations: the recurrence residual reached %.2e < rtol = %.2e but the true residual "
-                     "|b - A x| / |b| stays at %.2e: rtol is below the accuracy attainable in fp64 on this mesh", st->iters, best, rtol, st->relres);
-        else
-            snprintf(buf, sizeof buf, "not converged after %d iterations: |b - A x| / |b| = %.2e, rtol = %.2e", st->iters, st->relres, rtol);
-        g_last_error = buf;
+    int worst = MG_OK;                                                // over the planes: breakdown > not converged > ok
+    for (int p = 0; p < P; p++) {
+        const GmresState* st = &h->h_state[p];
+        if (iters) iters[p] = st->iters;
+        if (final_relres) final_relres[p] = st->relres;
+        const int r1 = (st->status == 1 || st->status == 4) ? MG_OK : (st->status == 3 ? MG_BREAKDOWN : MG_NOT_CONVERGED);
+        if (r1 == MG_NOT_CONVERGED) {
+            // If the recurrence residual (Eq. 23 inside a cycle, rule K3) went below rtol while the recomputed true residual
+            // (rule K5) did not, the solve sits on the fp64 floor of evaluating b - A x, about eps |A||x| / |b| ~ 1/h^2
+            // (DESIGN.md "Attainable accuracy"); the paper has no stagnation exit, so the call only says so.
+            const int k = std::min(st->iters, 512);
+            double best = 1e300;
+            for (int i = 0; i < k; i++) best = std::min(best, st->hist[i]);
+            char buf[360];
+            if (k > 0 && best < rtol)
+                snprintf(buf, sizeof buf, "plane %d not converged after %d iterations: the recurrence residual reached %.2e < rtol = %.2e but the true "
+                         "residual |b - A x| / |b| stays at %.2e: rtol is below the accuracy attainable in fp64 on this mesh", p, st->iters, best, rtol, st->relres);
+            else
+                snprintf(buf, sizeof buf, "plane %d not converged after %d iterations: |b - A x| / |b| = %.2e, rtol = %.2e", p, st->iters, st->relres, rtol);
+            g_last_error = buf;
+        }
+        worst = std::max(worst, r1);
     }
-    return MG_NOT_CONVERGED;
+    return worst;
 }
 
 static int ensure_stage(mg_handle h, cudaStream_t s) {
     for (int k = 0; k < 3; k++)
-        if (!h->stage[k]) { int rc = dev_alloc(h, (void**)&h->stage[k], sizeof(double) * (size_t)h->n, s); if (rc) return rc; }
+        if (!h->stage[k]) { int rc = dev_alloc(h, (void**)&h->stage[k], sizeof(double) * (size_t)h->n * h->P, s); if (rc) return rc; }
     return MG_OK;
 }
 
@@ -562,8 +588,8 @@ int mg_update_coeffs_host(mg_handle h, const double* h_lambda, const double* h_c
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
-    CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
     return mg_update_coeffs(h, h->stage[0], h->stage[1], stream);
 }
 
@@ -574,10 +600,10 @@ int mg_update_coeffs3_host(mg_handle h, const double* h_lambda, const double* h_
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
-    if (!h->stage_xi) { rc = dev_alloc(h, (void**)&h->stage_xi, sizeof(double) * (size_t)h->n, s); if (rc) return rc; }
-    CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
-    CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
-    CU(cudaMemcpyAsync(h->stage_xi, h_xi, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    if (!h->stage_xi) { rc = dev_alloc(h, (void**)&h->stage_xi, sizeof(double) * (size_t)h->n * h->P, s); if (rc) return rc; }
+    CU(cudaMemcpyAsync(h->stage[0], h_lambda, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[1], h_c, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage_xi, h_xi, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
     return mg_update_coeffs3(h, h->stage[0], h->stage_xi, h->stage[1], stream);
 }
 
@@ -588,11 +614,11 @@ int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->stage[0], h_f, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
-    CU(cudaMemcpyAsync(h->stage[1], h_x0, sizeof(double) * h->n, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[0], h_f, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(h->stage[1], h_x0, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
     rc = mg_solve(h, h->stage[0], h->stage[1], h->stage[2], rtol, iters, final_relres, stream);
     if (rc < 0) return rc;
-    CU(cudaMemcpyAsync(h_x, h->stage[2], sizeof(double) * h->n, cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(h_x, h->stage[2], sizeof(double) * h->n * h->P, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     return rc;
 }
@@ -754,89 +780,89 @@ int mg_level_xi(mg_handle h, int level, double* h_xi, void* stream) {
 
 int mg_apply(mg_handle h, int level, const double* d_x, double* d_y, void* stream) {
     CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_y);
-    Launch L = LZ(h, (cudaStream_t)stream);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
     const int64_t n = h->hh.lev[level].n;
-    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n, 0);
     launch_apply(L, h->lev[level], vec(h->buf[level].x), vec(nullptr), vec(h->buf[level].d), 0);
-    launch_scatter(L, h->buf[level].d, h->buf[level].canon2slot, d_y, n);
+    launch_scatter(L, h->buf[level].d, h->buf[level].canon2slot, d_y, n, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
 int mg_smooth(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, void* stream) {
     CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_b && sweeps >= 0);
-    Launch L = LZ(h, (cudaStream_t)stream);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
     const int64_t n = h->hh.lev[level].n;
-    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
-    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n, 0);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n, 0);
     CU(cudaEventRecord(h->ev[4], L.stream));
     VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].tb), sweeps, false);
     CU(cudaEventRecord(h->ev[5], L.stream));
     h->step_timed = true;
-    launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n);
+    launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
 int mg_smooth_restrict(mg_handle h, int level, double* d_x, const double* d_b, int sweeps, double* d_coarse, void* stream) {
     CHECK_LEVEL(level >= 0 && level + 1 < h->L && d_x && d_b && d_coarse && sweeps >= 1);
-    Launch L = LZ(h, (cudaStream_t)stream);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
     const int64_t n = h->hh.lev[level].n;
-    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
-    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n, 0);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n, 0);
     CU(cudaEventRecord(h->ev[4], L.stream));
     VecRef fin = enqueue_smooth(L, h->lev[level], vec(h->buf[level].x), vec(h->buf[level].x2), vec(h->buf[level].tb), sweeps, false,
                                 &h->lev[level + 1], h->buf[level + 1].b);
     CU(cudaEventRecord(h->ev[5], L.stream));
     h->step_timed = true;
-    launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n);
-    launch_scatter(L, h->buf[level + 1].b, h->buf[level + 1].canon2slot, d_coarse, h->hh.lev[level + 1].n);
+    launch_scatter(L, fin.base, h->buf[level].canon2slot, d_x, n, 0);
+    launch_scatter(L, h->buf[level + 1].b, h->buf[level + 1].canon2slot, d_coarse, h->hh.lev[level + 1].n, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
 int mg_restrict(mg_handle h, int level, const double* d_fine, double* d_coarse, void* stream) {
     CHECK_LEVEL(level >= 0 && level + 1 < h->L && d_fine && d_coarse);
-    Launch L = LZ(h, (cudaStream_t)stream);
-    launch_gather(L, d_fine, h->buf[level].canon2slot, h->buf[level].d, h->hh.lev[level].n);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
+    launch_gather(L, d_fine, h->buf[level].canon2slot, h->buf[level].d, h->hh.lev[level].n, 0);
     launch_restrict(L, h->lev[level], h->lev[level + 1], h->buf[level].d, h->buf[level + 1].b);
-    launch_scatter(L, h->buf[level + 1].b, h->buf[level + 1].canon2slot, d_coarse, h->hh.lev[level + 1].n);
+    launch_scatter(L, h->buf[level + 1].b, h->buf[level + 1].canon2slot, d_coarse, h->hh.lev[level + 1].n, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
 int mg_prolong_correct(mg_handle h, int level, const double* d_coarse_e, double* d_x_fine, void* stream) {
     CHECK_LEVEL(level >= 0 && level + 1 < h->L && d_coarse_e && d_x_fine);
-    Launch L = LZ(h, (cudaStream_t)stream);
-    launch_gather(L, d_coarse_e, h->buf[level + 1].canon2slot, h->buf[level + 1].x, h->hh.lev[level + 1].n);
-    launch_gather(L, d_x_fine, h->buf[level].canon2slot, h->buf[level].x, h->hh.lev[level].n);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
+    launch_gather(L, d_coarse_e, h->buf[level + 1].canon2slot, h->buf[level + 1].x, h->hh.lev[level + 1].n, 0);
+    launch_gather(L, d_x_fine, h->buf[level].canon2slot, h->buf[level].x, h->hh.lev[level].n, 0);
     launch_prolong_correct(L, h->lev[level], h->lev[level + 1], h->buf[level + 1].x, h->buf[level].d, vec(h->buf[level].x));
-    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x_fine, h->hh.lev[level].n);
+    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x_fine, h->hh.lev[level].n, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
 int mg_coarse_solve(mg_handle h, const double* d_b, double* d_x, void* stream) {
     CHECK_LEVEL(d_b && d_x);
-    Launch L = LZ(h, (cudaStream_t)stream);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
     const int l = h->L - 1;
-    launch_gather(L, d_b, h->buf[l].canon2slot, h->buf[l].tb, h->nL);
+    launch_gather(L, d_b, h->buf[l].canon2slot, h->buf[l].tb, h->nL, 0);
     launch_coarse_solve(L, h->Ainv, h->cslot, h->nL, vec(h->buf[l].tb), vec(h->buf[l].x));
-    launch_scatter(L, h->buf[l].x, h->buf[l].canon2slot, d_x, h->nL);
+    launch_scatter(L, h->buf[l].x, h->buf[l].canon2slot, d_x, h->nL, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
 int mg_vcycle(mg_handle h, int level, double* d_x, const double* d_b, void* stream) {
     CHECK_LEVEL(level >= 0 && level < h->L && d_x && d_b);
-    Launch L = LZ(h, (cudaStream_t)stream);
+    Launch L = LZ1(h, (cudaStream_t)stream);      // plane 0
     const int64_t n = h->hh.lev[level].n;
     // level buffers x/b of `level` are free here: the recursion only uses those of the coarser levels
-    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n);
-    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n);
+    launch_gather(L, d_x, h->buf[level].canon2slot, h->buf[level].x, n, 0);
+    launch_gather(L, d_b, h->buf[level].canon2slot, h->buf[level].tb, n, 0);
     enqueue_cycle(h, L, level, vec(h->buf[level].x), vec(h->buf[level].tb), false);
     CU(h->tail_err);
-    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n);
+    launch_scatter(L, h->buf[level].x, h->buf[level].canon2slot, d_x, n, 0);
     CU(cudaGetLastError());
     return MG_OK;
 }

@@ -25,6 +25,8 @@ __global__ void k_coarse_assemble(LevelDev lv, const int32_t* __restrict__ cslot
                                   int n, double* __restrict__ W) {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
+    lv = plane_of(lv, blockIdx.y);
+    W += blockIdx.y * coarse_work_doubles(n);
     double* row = W + (size_t)r * 2 * n;
     for (int k = 0; k < 2 * n; k++) row[k] = 0.0;
     row[n + r] = 1.0;
@@ -80,6 +82,7 @@ __global__ void __launch_bounds__(CT) k_coarse_invert(int n, double* __restrict_
     __shared__ int redi[CT / 32];
     __shared__ int piv;
     const int tid = threadIdx.x, n2 = 2 * n;
+    Wg += blockIdx.y * coarse_work_doubles(n); Ainv += (size_t)blockIdx.y * n * n;
     double* W = Wg;
     if (in_smem) {
         for (int e = tid; e < n * n2; e += CT) wsm[e] = Wg[e];
@@ -205,9 +208,11 @@ __global__ void __launch_bounds__(CIT) k_coarse_invert_coop(int n, int cpb, cons
 __global__ void __launch_bounds__(CT) k_coarse_solve(const double* __restrict__ Ainv, const int32_t* __restrict__ cslot, int n,
                                                      VecRef br, VecRef xr, const int* __restrict__ stop) {
     __shared__ double sb[1024];
-    if (stop != nullptr && *stop) return;
-    const double* __restrict__ b = resolve(br);
-    double* __restrict__ x = resolve(xr);
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    Ainv += (size_t)pl * n * n;
+    const double* __restrict__ b = resolve(br, pl);
+    double* __restrict__ x = resolve(xr, pl);
     for (int r = threadIdx.x; r < n; r += CT) sb[r] = b[cslot[r]];
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -223,7 +228,7 @@ __global__ void __launch_bounds__(CT) k_coarse_solve(const double* __restrict__ 
 
 void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
                           double* work, double* Ainv, int* bad) {
-    k_coarse_assemble<<<(n + 127) / 128, 128, 0, L.stream>>>(lv, cslot, slot2row, n, work);
+    k_coarse_assemble<<<dim3((n + 127) / 128, L.planes), 128, 0, L.stream>>>(lv, cslot, slot2row, n, work);
     const size_t wbytes = (size_t)n * 2 * n * sizeof(double);
     const int in_smem = wbytes <= 200 * 1024;
     ensure_dyn_smem((const void*)k_coarse_invert, 200 * 1024);
@@ -235,21 +240,25 @@ void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cs
         G = (2 * n + cpb - 1) / cpb;
         const size_t smem = ((size_t)cpb * n + n + 2 * (size_t)cpb) * sizeof(double);
         if (smem <= 200 * 1024) {
-            double* colbuf = work + (size_t)2 * n * n;        // 2 n doubles + 2 ints behind [A | I] (allocated by mg_setup)
-            int* pivbuf = reinterpret_cast<int*>(colbuf + 2 * n);
-            const double* Wg = work;
-            void* args[] = {(void*)&n, (void*)&cpb, (void*)&Wg, (void*)&Ainv, (void*)&colbuf, (void*)&pivbuf, (void*)&bad};
-            cudaLaunchCooperativeKernel((const void*)k_coarse_invert_coop, dim3(G), dim3(CIT), args, smem, L.stream);
-            if (L.counter) *L.counter += 2;
+            for (int pl = 0; pl < L.planes; pl++) {           // one cooperative grid per plane
+                double* wp = work + (size_t)pl * coarse_work_doubles(n);
+                double* colbuf = wp + (size_t)2 * n * n;      // 2 n doubles + 2 ints behind [A | I] (allocated by mg_setup)
+                int* pivbuf = reinterpret_cast<int*>(colbuf + 2 * n);
+                const double* Wg = wp;
+                double* ai = Ainv + (size_t)pl * n * n;
+                void* args[] = {(void*)&n, (void*)&cpb, (void*)&Wg, (void*)&ai, (void*)&colbuf, (void*)&pivbuf, (void*)&bad};
+                cudaLaunchCooperativeKernel((const void*)k_coarse_invert_coop, dim3(G), dim3(CIT), args, smem, L.stream);
+            }
+            if (L.counter) *L.counter += 1 + L.planes;
             return;
         }
     }
-    k_coarse_invert<<<1, CT, in_smem ? wbytes : 0, L.stream>>>(n, work, Ainv, in_smem, bad);
+    k_coarse_invert<<<dim3(1, L.planes), CT, in_smem ? wbytes : 0, L.stream>>>(n, work, Ainv, in_smem, bad);
     if (L.counter) *L.counter += 2;
 }
 
 void launch_coarse_solve(const Launch& L, const double* Ainv, const int32_t* cslot, int n, VecRef b_tiled, VecRef x_tiled) {
-    k_coarse_solve<<<1, CT, 0, L.stream>>>(Ainv, cslot, n, b_tiled, x_tiled, L.stop);
+    k_coarse_solve<<<dim3(1, L.planes), CT, 0, L.stream>>>(Ainv, cslot, n, b_tiled, x_tiled, L.stop);
     if (L.counter) *L.counter += 1;
 }
 

@@ -47,21 +47,6 @@ struct LevelDev {
     double* xi;              // xi on every present point (grid-transferred like lambda and c)
 };
 
-// A vector that may be one column of a Krylov basis selected on the device:
-// address = base + (idx ? *idx + off : 0) * stride.
-struct VecRef {
-    double* base;
-    int64_t stride;
-    const int* idx;
-    int off;
-};
-__host__ __device__ inline VecRef vec(double* p) { return VecRef{p, 0, nullptr, 0}; }
-#ifdef __CUDACC__
-__device__ __forceinline__ double* resolve(const VecRef& v) {
-    return v.base + (v.idx ? (int64_t)(*v.idx + v.off) * v.stride : 0);
-}
-#endif
-
 // fGMRES state, resident on the device (rules K1-K5).  Givens rotations, the least-squares
 // right-hand side and the stop test live here so that no iteration needs the host.
 struct GmresState {
@@ -84,11 +69,59 @@ struct GmresState {
     double orth[512];               // ||V^T w'|| / ||w'|| after the first Gram-Schmidt projection, per iteration (fused path)
 };
 
+// Planes (one elliptic solve per poloidal plane, all on the same mesh).  A handle created
+// with P planes keeps the mesh data (codes, tile tables) once and every vector P times, plane p at p * (plane stride);
+// all kernels take the plane from blockIdx.y, so one launch (one captured graph) serves all planes, each with its own
+// fGMRES state and convergence flag.
+constexpr int ST_INTS = (int)(sizeof(GmresState) / sizeof(int));   // distance between the states of two planes, in ints
+
+// A vector that may be one column of a Krylov basis selected on the device:
+// address = base + plane * pstride + (idx ? idx[plane * ST_INTS] + off : 0) * stride.
+struct VecRef {
+    double* base;
+    int64_t stride;
+    const int* idx;
+    int off;
+    int64_t pstride;
+};
+__host__ __device__ inline VecRef vec(double* p, int64_t pstride = 0) { return VecRef{p, 0, nullptr, 0, pstride}; }
+#ifdef __CUDACC__
+__device__ __forceinline__ double* resolve(const VecRef& v, int plane = 0) {
+    return v.base + plane * v.pstride + (v.idx ? (int64_t)(v.idx[(int64_t)plane * ST_INTS] + v.off) * v.stride : 0);
+}
+// plane p of a level: the coefficient arrays advance by p * nslots; codes and tile tables are shared
+__device__ __forceinline__ LevelDev plane_of(LevelDev lv, int p) {
+    const int64_t o = (int64_t)p * lv.nslots;
+    lv.lam += o; lv.c += o; lv.rd += o;
+    if (lv.xi) lv.xi += o;
+    return lv;
+}
+// Inner row of rule D1 in difference form, lambda x_l + a_W (x_l - x_W) + a_E (x_l - x_E) + a_S (x_l - x_S) + a_N (x_l - x_N),
+// with the rounding sequence spelled out (one product, four fused multiply-adds in the order W, E, S, N) so that every
+// kernel that evaluates a row — stand-alone, fused into a smoother launch, shared-memory or register-tiled — produces the
+// same bits and the choice of kernel (level size, number of planes) never shows in a result.
+__device__ __forceinline__ double row_d1(double lam, double xl, double aW, double xW, double aE, double xE, double aS, double xS,
+                                         double aN, double xN) {
+    double r = __dmul_rn(lam, xl);
+    r = __fma_rn(aW, __dsub_rn(xl, xW), r);
+    r = __fma_rn(aE, __dsub_rn(xl, xE), r);
+    r = __fma_rn(aS, __dsub_rn(xl, xS), r);
+    r = __fma_rn(aN, __dsub_rn(xl, xN), r);
+    return r;
+}
+// Eq. 16 solved for the guard point, x_l = (sum_{k != l} w_k x_k - delta b_l) / (1 - w_l), rounding sequence fixed likewise
+__device__ __forceinline__ double neumann_point(double sum, double delta, double b, double wself) {
+    return __ddiv_rn(__fma_rn(-delta, b, sum), __dsub_rn(1.0, wself));
+}
+__device__ __forceinline__ bool stopped(const int* stop, int plane) { return stop != nullptr && stop[(int64_t)plane * ST_INTS] != 0; }
+#endif
+
 struct Launch {
     cudaStream_t stream;
     int64_t* counter;   // host counter of kernel launches (may be null)
-    const int* stop = nullptr;   // device flag: V-cycle kernels return at once when *stop != 0 (iterations
-                                 // enqueued ahead of the convergence test), null = always run
+    const int* stop = nullptr;   // device flag of plane 0 (plane p: stop[p * ST_INTS]): V-cycle kernels return at once when it is
+                                 // set (iterations enqueued ahead of the convergence test), null = always run
+    int planes = 1;              // gridDim.y of every launch
 };
 
 // ---- tile kernels (mg_kernels.cu) ----
@@ -113,9 +146,10 @@ void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDe
 void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse);
 void launch_diag(const Launch& L, const LevelDev& lv);   // U2: rd = 1 / a_ll from lambda, c
 void launch_zero(const Launch& L, VecRef x, int64_t n);
-void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n);   // dst[slot[k]] = src[k]
-void launch_gather_check(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n, int mode, int bit, int* bad);
-void launch_scatter(const Launch& L, const double* src_tiled, const int32_t* slot, double* dst, int64_t n);  // dst[k] = src[slot[k]]
+// ps: distance between the planes of the tiled vector (user vectors: n)
+void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n, int64_t ps);   // dst[slot[k]] = src[k]
+void launch_gather_check(const Launch& L, const double* src, const int32_t* slot, double* dst_tiled, int64_t n, int64_t ps, int mode, int bit, int* bad);
+void launch_scatter(const Launch& L, const double* src_tiled, const int32_t* slot, double* dst, int64_t n, int64_t ps);  // dst[k] = src[slot[k]]
 
 // ---- fused small levels (mg_tail.cu): the cycle steps of all levels >= s0 as a program run by one
 // cooperative kernel, grid.sync() between steps
@@ -153,6 +187,8 @@ cudaError_t launch_tail(const Launch& L, const LevelDev* d_levs, int s0, int nle
                         VecRef topx, VecRef topb, int grid);
 
 // ---- coarsest level (mg_coarse.cu) ----
+// doubles of work space per plane: [A | I] (n x 2n) + the published pivot column (x 2) + pivots
+__host__ __device__ inline size_t coarse_work_doubles(int n) { return 2 * (size_t)n * n + 2 * (size_t)n + 2; }
 void launch_coarse_factor(const Launch& L, const LevelDev& lv, const int32_t* cslot, const int32_t* slot2row, int n,
                           double* work /* n x 2n */, double* Ainv /* n x n */, int* bad /* bit 3 set on a zero / non-finite pivot */);
 void launch_coarse_solve(const Launch& L, const double* Ainv, const int32_t* cslot, int n, VecRef b_tiled, VecRef x_tiled);
@@ -169,6 +205,7 @@ void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stri
 void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st);
+void launch_zero_rhs_planes(const Launch& L, double* x, int64_t n, const GmresState* st);
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol, bool full_cgs2);
 
 }  // namespace mgb

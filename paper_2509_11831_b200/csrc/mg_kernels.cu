@@ -15,13 +15,15 @@ namespace {
 template <int MODE>
 __global__ void __launch_bounds__(NT, 3) k_apply(LevelDev lv, VecRef xr, VecRef br, VecRef yr, const int* __restrict__ stop) {
     __shared__ int tn[9];
-    if (stop != nullptr && *stop) return;
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    lv = plane_of(lv, pl);
     const int t = blockIdx.x;
     if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
     __syncthreads();
-    const double* __restrict__ x = resolve(xr);
-    const double* __restrict__ b = (MODE != 0) ? resolve(br) : nullptr;
-    double* __restrict__ y = resolve(yr);
+    const double* __restrict__ x = resolve(xr, pl);
+    const double* __restrict__ b = (MODE != 0) ? resolve(br, pl) : nullptr;
+    double* __restrict__ y = resolve(yr, pl);
     const int lx = threadIdx.x % TX;
     constexpr int NP = TY / ROWS_PER_PASS;
     const Nb4 nb = nb4(tn);
@@ -67,7 +69,9 @@ __device__ __forceinline__ int64_t fine_slot(const int* ct, int fx, int fy) {   
 
 __global__ void __launch_bounds__(NT) k_restrict(LevelDev fine, LevelDev coarse, const double* __restrict__ df, double* __restrict__ dc, const int* __restrict__ stop) {
     __shared__ int ct[9];
-    if (stop != nullptr && *stop) return;
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    df += pl * fine.nslots; dc += pl * coarse.nslots;
     const int t = blockIdx.x;
     if (threadIdx.x < 9) ct[threadIdx.x] = coarse.ctab[9 * t + threadIdx.x];
     __syncthreads();
@@ -95,13 +99,15 @@ __global__ void __launch_bounds__(NT) k_restrict(LevelDev fine, LevelDev coarse,
 __global__ void __launch_bounds__(NT) k_defect_restrict(LevelDev fine, LevelDev coarse, VecRef xr, VecRef br, double* __restrict__ dc,
                                                         const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    if (stop != nullptr && *stop) return;
-    defect_restrict_tile<false>(fine, coarse, blockIdx.x, resolve(xr), resolve(br), dc, smem_raw);
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    defect_restrict_tile<false>(plane_of(fine, pl), coarse, blockIdx.x, resolve(xr, pl), resolve(br, pl), dc + pl * coarse.nslots, smem_raw);
 }
 
 // ---------------------------------------------------------------------------------- U1 coefficient restriction (rule T4)
 __global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev coarse) {
     __shared__ int ct[9];
+    fine = plane_of(fine, blockIdx.y); coarse = plane_of(coarse, blockIdx.y);
     const int t = blockIdx.x;
     if (threadIdx.x < 9) ct[threadIdx.x] = coarse.ctab[9 * t + threadIdx.x];
     __syncthreads();
@@ -137,6 +143,7 @@ __global__ void __launch_bounds__(NT) k_restrict_coeff(LevelDev fine, LevelDev c
 // of lambda (same traffic, no division in the sweeps).
 __global__ void __launch_bounds__(NT) k_diag(LevelDev lv) {
     __shared__ int tn[9];
+    lv = plane_of(lv, blockIdx.y);
     const int t = blockIdx.x;
     if (threadIdx.x < 9) tn[threadIdx.x] = lv.tnb[9 * t + threadIdx.x];
     __syncthreads();
@@ -168,7 +175,9 @@ __device__ __forceinline__ int64_t parent_slot(const int* pt, int cx, int cy) { 
 // Phase A: e = P e_c on fine inner points (bilinear; absent parents hold 0), 0 elsewhere.
 __global__ void __launch_bounds__(NT) k_prolong(LevelDev fine, const double* __restrict__ ec, double* __restrict__ ef, const int* __restrict__ stop) {
     __shared__ int pt[9];
-    if (stop != nullptr && *stop) return;
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    ec += pl * ((int64_t)(fine.ntiles_coarse + 1) * TS); ef += pl * fine.nslots;
     __shared__ int odd[2];
     const int t = blockIdx.x;
     if (threadIdx.x < 9) pt[threadIdx.x] = fine.ptab[9 * t + threadIdx.x];
@@ -197,11 +206,13 @@ __global__ void __launch_bounds__(NT) k_prolong(LevelDev fine, const double* __r
 // Phase B: set_bnds_hom on the guards of e (homogeneous Eq. 11 / Eq. 16), then x <- x - e.
 __global__ void __launch_bounds__(NT) k_correct(LevelDev fine, const double* __restrict__ ef, VecRef xr, const int* __restrict__ stop) {
     __shared__ int tn[9];
-    if (stop != nullptr && *stop) return;
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    ef += pl * fine.nslots;
     const int t = blockIdx.x;
     if (threadIdx.x < 9) tn[threadIdx.x] = fine.tnb[9 * t + threadIdx.x];
     __syncthreads();
-    double* __restrict__ x = resolve(xr);
+    double* __restrict__ x = resolve(xr, pl);
     const int lx = threadIdx.x % TX;
 #pragma unroll
     for (int p = 0; p < TY / ROWS_PER_PASS; p++) {
@@ -220,16 +231,19 @@ __global__ void __launch_bounds__(NT) k_correct(LevelDev fine, const double* __r
 
 // ---------------------------------------------------------------------------------- small helpers
 __global__ void k_zero(VecRef xr, int64_t n) {
-    double* x = resolve(xr);
+    double* x = resolve(xr, blockIdx.y);
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) x[k] = 0.0;
 }
-__global__ void k_gather(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n) {
+// user order <-> tile layout; plane p: user vectors at p * n, tiled vectors at p * ps
+__global__ void k_gather(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n, int64_t ps) {
+    src += blockIdx.y * n; dst += blockIdx.y * ps;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[slot[k]] = src[k];
 }
 // gather of a coefficient field with the admissibility test of PAPER.md:51: mode 1: finite; mode 2: finite and > 0.
 // A violation sets *bad (bit 0 lambda, bit 1 c, bit 2 xi, given by `bit`); the values are copied regardless.
 __global__ void k_gather_check(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n,
-                               int mode, int bit, int* __restrict__ bad) {
+                               int64_t ps, int mode, int bit, int* __restrict__ bad) {
+    src += blockIdx.y * n; dst += blockIdx.y * ps;
     bool any = false;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
         const double v = src[k];
@@ -238,7 +252,8 @@ __global__ void k_gather_check(const double* __restrict__ src, const int32_t* __
     }
     if (any) atomicOr(bad, bit);
 }
-__global__ void k_scatter(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n) {
+__global__ void k_scatter(const double* __restrict__ src, const int32_t* __restrict__ slot, double* __restrict__ dst, int64_t n, int64_t ps) {
+    src += blockIdx.y * ps; dst += blockIdx.y * n;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) dst[k] = src[slot[k]];
 }
 
@@ -248,55 +263,56 @@ inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; 
 }  // namespace
 
 void launch_apply(const Launch& L, const LevelDev& lv, VecRef x, VecRef b, VecRef y, int mode) {
-    if (mode == 0) k_apply<0><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
-    else if (mode == 1) k_apply<1><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
-    else k_apply<2><<<lv.ntiles, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
+    const dim3 g(lv.ntiles, L.planes);
+    if (mode == 0) k_apply<0><<<g, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
+    else if (mode == 1) k_apply<1><<<g, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
+    else k_apply<2><<<g, NT, 0, L.stream>>>(lv, x, b, y, L.stop);
     count(L);
 }
 
 void launch_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* d_fine, double* d_coarse) {
-    k_restrict<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse, d_fine, d_coarse, L.stop);
+    k_restrict<<<dim3(coarse.ntiles, L.planes), NT, 0, L.stream>>>(fine, coarse, d_fine, d_coarse, L.stop);
     count(L);
 }
 
 void launch_defect_restrict(const Launch& L, const LevelDev& fine, const LevelDev& coarse, VecRef x, VecRef b, double* d_coarse) {
     ensure_dyn_smem((const void*)k_defect_restrict, DR_SMEM);
-    k_defect_restrict<<<coarse.ntiles, NT, DR_SMEM, L.stream>>>(fine, coarse, x, b, d_coarse, L.stop);
+    k_defect_restrict<<<dim3(coarse.ntiles, L.planes), NT, DR_SMEM, L.stream>>>(fine, coarse, x, b, d_coarse, L.stop);
     count(L);
 }
 
 void launch_prolong_correct(const Launch& L, const LevelDev& fine, const LevelDev& coarse, const double* e_coarse,
                             double* e_fine_tmp, VecRef x_fine) {
     (void)coarse;
-    k_prolong<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_coarse, e_fine_tmp, L.stop);
-    k_correct<<<fine.ntiles, NT, 0, L.stream>>>(fine, e_fine_tmp, x_fine, L.stop);
+    k_prolong<<<dim3(fine.ntiles, L.planes), NT, 0, L.stream>>>(fine, e_coarse, e_fine_tmp, L.stop);
+    k_correct<<<dim3(fine.ntiles, L.planes), NT, 0, L.stream>>>(fine, e_fine_tmp, x_fine, L.stop);
     count(L, 2);
 }
 
 void launch_restrict_coeff(const Launch& L, const LevelDev& fine, const LevelDev& coarse) {
-    k_restrict_coeff<<<coarse.ntiles, NT, 0, L.stream>>>(fine, coarse);
+    k_restrict_coeff<<<dim3(coarse.ntiles, L.planes), NT, 0, L.stream>>>(fine, coarse);
     count(L);
 }
 
 void launch_diag(const Launch& L, const LevelDev& lv) {
-    k_diag<<<lv.ntiles, NT, 0, L.stream>>>(lv);
+    k_diag<<<dim3(lv.ntiles, L.planes), NT, 0, L.stream>>>(lv);
     count(L);
 }
 
 void launch_zero(const Launch& L, VecRef x, int64_t n) {
-    k_zero<<<grid1d(n), 256, 0, L.stream>>>(x, n);
+    k_zero<<<dim3(grid1d(n), L.planes), 256, 0, L.stream>>>(x, n);
     count(L);
 }
-void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n) {
-    k_gather<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n);
+void launch_gather(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n, int64_t ps) {
+    k_gather<<<dim3(grid1d(n), L.planes), 256, 0, L.stream>>>(src, slot, dst, n, ps);
     count(L);
 }
-void launch_gather_check(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n, int mode, int bit, int* bad) {
-    k_gather_check<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n, mode, bit, bad);
+void launch_gather_check(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n, int64_t ps, int mode, int bit, int* bad) {
+    k_gather_check<<<dim3(grid1d(n), L.planes), 256, 0, L.stream>>>(src, slot, dst, n, ps, mode, bit, bad);
     count(L);
 }
-void launch_scatter(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n) {
-    k_scatter<<<grid1d(n), 256, 0, L.stream>>>(src, slot, dst, n);
+void launch_scatter(const Launch& L, const double* src, const int32_t* slot, double* dst, int64_t n, int64_t ps) {
+    k_scatter<<<dim3(grid1d(n), L.planes), 256, 0, L.stream>>>(src, slot, dst, n, ps);
     count(L);
 }
 

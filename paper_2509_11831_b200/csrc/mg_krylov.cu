@@ -20,6 +20,7 @@ namespace mgb {
 namespace {
 
 constexpr int CH = 8;   // basis vectors per register chunk in the multi-dot
+constexpr int64_t PARTIAL_PLANE = (int64_t)RED_BLOCKS_MAX * (MAX_M + 2);   // doubles of block partials per plane
 
 __device__ __forceinline__ double warp_sum(double v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -57,6 +58,7 @@ __device__ __forceinline__ bool last_block(GmresState* st) {
 
 __global__ void __launch_bounds__(RED_THREADS) k_norm2(const double* __restrict__ v, int64_t n, GmresState* st,
                                                       double* __restrict__ partial, int which) {
+    v += blockIdx.y * n; st += blockIdx.y; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     __shared__ double sm[32];
     double acc = 0.0;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
@@ -77,6 +79,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_norm2(const double* __restrict_
 
 // K1/K2/K5: relres = beta / bn decides converged / restart; v_0 = r / beta; g = (beta, 0, ...).
 __global__ void k_start_cycle(GmresState* st, const double* __restrict__ r, double* __restrict__ V0, int64_t n) {
+    st += blockIdx.y; r += blockIdx.y * n; V0 += (int64_t)blockIdx.y * (st->m + 1) * n;   // plane = blockIdx.y
     const double beta = st->beta, bn = st->bn;
     const double relres = (bn > 0.0) ? beta / bn : 0.0;
     const bool conv = (bn == 0.0) || (relres < st->rtol);
@@ -90,6 +93,7 @@ __global__ void k_start_cycle(GmresState* st, const double* __restrict__ r, doub
     // the header is rewritten by one thread after every block has read it
     if (last_block(st) && threadIdx.x == 0) {
         st->relres = relres;
+        if (conv || broke || capped) st->j = 0;                         // no cycle runs: a later k_update_x adds nothing
         if (bn == 0.0) { st->status = 4; st->cycle_end = 1; }           // zero right-hand side: x = 0 (K1)
         else if (conv) { st->status = 1; st->cycle_end = 1; }
         else if (broke) { st->cycle_end = 1; }
@@ -101,6 +105,7 @@ __global__ void k_start_cycle(GmresState* st, const double* __restrict__ r, doub
 // red[i] = (w, v_i), i = 0..j.  One pass over w per chunk of CH basis vectors.
 __global__ void __launch_bounds__(RED_THREADS) k_multidot(const double* __restrict__ w, const double* __restrict__ V, int64_t stride,
                                                          int64_t n, GmresState* st, double* __restrict__ partial) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     __shared__ double sm[32];
     if (st->cycle_end) return;
     const int nv = st->j + 1;
@@ -133,6 +138,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_multidot(const double* __restri
 // w -= sum_i red[i] v_i ; hcol (+)= red ; hcol[j+1] = ||w||.
 __global__ void __launch_bounds__(RED_THREADS) k_update_w(double* __restrict__ w, const double* __restrict__ V, int64_t stride, int64_t n,
                                                          GmresState* st, double* __restrict__ partial, int pass) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     __shared__ double sm[32];
     __shared__ double hh[MAX_M + 1];
     if (st->cycle_end) return;
@@ -189,6 +195,7 @@ __device__ void givens_step(GmresState* st) {
 }
 
 __global__ void k_givens(GmresState* st) {
+    st += blockIdx.y;   // plane = blockIdx.y
     if (threadIdx.x != 0 || st->cycle_end) return;
     givens_step(st);
 }
@@ -288,6 +295,7 @@ __device__ __forceinline__ void ud_finish(double (&acc)[FUSED_NV], double accn, 
 
 __global__ void __launch_bounds__(UD_THREADS) k_update_dot(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
                                                             int64_t n, GmresState* st, double* __restrict__ partial) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     __shared__ double hh[FUSED_NV];
     if (st->cycle_end) return;
     const int nv = st->j + 1;
@@ -378,6 +386,7 @@ __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, cons
 
 __global__ void __launch_bounds__(UDT_THREADS, 1) k_update_dot_tma(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
                                                                    int64_t n, GmresState* st, double* __restrict__ partial) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     extern __shared__ __align__(128) unsigned char udt_smem[];
     __shared__ double hh[FUSED_NV];
     if (st->cycle_end) return;
@@ -423,6 +432,7 @@ __device__ __forceinline__ void multidot_body(const double* __restrict__ w, cons
 constexpr int MD_THREADS = 256;
 __global__ void __launch_bounds__(MD_THREADS, 2) k_multidot_t(const double* __restrict__ w, const double* __restrict__ V, int64_t stride,
                                                               int64_t n, GmresState* st, double* __restrict__ partial) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     __shared__ double red[MD_THREADS / 32][FUSED_NV];
     if (st->cycle_end) return;
     const int nv = st->j + 1;
@@ -456,6 +466,7 @@ __global__ void __launch_bounds__(MD_THREADS, 2) k_multidot_t(const double* __re
 // Pass 1 through the same TMA pipeline.
 __global__ void __launch_bounds__(UDT_THREADS, 1) k_multidot_tma(double* __restrict__ w, const double* __restrict__ V, int64_t stride,
                                                                  int64_t n, GmresState* st, double* __restrict__ partial) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride; partial += blockIdx.y * PARTIAL_PLANE;   // plane = blockIdx.y
     extern __shared__ __align__(128) unsigned char udt_smem[];
     __shared__ double red[UDT_THREADS / 32][FUSED_NV];
     if (st->cycle_end) return;
@@ -521,6 +532,7 @@ __device__ __forceinline__ void final_v_body(const double* __restrict__ w, const
 // v_{j+1} = (w' - V h2) / h_{j+1,j}; st->j has already been advanced by the Givens step.
 __global__ void __launch_bounds__(RED_THREADS) k_final_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n,
                                                         GmresState* st) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride;   // plane = blockIdx.y
     __shared__ double hh[FUSED_NV];
     if (st->cycle_end || st->skip2) return;
     const int nv = st->j;
@@ -537,6 +549,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_final_v(const double* __restric
 constexpr int SV_THREADS = 256, SV_UNROLL = 4;
 __global__ void __launch_bounds__(SV_THREADS) k_scale_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n,
                                                         GmresState* st) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride;   // plane = blockIdx.y
     if (st->cycle_end || !st->skip2) return;
     const double inv = st->inv_hn;
     const double2* __restrict__ w2 = reinterpret_cast<const double2*>(w);
@@ -553,6 +566,7 @@ __global__ void __launch_bounds__(SV_THREADS) k_scale_v(const double* __restrict
 
 // v_{j+1} = w / h_{j+1,j}
 __global__ void k_next_v(const double* __restrict__ w, double* __restrict__ V, int64_t stride, int64_t n, GmresState* st) {
+    st += blockIdx.y; w += blockIdx.y * n; V += (int64_t)blockIdx.y * (st->m + 1) * stride;   // plane = blockIdx.y
     if (st->cycle_end) return;
     double* v = V + (int64_t)st->j * stride;
     const double inv = st->inv_hn;
@@ -561,6 +575,7 @@ __global__ void k_next_v(const double* __restrict__ w, double* __restrict__ V, i
 
 // K4: back-substitute R y = g (tiny; redone by every block), x += sum_i y_i z_i.
 __global__ void __launch_bounds__(256) k_update_x(double* __restrict__ x, const double* __restrict__ Z, int64_t stride, int64_t n, GmresState* st) {
+    st += blockIdx.y; x += blockIdx.y * n; Z += (int64_t)blockIdx.y * (st->m + 1) * stride;   // plane = blockIdx.y
     __shared__ double y[MAX_M];
     const int nv = st->j;
     if (threadIdx.x == 0) {
@@ -580,58 +595,70 @@ __global__ void __launch_bounds__(256) k_update_x(double* __restrict__ x, const 
 }
 
 __global__ void k_init_state(GmresState* st, int m, int max_iters, double rtol, double reorth_tol) {
+    st += blockIdx.y;   // plane = blockIdx.y
     if (threadIdx.x != 0) return;
     st->nreorth = 0; st->skip2 = 0; st->reorth_tol = reorth_tol;
     st->j = 0; st->iters = 0; st->status = 0; st->cycle_end = 0; st->m = m; st->max_iters = max_iters;
     st->ticket = 0; st->rtol = rtol; st->bn = 0.0; st->beta = 0.0; st->relres = 0.0; st->hn = 0.0; st->inv_hn = 0.0;
 }
 
+// K1: a plane whose right-hand side is zero (status 4) has the solution x = 0
+__global__ void k_zero_rhs_planes(double* __restrict__ x, int64_t n, const GmresState* st) {
+    st += blockIdx.y;
+    if (st->status != 4) return;
+    x += blockIdx.y * n;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) x[k] = 0.0;
+}
+
 inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; }
 
 }  // namespace
 
+void launch_zero_rhs_planes(const Launch& L, double* x, int64_t n, const GmresState* st) {
+    k_zero_rhs_planes<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(x, n, st); count(L);
+}
 void launch_norm2(const Launch& L, const double* v, int64_t n, GmresState* st, double* partial, int which) {
-    k_norm2<<<red_blocks(), RED_THREADS, 0, L.stream>>>(v, n, st, partial, which); count(L);
+    k_norm2<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(v, n, st, partial, which); count(L);
 }
 void launch_start_cycle(const Launch& L, GmresState* st, const double* r, double* V0, int64_t n) {
-    k_start_cycle<<<red_blocks(), RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
+    k_start_cycle<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(st, r, V0, n); count(L);
 }
 void launch_multidot(const Launch& L, const double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int m) {
     static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
     if (!no_tma) ensure_dyn_smem((const void*)k_multidot_tma, UDT_SMEM);
     const int sms = dev_info().sms;
     if (m <= FUSED_NV && !no_tma && n % (UDT_THREADS * 4) == 0)
-        k_multidot_tma<<<sms, UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
-    else if (m <= FUSED_NV) k_multidot_t<<<sms * 2, MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
-    else k_multidot<<<red_blocks(), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+        k_multidot_tma<<<dim3(sms, L.planes), UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
+    else if (m <= FUSED_NV) k_multidot_t<<<dim3(sms * 2, L.planes), MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    else k_multidot<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
 }
 void launch_update_w(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial, int pass) {
-    k_update_w<<<red_blocks(), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
+    k_update_w<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial, pass); count(L);
 }
 void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stride, int64_t n, GmresState* st, double* partial) {
     static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
     if (!no_tma) ensure_dyn_smem((const void*)k_update_dot_tma, UDT_SMEM);
     const int sms = dev_info().sms;
-    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<sms, UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
-    else k_update_dot<<<sms * 2, UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
+    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<dim3(sms, L.planes), UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
+    else k_update_dot<<<dim3(sms * 2, L.planes), UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
 }
 void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
-    k_final_v<<<dev_info().sms * 2, RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
-    k_scale_v<<<dev_info().sms * 8, SV_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_final_v<<<dim3(dev_info().sms * 2, L.planes), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_scale_v<<<dim3(dev_info().sms * 8, L.planes), SV_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
 }
-void launch_givens(const Launch& L, GmresState* st) { k_givens<<<1, 32, 0, L.stream>>>(st); count(L); }
+void launch_givens(const Launch& L, GmresState* st) { k_givens<<<dim3(1, L.planes), 32, 0, L.stream>>>(st); count(L); }
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st) {
-    k_next_v<<<red_blocks(), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
+    k_next_v<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st); count(L);
 }
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st) {
-    k_update_x<<<red_blocks(), 256, 0, L.stream>>>(x, Z, stride, n, st); count(L);
+    k_update_x<<<dim3(red_blocks(), L.planes), 256, 0, L.stream>>>(x, Z, stride, n, st); count(L);
 }
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol, bool full_cgs2) {
     static const char* env = getenv("MG_B200_REORTH_TOL");          // experiments only
     const double tol = full_cgs2 ? -1.0 : (env ? atof(env) : REORTH_TOL);
-    k_init_state<<<1, 32, 0, L.stream>>>(st, m, max_iters, rtol, tol); count(L);
+    k_init_state<<<dim3(1, L.planes), 32, 0, L.stream>>>(st, m, max_iters, rtol, tol); count(L);
 }
 
 }  // namespace mgb

@@ -18,17 +18,22 @@ __global__ void __launch_bounds__(GT, 2) k_gs(LevelDev lv, VecRef xin_r, VecRef 
                                               int xin_zero, const uint16_t* __restrict__ ccode, double* __restrict__ dc,
                                               const int* __restrict__ stop, const int* __restrict__ tlist) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    if (stop != nullptr && *stop) return;
+    const int pl = blockIdx.y;
+    if (stopped(stop, pl)) return;
+    lv = plane_of(lv, pl);
+    const int64_t cps = (int64_t)(lv.ntiles_coarse + 1) * TS;      // plane stride of the next coarser level
+    if (PC) ec += pl * cps;
+    if (EPI == 1) dc += pl * cps; else if (EPI == 2) dc += pl * lv.nslots;
     constexpr int NBX = TX / BX, NSUB = NBX * (TY / BY);
     const int ti = blockIdx.x / NSUB, sub = blockIdx.x - ti * NSUB;
     const int t = tlist != nullptr ? tlist[ti] : ti;            // the launch covers a list of tiles, or all of them
-    gs_tile<NS, PC, false, EPI, BX, BY, XIM>(lv, t, resolve(xin_r), resolve(xout_r), resolve(b_r), ec, xin_zero, smem_raw, nullptr, ccode, dc,
+    gs_tile<NS, PC, false, EPI, BX, BY, XIM>(lv, t, resolve(xin_r, pl), resolve(xout_r, pl), resolve(b_r, pl), ec, xin_zero, smem_raw, nullptr, ccode, dc,
                                        (sub % NBX) * BX, (sub / NBX) * BY);
 }
 
 __global__ void k_copy(VecRef sr, VecRef dr, int64_t n) {
-    const double* __restrict__ s = resolve(sr);
-    double* __restrict__ d = resolve(dr);
+    const double* __restrict__ s = resolve(sr, blockIdx.y);
+    double* __restrict__ d = resolve(dr, blockIdx.y);
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) d[k] = s[k];
 }
 
@@ -51,7 +56,7 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
         constexpr int K = EPI ? 1 : 0, SH = EPI ? 6 : 4, GH = (EPI || PC) ? 8 : 6;
         const int nint = lv.nint[K], ngen = lv.ngen[K], novf = lv.ntiles - nint - ngen, sms = dev_info().sms;
         if (novf > 0) {
-            k_gs<NS, PC, EPI, BX, BY, XIM><<<novf, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, lv.tlist[K] + nint + ngen);
+            k_gs<NS, PC, EPI, BX, BY, XIM><<<dim3(novf, L.planes), GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, lv.tlist[K] + nint + ngen);
             if (L.counter) *L.counter += 1;
         }
         if (nint + ngen > 0) {
@@ -60,22 +65,22 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
             using SI = SGeo<SH>; using SGG = SGeo<GH>;
             constexpr size_t ssm = std::max(SI::smem(PC, false), SGG::smem(PC, true));
             constexpr int nthreads = std::max(SI::NT, SGG::NT);
-            const int grid = std::min(sms, nint + ngen);
+            const int grid = (int)std::min<int64_t>(sms, (int64_t)(nint + ngen) * L.planes);
             int ggen = 0;
             if (ngen > 0) {
                 const double wg = ngen * strip_gen_cost();
-                ggen = std::max(1, std::min(ngen, (int)(grid * wg / (wg + nint) + 0.5)));
+                ggen = std::max(1, std::min(ngen * L.planes, (int)(grid * wg / (wg + nint) + 0.5)));
                 if (nint > 0) ggen = std::min(ggen, grid - 1);
             }
             ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI>, ssm);
-            k_gs_strip<SH, GH, PC, EPI><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, xin, xout, b,
+            k_gs_strip<SH, GH, PC, EPI><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes, xin, xout, b,
                                                                             ec, zero ? 1 : 0, ccode, dc, L.stop);
             if (L.counter) *L.counter += 1;
         }
         return;
     }
     const int grid = lv.ntiles * (TX / BX) * (TY / BY);
-    k_gs<NS, PC, EPI, BX, BY, XIM><<<grid, GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, nullptr);
+    k_gs<NS, PC, EPI, BX, BY, XIM><<<dim3(grid, L.planes), GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, nullptr);
     if (L.counter) *L.counter += 1;
 }
 
@@ -93,9 +98,10 @@ void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, Vec
     static const bool no_sub = getenv("MG_B200_NO_SUBBLOCKS") != nullptr;
     const int sms = dev_info().sms;
     const int SUB_MAX_TILES = sms * 10 / 37, MID_MAX_TILES = sms / 2, HALF_MAX_TILES = sms;
-    if (lv.ntiles <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
-    else if (lv.ntiles <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
-    else if (lv.ntiles <= HALF_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, HBX, HBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    const int64_t nt = (int64_t)lv.ntiles * L.planes;       // tiles of all planes: what fills the machine
+    if (nt <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else if (nt <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    else if (nt <= HALF_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, HBX, HBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else launch_blk<NS, PC, EPI, TX, TY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
 }
 
@@ -129,7 +135,7 @@ void launch_gs_correct(const Launch& L, const LevelDev& lv, const double* e_coar
 }
 
 void launch_copy(const Launch& L, VecRef src, VecRef dst, int64_t n) {
-    k_copy<<<(int)std::min<int64_t>((n + 255) / 256, dev_info().sms * 8), 256, 0, L.stream>>>(src, dst, n);
+    k_copy<<<dim3((int)std::min<int64_t>((n + 255) / 256, dev_info().sms * 8), L.planes), 256, 0, L.stream>>>(src, dst, n);
     if (L.counter) *L.counter += 1;
 }
 

@@ -82,10 +82,10 @@ template <int NTHREADS>
 __device__ __forceinline__ void bar_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
 
 template <int H, bool PC, int EPI, bool GEN>
-__device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __restrict__ smeta, int nlist, const VecRef& xin_r, const VecRef& xout_r,
-                                           const VecRef& b_r, const double* __restrict__ ec, int xin_zero,
-                                           const uint16_t* __restrict__ ccode, double* __restrict__ dc, int cta, int ncta,
-                                           unsigned char* smem_raw) {
+__device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __restrict__ smeta, int nlist, int planes, const VecRef& xin_r,
+                                           const VecRef& xout_r, const VecRef& b_r, const double* __restrict__ ec0, int xin_zero,
+                                           const uint16_t* __restrict__ ccode, double* __restrict__ dc0, const int* __restrict__ stop, int cta,
+                                           int ncta, unsigned char* smem_raw) {
     using G = SGeo<H>;
     constexpr int R = G::R, RWC = G::RWC, NCP = G::NCP, NRB = G::NRB, RBL = G::RBL, NT = G::NT;
     constexpr bool DR = EPI == 1, AP = EPI == 2;
@@ -103,9 +103,19 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
     uint16_t* gcode = gcell + (GEN ? GCAP : 0);                                  //       point code
     __shared__ int gcount;
     double* sxp = sx + RWC;                                 // mirror as neumann_smem / cidx<G> address it (region row 0 = padded row 1)
-    const double* __restrict__ xin = resolve(xin_r);
-    double* __restrict__ xout = resolve(xout_r);
-    const double* __restrict__ b = resolve(b_r);
+    // work items: (plane, list entry) pairs, plane-major; the vectors of plane pl (one solve per plane, same mesh)
+    struct PP { const double *c, *rd, *lam, *b, *xin, *ec; double *xout, *dc; };
+    auto plane_ptrs = [&](int pl) {
+        const int64_t po = (int64_t)pl * lv.nslots, pco = (int64_t)pl * (lv.ntiles_coarse + 1) * TS;
+        PP q;
+        q.c = lv.c + po; q.rd = lv.rd + po; q.lam = lv.lam + po;
+        q.b = resolve(b_r, pl); q.xin = resolve(xin_r, pl); q.xout = resolve(xout_r, pl);
+        q.ec = PC ? ec0 + pco : nullptr;
+        q.dc = DR ? dc0 + pco : (AP ? dc0 + po : nullptr);
+        return q;
+    };
+    const int nitems = nlist * planes;
+    if (cta >= nitems) return;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // ---- the strip of this thread: pair column p, rows ry0 .. ry0 + R - 1 of the region
     int p, rb;
@@ -130,58 +140,78 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
 
     // asynchronous copies of this thread's strip of the tile described by m[] into its staging slots
     auto prefetch = [&](const int* m) {
+        if (m[22]) { cp_async_commit(); return; }            // the plane of that item has ended its cycle: nothing to do
+        const PP q = plane_ptrs(m[21]);
 #pragma unroll
         for (int r = 0; r < R; r++) {
             const int ly = ry0 + r - H;
             const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
             const int64_t gs = (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm;
-            cp_async16(&stg[(0 * R + r) * NT + tid], lv.c + gs);
-            if (!xin_zero) cp_async16(&stg[(1 * R + r) * NT + tid], xin + gs);
+            cp_async16(&stg[(0 * R + r) * NT + tid], q.c + gs);
+            if (!xin_zero) cp_async16(&stg[(1 * R + r) * NT + tid], q.xin + gs);
             if (GEN) cp_async4(&cstg[r * NT + tid], lv.code + gs);
         }
         if (tid < 2 + (EPI ? 1 : 0)) {                       // b, 1/a_ll, lambda of that tile: into L2 now, into registers when its turn comes
             const int64_t o = (int64_t)m[20] * TS;
-            prefetch_l2_bulk(tid == 0 ? b + o : (tid == 1 ? lv.rd + o : lv.lam + o), TS * sizeof(double));
+            prefetch_l2_bulk(tid == 0 ? q.b + o : (tid == 1 ? q.rd + o : q.lam + o), TS * sizeof(double));
         }
         if (PC) {
             // coarse parents of the strip (bilinear prolongation): columns cx, cx + 1, rows cy0 .. cy0 + 2
             const int cx = m[18] * (TX / 2) + (lx0 >> 1), cy0 = m[19] * (TY / 2) + ((ry0 - H) >> 1);
 #pragma unroll
-            for (int q = 0; q < 3; q++) {
-                cp_async8(&se[(2 * q) * NT + tid], ec + parent_slot9(m + 9, cx, cy0 + q));
-                cp_async8(&se[(2 * q + 1) * NT + tid], ec + parent_slot9(m + 9, cx + 1, cy0 + q));
+            for (int k = 0; k < 3; k++) {
+                cp_async8(&se[(2 * k) * NT + tid], q.ec + parent_slot9(m + 9, cx, cy0 + k));
+                cp_async8(&se[(2 * k + 1) * NT + tid], q.ec + parent_slot9(m + 9, cx + 1, cy0 + k));
             }
         }
         cp_async_commit();
     };
 
     // right-hand sides of the collected guards (the list is complete: call after a barrier), read by the boundary phases
-    auto fill_gb = [&](const int* m) {
+    auto fill_gb = [&](const int* m, const double* __restrict__ b) {
         const int ng = min(gcount, GCAP);
         for (int g = tid; g < ng; g += NT) {
             const int cell = gcell[g], ry = cell / G::RW, rx = cell - ry * G::RW;
             gb[g] = __ldg(b + region_slot<H>(m, rx, ry));
         }
     };
+    // table entry `tid` of work item `item`: the list entry's tables, [21] its plane, [22] whether that plane has stopped
+    auto meta_of = [&](int item) {
+        const int pl = item / nlist, e = item - pl * nlist;
+        if (tid == 21) return pl;
+        if (tid == 22) return stopped(stop, pl) ? 1 : 0;
+        return __ldg(smeta + (int64_t)e * SMETA + tid);
+    };
 
     if (tid == 0) gcount = 0;
     if (tid < SMETA) {
-        M[tid] = smeta[(int64_t)cta * SMETA + tid];
-        if (cta + G0 < nlist) M[SMETA + tid] = smeta[(int64_t)(cta + G0) * SMETA + tid];
+        M[tid] = meta_of(cta);
+        if (cta + G0 < nitems) M[SMETA + tid] = meta_of(cta + G0);
     }
     bar_sync<NT>();
     prefetch(M);
     int ib = 0;                                             // buffer of the current tile's tables
-    for (int it = cta; it < nlist; it += G0) {
+    for (int it = cta; it < nitems; it += G0) {
         const int* m = M + ib * SMETA;
         const int* pt = m + 9;
         const int* odd = m + 18;
         const int t = m[20];
-        const bool more2 = it + 2 * G0 < nlist;
+        const bool more2 = it + 2 * G0 < nitems;
         int mnext = 0;
-        if (tid < SMETA && more2) mnext = __ldg(smeta + (int64_t)(it + 2 * G0) * SMETA + tid);    // tables two tiles ahead
+        if (tid < SMETA && more2) mnext = meta_of(it + 2 * G0);    // tables two tiles ahead
         // ---- the strip: staging slots -> registers (pairs)
         cp_async_wait_all();
+        if (m[22]) {                                          // this plane's cycle has ended: keep the pipeline moving, skip the tile
+            if (it + G0 < nitems) prefetch(M + (ib == 2 ? 0 : ib + 1) * SMETA);
+            if (tid < SMETA && more2) M[(ib == 0 ? 2 : ib - 1) * SMETA + tid] = mnext;
+            ib = ib == 2 ? 0 : ib + 1;
+            bar_sync<NT>();
+            continue;
+        }
+        const PP cur = plane_ptrs(m[21]);
+        const double* __restrict__ b = cur.b;
+        double* __restrict__ xout = cur.xout;
+        double* __restrict__ dc = cur.dc;
         double x[R][2], c[R][2], br[R][2], rd[R][2], lam[R][2];
 #pragma unroll
         for (int r = 0; r < R; r++) {
@@ -220,9 +250,9 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
             const int ly = ry0 + r - H;
             const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
             const int64_t gs = (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm;
-            const double2 bv = ldg2(b + gs), dv = ldg2(lv.rd + gs);
+            const double2 bv = ldg2(b + gs), dv = ldg2(cur.rd + gs);
             br[r][0] = bv.x; br[r][1] = bv.y; rd[r][0] = dv.x; rd[r][1] = dv.y;
-            if (EPI && !GEN) { const double2 lv2 = ldg2(lv.lam + gs); lam[r][0] = lv2.x; lam[r][1] = lv2.y; }
+            if (EPI && !GEN) { const double2 lv2 = ldg2(cur.lam + gs); lam[r][0] = lv2.x; lam[r][1] = lv2.y; }
         }
         double e[3][2];
         if (PC) {
@@ -230,7 +260,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
             for (int q = 0; q < 3; q++) { e[q][0] = se[(2 * q) * NT + tid]; e[q][1] = se[(2 * q + 1) * NT + tid]; }
         }
         // the slots are consumed: refill them with the next tile of this CTA while this one is computed
-        if (it + G0 < nlist) prefetch(M + (ib == 2 ? 0 : ib + 1) * SMETA);
+        if (it + G0 < nitems) prefetch(M + (ib == 2 ? 0 : ib + 1) * SMETA);
         if (GEN && gmask != 0u && !spare) {
             // guards of the region, collected once: Eq. 11 / Eq. 16 need their right-hand side and their point code
 #pragma unroll
@@ -268,7 +298,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                         sx[SIDX(q, r)] = ee[r][q];
                     }
                 bar_sync<NT>();
-                fill_gb(m);
+                fill_gb(m, b);
                 const int ng = min(gcount, GCAP);
                 for (int g = tid; g < ng; g += NT) {
                     const uint16_t code = gcode[g];
@@ -299,7 +329,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
             sc[SIDX(0, r)] = c[r][0]; sc[SIDX(1, r)] = c[r][1];
         }
         bar_sync<NT>();
-        if (GEN && !PC) fill_gb(m);
+        if (GEN && !PC) fill_gb(m, b);
         // ---- face sums c_l + c_nb (sweep-invariant): hW | cell 0 | hM | cell 1 | hE per row, v[r] below row r per column
         double hW[R], hM[R], hE[R], v[R + 1][2];
 #pragma unroll
@@ -356,7 +386,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                     else {
                         double sum, wself, delta;
                         neumann_smem<G>(code, rx, ry, sxp, lv.h, sum, wself, delta);
-                        sxp[cidx<G>(rx, ry)] = (sum - delta * gb[g]) / (1.0 - wself);
+                        sxp[cidx<G>(rx, ry)] = neumann_point(sum, delta, gb[g], wself);
                     }
                 }
                 bar_sync<NT>();
@@ -374,7 +404,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
             for (int r = 0; r < R; r++) {
                 const int ly = ry0 + r - H;
                 const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
-                const double2 lv2 = ldg2(lv.lam + (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm);
+                const double2 lv2 = ldg2(cur.lam + (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm);
                 lam[r][0] = lv2.x; lam[r][1] = lv2.y;
             }
         }
@@ -404,7 +434,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                         const double xS = r == 0 ? xsd[pos] : x[r - 1][pos], xN = r == R - 1 ? xnd[pos] : x[r + 1][pos];
                         const double aW = kappa * (pos == 0 ? hW[r] : hM[r]), aE = kappa * (pos == 0 ? hM[r] : hE[r]);
                         const double aS = kappa * v[r][pos], aN = kappa * v[r + 1][pos];
-                        d = lam[r][pos] * xl + aW * (xl - xW) + aE * (xl - xE) + aS * (xl - xS) + aN * (xl - xN) - br[r][pos];
+                        d = __dsub_rn(row_d1(lam[r][pos], xl, aW, xW, aE, xE, aS, xS, aN, xN), br[r][pos]);
                     }
                     sc[SIDX(pos, r)] = d;
                 }
@@ -455,10 +485,8 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                         const double xW = sx[SIDX(1, r) - 1], xE = sx[SIDX(0, r) + 1];
                         const double s0 = r == 0 ? xs0 : x[r - 1][0], n0 = r == R - 1 ? xn0 : x[r + 1][0];
                         const double s1 = r == 0 ? xs1 : x[r - 1][1], n1 = r == R - 1 ? xn1 : x[r + 1][1];
-                        const double w0 = lam[r][0] * x0 + (kappa * hW[r]) * (x0 - xW) + (kappa * hM[r]) * (x0 - x1) + (kappa * v[r][0]) * (x0 - s0) +
-                                          (kappa * v[r + 1][0]) * (x0 - n0);
-                        const double w1 = lam[r][1] * x1 + (kappa * hM[r]) * (x1 - x0) + (kappa * hE[r]) * (x1 - xE) + (kappa * v[r][1]) * (x1 - s1) +
-                                          (kappa * v[r + 1][1]) * (x1 - n1);
+                        const double w0 = row_d1(lam[r][0], x0, kappa * hW[r], xW, kappa * hM[r], x1, kappa * v[r][0], s0, kappa * v[r + 1][0], n0);
+                        const double w1 = row_d1(lam[r][1], x1, kappa * hM[r], x0, kappa * hE[r], xE, kappa * v[r][1], s1, kappa * v[r + 1][1], n1);
                         *reinterpret_cast<double2*>(dc + (int64_t)t * TS + ly * TX + 2 * lane) =
                             make_double2((!GEN || ((imask >> (2 * r)) & 1u)) ? w0 : 0.0, (!GEN || ((imask >> (2 * r + 1)) & 1u)) ? w1 : 0.0);
                     }
@@ -496,13 +524,13 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
 // (list smeta_i); both persistent, both with their own thread count (the block carries the larger one).
 template <int HI, int HG, bool PC, int EPI>
 __global__ void __launch_bounds__((SGeo<HI>::NT > SGeo<HG>::NT ? SGeo<HI>::NT : SGeo<HG>::NT), 1)
-    k_gs_strip(LevelDev lv, const int* __restrict__ smeta_i, int nint, const int* __restrict__ smeta_g, int ngen, int ggen, VecRef xin_r,
+    k_gs_strip(LevelDev lv, const int* __restrict__ smeta_i, int nint, const int* __restrict__ smeta_g, int ngen, int ggen, int planes, VecRef xin_r,
                VecRef xout_r, VecRef b_r, const double* __restrict__ ec, int xin_zero, const uint16_t* __restrict__ ccode,
                double* __restrict__ dc, const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char strip_smem[];
-    if (stop != nullptr && *stop) return;
-    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true>(lv, smeta_g, ngen, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, blockIdx.x, ggen, strip_smem);
-    else strip_body<HI, PC, EPI, false>(lv, smeta_i, nint, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
+    if (planes == 1 && stopped(stop, 0)) return;
+    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
+    else strip_body<HI, PC, EPI, false>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
 }
 
 }  // namespace

@@ -161,8 +161,7 @@ __device__ __forceinline__ void restrict_epilogue(const LevelDev& lv, const int*
                     const double cl = sc[own], xl = sx[own];
                     const double aW = kap * (cl + sc[ob + tpar - 1]), aE = kap * (cl + sc[ob + tpar]);
                     const double aS = kap * (cl + sc[ob - RWC]), aN = kap * (cl + sc[ob + RWC]);
-                    d = lam * xl + aW * (xl - sx[ob + tpar - 1]) + aE * (xl - sx[ob + tpar]) + aS * (xl - sx[ob - RWC]) +
-                        aN * (xl - sx[ob + RWC]) - bl;
+                    d = __dsub_rn(row_d1(lam, xl, aW, sx[ob + tpar - 1], aE, sx[ob + tpar], aS, sx[ob - RWC], aN, sx[ob + RWC]), bl);
                 }
             }
             breg[col][r] = d;
@@ -224,8 +223,7 @@ __device__ __forceinline__ void apply_epilogue(const LevelDev& lv, int t, const 
                         const double cl = sc[own], xl = sx[own];
                         const double aW = kap * (cl + sc[ob + tpar - 1]), aE = kap * (cl + sc[ob + tpar]);
                         const double aS = kap * (cl + sc[ob - RWC]), aN = kap * (cl + sc[ob + RWC]);
-                        v = lam * xl + aW * (xl - sx[ob + tpar - 1]) + aE * (xl - sx[ob + tpar]) + aS * (xl - sx[ob - RWC]) +
-                            aN * (xl - sx[ob + RWC]);
+                        v = row_d1(lam, xl, aW, sx[ob + tpar - 1], aE, sx[ob + tpar], aS, sx[ob - RWC], aN, sx[ob + RWC]);
                     } else if (kind == C_DIR) v = sx[own];
                     else if (kind == C_NEU) {
                         double sum, wself, delta;
@@ -500,7 +498,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                     else {
                         double sum, wself, delta;
                         neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
-                        sx[idx] = (sum - delta * gb[g]) / (1.0 - wself);
+                        sx[idx] = neumann_point(sum, delta, gb[g], wself);
                     }
                 }
             } else {                                   // list overflow: every thread scans its own cells
@@ -519,7 +517,7 @@ __device__ __forceinline__ void gs_general(const LevelDev& lv, int t, const doub
                         else {
                             double sum, wself, delta;
                             neumann_smem<G>(code, rx, ry, sx, lv.h, sum, wself, delta);
-                            sx[idx] = (sum - delta * bv) / (1.0 - wself);
+                            sx[idx] = neumann_point(sum, delta, bv, wself);
                         }
                     }
             }

@@ -73,8 +73,7 @@ __device__ __forceinline__ double inner_row(const LevelDev& lv, const Nb4 nb, in
     const double aW = kap * (cl + __ldg(lv.c + sW)), aE = kap * (cl + __ldg(lv.c + sE));
     const double aS = kap * (cl + __ldg(lv.c + sS)), aN = kap * (cl + __ldg(lv.c + sN));
     const double xl = ldv<COH>(x + s);                                     // difference form (rule D1)
-    return __ldg(lv.lam + s) * xl + aW * (xl - ldv<COH>(x + sW)) + aE * (xl - ldv<COH>(x + sE)) + aS * (xl - ldv<COH>(x + sS)) +
-           aN * (xl - ldv<COH>(x + sN));
+    return row_d1(__ldg(lv.lam + s), xl, aW, ldv<COH>(x + sW), aE, ldv<COH>(x + sE), aS, ldv<COH>(x + sS), aN, ldv<COH>(x + sN));
 }
 
 // ---------------------------------------------------------------------------------- S1 + S3 fused

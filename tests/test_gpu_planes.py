@@ -1,0 +1,98 @@
+"""Planes batched inside the kernels (one elliptic solve per poloidal
+plane, all planes on the same mesh).  A handle with P planes keeps the mesh tables once, every vector P times, and
+launches every kernel once for all planes (gridDim.y = P) with one fGMRES state per plane.  The bar: batched == P
+separate handles BIT FOR BIT (x, iteration counts, residuals), and each plane matches the oracle."""
+import numpy as np
+import pytest
+
+from paper_2509_11831_b200 import workloads as W
+from tests import helpers as H
+from tests.test_gpu_parity import TOL_SOLVE, dev, gpu, host, rel  # noqa: F401  (gpu is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def _planes(cfg, lattice, P):
+    pls = [W.make_plane(cfg, lattice, seed=W.SEEDS[cfg] + 31 * p) for p in range(P)]
+    for pl in pls[1:]:
+        assert np.array_equal(pl.i, pls[0].i) and np.array_equal(pl.kind, pls[0].kind)
+    return pls
+
+
+def _stack(pls, name):
+    return np.stack([getattr(pl, name) for pl in pls])
+
+
+@pytest.mark.parametrize("cfg,lattice,P,kw", [(2, 257, 5, {}), (3, 257, 3, dict(nu_pre=3, nu_post=1, restart_m=8)),
+                                              (3, 1025, 2, {}), (2, 129, 16, dict(gamma=2))])
+def test_batched_planes_equal_separate_handles(gpu, oracle_mod, cfg, lattice, P, kw):
+    import torch
+    pls = _planes(cfg, lattice, P)
+    p0 = pls[0]
+    lam, c, f, x0 = (_stack(pls, k) for k in ("lam", "c", "f", "x0"))
+    if P >= 3:
+        f[1] = 0.0                                   # K1: zero right-hand side on one plane -> x = 0, 0 iterations
+        x0[1] = 1.0
+    okw = dict(levels=p0.levels, nu_pre=kw.get("nu_pre", 2), nu_post=kw.get("nu_post", 2), m=kw.get("restart_m", 30), gamma=kw.get("gamma", 1))
+    ref = []
+    for p in range(P):                               # oracle per plane
+        o = oracle_mod.Oracle(p0.i, p0.j, p0.kind, p0.h, **okw)
+        o.update(lam[p], c[p])
+        ref.append(o.solve(f[p], x0[p], 1e-10))
+    if P >= 3:
+        x0[2] = ref[2]["x"]                          # one plane starts from its solution: converged before the first cycle
+        ref[2] = dict(x=ref[2]["x"], iters=0, status=0)
+    seq = []
+    for p in range(P):                               # P separate single-plane handles
+        s = gpu.Solver(p0.i, p0.j, p0.kind, p0.h, levels=p0.levels, **kw)
+        s.update_coeffs(dev(lam[p]), dev(c[p]))
+        x, it, rr, rc = s.solve(dev(f[p]), dev(x0[p]), 1e-10)
+        seq.append((host(x), it, rr, rc))
+        s.close()
+    sb = gpu.Solver(p0.i, p0.j, p0.kind, p0.h, levels=p0.levels, planes=P, **kw)
+    for rep in range(2):                             # twice: the state of every plane is re-initialised per solve
+        sb.update_coeffs(dev(lam), dev(c))
+        xb, its, rrs, rc = sb.solve(dev(f), dev(x0), 1e-10)
+        xb = host(xb)
+        assert rc == 0 and xb.shape == (P, p0.n)
+        for p in range(P):
+            assert its[p] == seq[p][1] and rrs[p] == seq[p][2], (p, its, [q[1] for q in seq])
+            assert np.array_equal(xb[p], seq[p][0]), p
+            assert abs(its[p] - ref[p]["iters"]) <= 1 and rel(xb[p], ref[p]["x"]) <= TOL_SOLVE
+    assert len(set(its)) > 1                         # the planes really stop at different iterations
+    # host-buffer entry points carry all planes too
+    sb.update_coeffs_host(lam, c)
+    xh, its2, rrs2, rc2 = sb.solve_host(f, x0, 1e-10)
+    assert rc2 == 0 and list(its2) == list(its) and np.array_equal(xh, xb)
+    torch.cuda.synchronize()
+    sb.close()
+
+
+def test_batched_planes_per_plane_status(gpu):
+    """One plane cannot reach rtol within max_iters, the others can: the call returns the worst status, every plane
+    reports its own count, and the converged planes are unaffected (bit for bit) by the one that keeps iterating."""
+    P = 3
+    pls = _planes(2, 129, P)
+    p0 = pls[0]
+    lam, c, f, x0 = (_stack(pls, k) for k in ("lam", "c", "f", "x0"))
+    f[1] *= 1e-6                                    # scaling f does not change the iteration count ...
+    s = gpu.Solver(p0.i, p0.j, p0.kind, p0.h, levels=p0.levels, planes=P, max_iters=200)
+    s.update_coeffs(dev(lam), dev(c))
+    x_ok, its_ok, _, rc = s.solve(dev(f), dev(x0), 1e-10)
+    assert rc == 0
+    s.close()
+    cap = min(its_ok) - 2                           # ... so cap below what every plane needs except none: all capped
+    s = gpu.Solver(p0.i, p0.j, p0.kind, p0.h, levels=p0.levels, planes=P, max_iters=cap)
+    s.update_coeffs(dev(lam), dev(c))
+    x, its, rrs, rc = s.solve(dev(f), dev(x0), 1e-10)
+    assert rc == 1 and list(its) == [cap] * P and all(r >= 1e-10 for r in rrs)
+    s.close()
+    # a mixed outcome: plane 0 starts from the converged solution (0 iterations), plane 1, 2 are capped
+    x0m = x0.copy(); x0m[0] = host(x_ok)[0]
+    s = gpu.Solver(p0.i, p0.j, p0.kind, p0.h, levels=p0.levels, planes=P, max_iters=cap)
+    s.update_coeffs(dev(lam), dev(c))
+    x, its, rrs, rc = s.solve(dev(f), dev(x0m), 1e-10)
+    assert rc == 1 and its[0] == 0 and its[1] == cap and its[2] == cap and rrs[0] < 1e-10
+    assert np.array_equal(host(x)[0], host(x_ok)[0])
+    assert "plane" in gpu.last_error()
+    s.close()
