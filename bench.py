@@ -392,6 +392,74 @@ def run_planes(args):
         dist.destroy_process_group()
 
 
+def run_planes_batched(args):
+    """P planes of one mesh solved TOGETHER by one handle (mg_options.planes): mesh tables shared,
+    vectors [plane][slot], every kernel launched once for all planes, one fGMRES state per plane (PAPER.md:211, 256,
+    320-324).  Secondary bench line: HBM-resident inputs only."""
+    import torch
+    import torch.distributed as dist
+    from paper_2509_11831_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.use_torch_allocator()
+    P = args.planes
+    planes = [W.make_plane(args.config, args.lattice, seed=plane_seed(args.config, rank * P + p)) for p in range(P)]
+    p0 = planes[0]
+    dev = lambda name: torch.from_numpy(np.stack([getattr(pl, name) for pl in planes])).cuda()
+    lam, c, f, x0 = dev("lam"), dev("c"), dev("f"), dev("x0")
+    x = torch.empty_like(f)
+    s = B.Solver(p0.i, p0.j, p0.kind, p0.h, levels=p0.levels, planes=P)
+    its = None
+
+    def steps(k):
+        nonlocal its
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ev0.record()
+        tot = 0
+        for _ in range(k):
+            s.update_coeffs(lam, c)
+            _, its, rr, rc = s.solve(f, x0, args.rtol, x=x)
+            assert rc == 0, (rc, its, rr)
+            tot += sum(its)
+        ev1.record()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        return ev0.elapsed_time(ev1), tot
+
+    steps(args.warmup)
+    l1 = s.kernel_launches
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms_loc, tot = steps(args.steps)
+    clocks = sampler.stop() if sampler else None
+    ms, work, value = whole_job(ms_loc, float(p0.n * tot), world, "cuda")
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": WORKLOADS[args.config], "unknowns_per_plane": p0.n, "planes": P * world,
+                           "planes_per_gpu": P, "concurrency": "planes batched in the kernels (one handle, gridDim.y = planes)",
+                           "rtol": args.rtol, "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels,
+                           "step": "mg_update_coeffs + mg_solve on all planes"},
+                "iters": list(its), "ms_per_plane_solve": ms / args.steps / P, "clocks": clocks,
+                "gpu_launches": s.kernel_launches - l1, "launches_per_step": (s.kernel_launches - l1) / args.steps,
+                "e2e": None, "roofline": None, "cpu_baseline": None}
+        print(json.dumps(line))
+    s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_paper_mms(args):
     """The paper's own scaling experiment: annulus of Eq. 19-22, h halved from 4e-3 with one more
     level per refinement (4 ... 9 levels, N = 2.4e4 ... 2.4e7), V-cycle with five pre- and post-smoothing sweeps, stop at 1e-8,
@@ -453,14 +521,15 @@ def main():
     ap.add_argument("--paper-mms", type=int, default=0, metavar="R",
                     help="run the paper's annulus MMS scaling experiment over R refinements (6 reaches its 24 M points) instead")
     ap.add_argument("--three-field", action="store_true", help="secondary line: the paper's three-field form with a seeded xi (mg_update_coeffs3)")
-    ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved concurrently (secondary line, SURVEY.md 8(f) NEXT-1)")
+    ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved together by one batched handle (secondary line, SURVEY.md 8(f) NEXT-1)")
+    ap.add_argument("--plane-streams", action="store_true", help="with --planes: one handle + stream + host thread per plane instead of the batched handle")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
     elif args.paper_mms > 0:
         run_paper_mms(args)
     elif args.planes > 1:
-        run_planes(args)
+        run_planes(args) if args.plane_streams else run_planes_batched(args)
     else:
         run_ours(args)
 

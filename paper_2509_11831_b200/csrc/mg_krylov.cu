@@ -11,6 +11,7 @@
 // orthogonality defect is already below REORTH_TOL (k_scale_v instead); longer restarts use the plain four-pass
 // form (k_multidot, k_update_w twice, k_givens, k_next_v).  Grid reductions: per-block partials +
 // last-block-done ticket, summed in a fixed order (deterministic run to run).
+#include <algorithm>
 #include <cstdlib>
 
 #include "mg_device.h"
@@ -611,6 +612,10 @@ __global__ void k_zero_rhs_planes(double* __restrict__ x, int64_t n, const Gmres
 }
 
 inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; }
+// CTAs per plane of the TMA-staged passes: one per SM, fewer for short vectors so that every CTA streams at least four
+// chunks through its pipeline.  A function of the vector length only — not of the number of planes — because the
+// block count fixes the summation tree: a batched handle must reduce exactly like a single-plane one.
+inline int tma_blocks(int64_t n, int sms) { return (int)std::max<int64_t>(1, std::min<int64_t>(sms, n / (UDT_THREADS * 4) / 4)); }
 
 }  // namespace
 
@@ -628,7 +633,7 @@ void launch_multidot(const Launch& L, const double* w, const double* V, int64_t 
     if (!no_tma) ensure_dyn_smem((const void*)k_multidot_tma, UDT_SMEM);
     const int sms = dev_info().sms;
     if (m <= FUSED_NV && !no_tma && n % (UDT_THREADS * 4) == 0)
-        k_multidot_tma<<<dim3(sms, L.planes), UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
+        k_multidot_tma<<<dim3(tma_blocks(n, sms), L.planes), UDT_THREADS, UDT_SMEM, L.stream>>>(const_cast<double*>(w), V, stride, n, st, partial);
     else if (m <= FUSED_NV) k_multidot_t<<<dim3(sms * 2, L.planes), MD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     else k_multidot<<<dim3(red_blocks(), L.planes), RED_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
@@ -640,7 +645,7 @@ void launch_update_dot(const Launch& L, double* w, const double* V, int64_t stri
     static const bool no_tma = getenv("MG_B200_NO_TMA") != nullptr;
     if (!no_tma) ensure_dyn_smem((const void*)k_update_dot_tma, UDT_SMEM);
     const int sms = dev_info().sms;
-    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<dim3(sms, L.planes), UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
+    if (!no_tma && n % (UDT_THREADS * 4) == 0) k_update_dot_tma<<<dim3(tma_blocks(n, sms), L.planes), UDT_THREADS, UDT_SMEM, L.stream>>>(w, V, stride, n, st, partial);
     else k_update_dot<<<dim3(sms * 2, L.planes), UD_THREADS, 0, L.stream>>>(w, V, stride, n, st, partial);
     count(L);
 }
