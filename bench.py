@@ -36,11 +36,24 @@ WORKLOADS = {
     4: "configs[3]: D-shape with X-point 4097x4097 (~11M unknowns), 10 levels",
     5: "configs[4]: D-shape 2049x2049 (~2.8M unknowns), 9 levels, time stepping",
 }
-# algorithmic bytes per point (SURVEY.md 8(d) / DESIGN.md section 6): one full RB-B GS sweep
-ROOF_BYTES_PER_POINT = 2 * 64.0 + 61.0
-# DRAM bytes per launch of the roofline kernel (dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full
-# capture per config; profiles/r01e_roofline_kernel_config4.md)
-ROOF_TRAFFIC_PER_LAUNCH = {4: 582.5e6}
+# Roofline kernel: the fused launch "two RB-B Gauss-Seidel sweeps + defect + full-weighting restriction" on level 0.
+# Algorithmic bytes per point of THAT launch: every array the operation needs, moved exactly once:
+# x in 8 + c 8 + b 8 + 1/a_ll 8 + lambda 8 + x out 8 + point code 2 + restricted defect 8/4 = 52 B.  The three-loop
+# formulation of SURVEY.md 8(d) (2 x 64 B/pt for two sweeps + 61 B/pt for defect + restriction = 189 B/pt) is reported
+# beside it as what the fusion avoids; it is not a statement about HBM.
+ROOF_BYTES_PER_POINT = 52.0
+UNFUSED_BYTES_PER_POINT = 2 * 64.0 + 61.0
+# DRAM bytes per launch of the roofline kernel (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
+# capture per config), kept in profiles/roofline_traffic.json with the command and the date of the capture
+
+
+def roofline_traffic(cfg):
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    try:
+        e = json.load(open(p))["configs"].get(str(cfg))
+        return (float(e["dram_bytes_per_launch"]), e.get("capture")) if e else (None, None)
+    except (OSError, KeyError, ValueError):
+        return None, None
 
 
 def peaks():
@@ -134,6 +147,41 @@ def run_reference(args):
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
+
+
+def spawn_command(gpus, argv, port=None):
+    """`python bench.py --gpus N` without a launcher: the torchrun command that starts one rank per GPU (what the driver
+    runs itself for N > 1)."""
+    if port is None:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def respawn(args, argv):
+    """--gpus N > 1 outside a launcher (no WORLD_SIZE in the environment): re-exec under torchrun so that N ranks exist."""
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        cmd = spawn_command(args.gpus, argv)
+        os.execv(cmd[0], cmd)
+
+
+def run_dry(args):
+    """MG_BENCH_DRY=1: the multi-rank plumbing without a GPU (gloo, CPU): every rank owns its plane's inputs, the two
+    reductions of whole_job run, rank 0 prints the line.  Used by tests/test_bench_sharding.py."""
+    import torch.distributed as dist
+    world, rank = int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    pl = W.make_plane(args.config, 65, seed=plane_seed(args.config, rank))
+    ms, work, value = whole_job(10.0 * (rank + 1), float(pl.n) * 7, world, "cpu")
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": ms / max(args.steps, 1), "scaling": "weak", "data": "dry run (no GPU work)", "dry": True}))
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def plane_seed(cfg, rank):
@@ -269,20 +317,35 @@ def run_ours(args):
         per_launch_ms = float(np.median(t[2:]))
         alg = ROOF_BYTES_PER_POINT * n0
         achieved = alg / (per_launch_ms * 1e-3) / 1e9
-        traffic = ROOF_TRAFFIC_PER_LAUNCH.get(args.config) if (args.lattice is None and not args.three_field) else None
-        roof = {"bound": "hbm", "kernel": "k_gs<2,false,true> level 0: two fused RB-B Gauss-Seidel sweeps + defect + FW restriction per launch",
+        traffic, capture = roofline_traffic(args.config) if (args.lattice is None and not args.three_field) else (None, None)
+        roof = {"bound": "hbm", "kernel": "k_gs_strip<6,8,0,1> (+ k_gs on overflow tiles) level 0: two fused RB-B Gauss-Seidel sweeps + defect + FW restriction per launch",
                 "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "algorithmic_bytes_per_launch": alg, "ms_per_launch": per_launch_ms,
-                "note": "algorithmic bytes = 2 x 64 B/pt (two sweeps of the three-loop formulation) + 61 B/pt (defect + restriction), "
-                        "SURVEY.md 8(d); temporal blocking and fusion move far fewer (traffic, ncu), so frac can exceed 1; "
-                        "frac_of_traffic = traffic / time / peak",
-                "frac_of_traffic": (traffic / (per_launch_ms * 1e-3) / 1e9 / peak) if traffic else None}
+                "note": "algorithmic bytes = 52 B/pt: every array of the fused launch moved once (DESIGN.md section 6); the kernel is bound by "
+                        "shared-memory / issue latency, not by HBM",
+                "unfused_formulation": {"bytes_per_launch": UNFUSED_BYTES_PER_POINT * n0,
+                                        "speedup_over_its_roofline": UNFUSED_BYTES_PER_POINT * n0 / (per_launch_ms * 1e-3) / 1e9 / peak}}
+        if traffic:
+            roof["traffic_capture"] = capture
+            roof["frac_of_traffic"] = traffic / (per_launch_ms * 1e-3) / 1e9 / peak
 
-    cpu = None
+    cpu = cpu_all = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         dt, it_o, _ = oracle_sample(pl, args.ref_iters, xi)
         cpu = {"value": pl.n * it_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"update + first {it_o} fGMRES iterations of the same plane, 1 thread, {dt:.1f} s"}
+        # second, separately labelled line: the same source built with -fopenmp, grid loops on all host cores (the
+        # analogue of the paper's OpenMP backend); a timing line only (reductions sum in another order)
+        from oracle import oracle as om
+        try:
+            om.use_openmp(True)
+            dt2, it2, _ = oracle_sample(pl, args.ref_iters, xi)
+            cpu_all = {"value": pl.n * it2 / dt2, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle, same source compiled with -fopenmp",
+                       "sample": f"update + first {it2} fGMRES iterations of the same plane, {os.cpu_count()} threads, {dt2:.1f} s"}
+        except Exception as e:                            # no OpenMP runtime on the box: say so, keep the line
+            cpu_all = {"unavailable": str(e)[:200]}
+        finally:
+            om.use_openmp(False)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -301,7 +364,7 @@ def run_ours(args):
                 "clocks": clocks, "gpu_launches": launches,
                 "e2e": {"value": value_e2e, "unit": UNIT, "h2d_bytes_per_step": (5 if args.three_field else 4) * pl.n * 8, "d2h_bytes_per_step": pl.n * 8,
                         "ms_per_step": ms_e2e / args.steps, "iters": outs_e[-1][0]},
-                "roofline": roof, "cpu_baseline": cpu}
+                "roofline": roof, "cpu_baseline": cpu, "cpu_baseline_allcores": cpu_all}
         print(json.dumps(line))
     s.close()
     if world > 1:
@@ -524,7 +587,10 @@ def main():
     ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved together by one batched handle (secondary line, SURVEY.md 8(f) NEXT-1)")
     ap.add_argument("--plane-streams", action="store_true", help="with --planes: one handle + stream + host thread per plane instead of the batched handle")
     args = ap.parse_args()
-    if args.impl == "reference":
+    respawn(args, sys.argv[1:])
+    if os.environ.get("MG_BENCH_DRY"):
+        run_dry(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.paper_mms > 0:
         run_paper_mms(args)

@@ -8,6 +8,9 @@
 // or garbled, the reading of DESIGN.md section 3 ("M*", "D*", "T*", "GS", "C", "V", "K*" rules).
 // Parity pins: every function here is pinned by tests/test_oracle_*.py (-m "not gpu"); none is
 // "parity unpinned".  Compile: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC.
+// The `#pragma omp` lines are inert in that build (single thread, the arithmetic the pins check).  bench.py's second,
+// separately labelled baseline compiles the same file with -fopenmp (grid loops on all host cores, the analogue of the
+// paper's OpenMP backend); there the reductions sum in another order, so it is a timing line only.
 //
 // Conventions: levels are 0-based here (level 0 = the paper's sigma=1, finest).  Every per-level
 // vector is in the level's canonical order: ascending (J, I) (rule M7).  User vectors (update/solve)
@@ -275,12 +278,14 @@ static inline double row_apply(const Level& lv, int64_t l, const double* x) {
 }
 
 static void apply(const Level& lv, const double* x, double* y) {
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < lv.n; l++) y[l] = row_apply(lv, l, x);
 }
 
 // One group of gauss_seidel_rbb: group 0 red inner, 1 black inner, 2 boundary.
 static void gs_group(const Level& lv, double* x, const double* b, int group) {
     const double kappa0 = 1.0 / (2.0 * lv.h * lv.h);
+#pragma omp parallel for schedule(static)      // the points of one group are independent
     for (int64_t l = 0; l < lv.n; l++) {
         if (lv.colour[l] != group) continue;
         if (lv.kind[l] == INNER) {
@@ -316,6 +321,7 @@ static const double FW[9] = {1.0 / 16, 2.0 / 16, 1.0 / 16, 2.0 / 16, 4.0 / 16, 2
 // T2: full-weighting restriction of the defect; fine guards/absent count 0;
 // coarse guard rows are reset to 0 ("boundary values can explicitly be reset").
 static void restrict_defect(const Level& f, const Level& c, const double* df, double* dc) {
+#pragma omp parallel for schedule(static)
     for (int64_t q = 0; q < c.n; q++) {
         if (c.kind[q] != INNER) { dc[q] = 0.0; continue; }
         double s = 0.0;
@@ -331,6 +337,7 @@ static void restrict_defect(const Level& f, const Level& c, const double* df, do
 // (homogeneous Eq. 11/16), then x <- x - e.
 static void prolong_correct(const Level& f, const double* ec, double* x, std::vector<double>& e) {
     e.assign(f.n, 0.0);
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < f.n; l++) {
         if (f.kind[l] != INNER) continue;
         double s = 0.0;
@@ -351,12 +358,14 @@ static void prolong_correct(const Level& f, const double* ec, double* x, std::ve
             e[l] = s / (1.0 - f.ns_wself[l]);
         }
     }
+#pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < f.n; l++) x[l] -= e[l];
 }
 
 // T4: coefficient restriction (P:153 last sentence): full weighting over the fine points present
 // in the mesh, renormalised by the weights present.
 static void restrict_coeff(const Level& f, const Level& c, const double* vf, double* vc) {
+#pragma omp parallel for schedule(static)
     for (int64_t q = 0; q < c.n; q++) {
         double s = 0.0, w = 0.0;
         for (int k = 0; k < 9; k++) {
@@ -438,6 +447,7 @@ static void mg_cycle(Oracle& o, int s, double* x, const double* b, int kind) {
 
 static double dot(const double* a, const double* b, int64_t n) {
     double s = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : s)
     for (int64_t k = 0; k < n; k++) s += a[k] * b[k];
     return s;
 }
@@ -662,7 +672,11 @@ int orc_solve_ex(void* h, const double* f_user, const double* x0_user, double* x
                 for (int i = 0; i <= j; i++) {
                     const double hij = dot(w.data(), V[i].data(), n);
                     H[(size_t)i * m + j] += hij;
-                    for (int64_t k = 0; k < n; k++) w[k] -= hij * V[i][k];
+                    {
+                        const double* vi = V[i].data();
+#pragma omp parallel for schedule(static)
+                        for (int64_t k = 0; k < n; k++) w[k] -= hij * vi[k];
+                    }
                 }
             const double hn = std::sqrt(dot(w.data(), w.data(), n));
             H[(size_t)(j + 1) * m + j] = hn;
@@ -688,7 +702,12 @@ int orc_solve_ex(void* h, const double* f_user, const double* x0_user, double* x
             y[i] = s / H[(size_t)i * m + i];
         }
         for (int i = 0; i < jdone; i++)
-            for (int64_t k = 0; k < n; k++) x[k] += y[i] * Z[i][k];
+            {
+                const double* zi = Z[i].data();
+                const double yi = y[i];
+#pragma omp parallel for schedule(static)
+                for (int64_t k = 0; k < n; k++) x[k] += yi * zi[k];
+            }
         if (first_cycle) {
             if (ncols) *ncols = jdone;
             if (Vd) for (int i = 0; i <= jdone && i <= m; i++) std::memcpy(Vd + (size_t)i * n, V[i].data(), 8 * n);

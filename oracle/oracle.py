@@ -14,7 +14,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mg_oracle.cpp")
 _LIB = os.path.join(_HERE, "libmg_oracle.so")
+_LIB_OMP = os.path.join(_HERE, "libmg_oracle_omp.so")
 _lib = None
+_lib_omp = None
 
 
 def build(force: bool = False) -> str:
@@ -25,26 +27,48 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+def build_omp(force: bool = False) -> str:
+    """The same source with -fopenmp: grid loops on all host cores (bench.py's `cpu_baseline_allcores`, a timing line only)."""
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c++17", "-shared", "-fPIC", "-o", _LIB_OMP, _SRC])
+    return _LIB_OMP
+
+
 def _p(a, ct):
     return None if a is None else a.ctypes.data_as(C.POINTER(ct))
+
+
+def _declare(_lib):
+    _lib.orc_create.restype = C.c_void_p
+    _lib.orc_create.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
+                                C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+    _lib.orc_last_error.restype = C.c_char_p
+    _lib.orc_level_n.restype = C.c_int64
+    _lib.orc_level_h.restype = C.c_double
+    for name in ("orc_destroy", "orc_num_levels", "orc_level_n", "orc_level_h", "orc_user_perm",
+                 "orc_level_arrays", "orc_transfer_tables", "orc_update", "orc_update3", "orc_level_xi", "orc_level_coeffs",
+                 "orc_apply", "orc_smooth", "orc_smooth_group", "orc_restrict", "orc_prolong_correct",
+                 "orc_restrict_coeff", "orc_coarse_solve", "orc_cycle", "orc_solve_ex"):
+        getattr(_lib, name).argtypes = None
+    return _lib
 
 
 def lib():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
-        _lib.orc_create.restype = C.c_void_p
-        _lib.orc_create.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double,
-                                    C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
-        _lib.orc_last_error.restype = C.c_char_p
-        _lib.orc_level_n.restype = C.c_int64
-        _lib.orc_level_h.restype = C.c_double
-        for name in ("orc_destroy", "orc_num_levels", "orc_level_n", "orc_level_h", "orc_user_perm",
-                     "orc_level_arrays", "orc_transfer_tables", "orc_update", "orc_update3", "orc_level_xi", "orc_level_coeffs",
-                     "orc_apply", "orc_smooth", "orc_smooth_group", "orc_restrict", "orc_prolong_correct",
-                     "orc_restrict_coeff", "orc_coarse_solve", "orc_cycle", "orc_solve_ex"):
-            getattr(_lib, name).argtypes = None
+        _lib = _declare(C.CDLL(build()))
     return _lib
+
+
+def use_openmp(on: bool = True):
+    """Route the wrapper to the -fopenmp build (bench.py timing line) or back to the single-threaded oracle."""
+    global _lib, _lib_omp
+    if on:
+        if _lib_omp is None:
+            _lib_omp = _declare(C.CDLL(build_omp()))
+        _lib = _lib_omp
+    else:
+        _lib = None
 
 
 def _d(a):

@@ -71,7 +71,9 @@ struct mg_handle_s {
     int32_t *cslot = nullptr, *slot2row = nullptr;
     double *cwork = nullptr, *Ainv = nullptr;
     // host-buffer staging
-    double* stage[3] = {nullptr, nullptr, nullptr};
+    double* stage[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // lambda, c, x out, f, x0
+    cudaStream_t copy_stream = nullptr;   // H2D of f, x0 overlaps the update's kernels (mg_solve_host)
+    cudaEvent_t copy_ev = nullptr;
     double* stage_xi = nullptr;
     bool three_field = false;             // the level structs carry xi (Eq. 3)
     bool have_coeffs = false;
@@ -304,6 +306,8 @@ int mg_destroy(mg_handle h) {
     cudaDeviceSynchronize();
     if (h->iter_graph) cudaGraphExecDestroy(h->iter_graph);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    if (h->copy_ev) cudaEventDestroy(h->copy_ev);
     for (auto& e : h->ev) if (e) cudaEventDestroy(e);
     for (auto& e : h->hev) if (e) cudaEventDestroy(e);
     if (h->h_hdr) cudaFreeHost(h->h_hdr);
@@ -577,7 +581,7 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
 }
 
 static int ensure_stage(mg_handle h, cudaStream_t s) {
-    for (int k = 0; k < 3; k++)
+    for (int k = 0; k < 5; k++)
         if (!h->stage[k]) { int rc = dev_alloc(h, (void**)&h->stage[k], sizeof(double) * (size_t)h->n * h->P, s); if (rc) return rc; }
     return MG_OK;
 }
@@ -614,9 +618,14 @@ int mg_solve_host(mg_handle h, const double* h_f, const double* h_x0, double* h_
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_stage(h, s);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->stage[0], h_f, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
-    CU(cudaMemcpyAsync(h->stage[1], h_x0, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, s));
-    rc = mg_solve(h, h->stage[0], h->stage[1], h->stage[2], rtol, iters, final_relres, stream);
+    // f and x0 travel on their own stream into their own buffers: the copies need not wait for the update's kernels
+    // (which are still reading the lambda / c staging buffers on `s`); the solve waits for the copies
+    if (!h->copy_stream) { CU(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking)); CU(cudaEventCreateWithFlags(&h->copy_ev, cudaEventDisableTiming)); }
+    CU(cudaMemcpyAsync(h->stage[3], h_f, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, h->copy_stream));
+    CU(cudaMemcpyAsync(h->stage[4], h_x0, sizeof(double) * h->n * h->P, cudaMemcpyHostToDevice, h->copy_stream));
+    CU(cudaEventRecord(h->copy_ev, h->copy_stream));
+    CU(cudaStreamWaitEvent(s, h->copy_ev, 0));
+    rc = mg_solve(h, h->stage[3], h->stage[4], h->stage[2], rtol, iters, final_relres, stream);
     if (rc < 0) return rc;
     CU(cudaMemcpyAsync(h_x, h->stage[2], sizeof(double) * h->n * h->P, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));

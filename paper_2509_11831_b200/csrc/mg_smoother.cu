@@ -72,9 +72,15 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
                 ggen = std::max(1, std::min(ngen * L.planes, (int)(grid * wg / (wg + nint) + 0.5)));
                 if (nint > 0) ggen = std::min(ggen, grid - 1);
             }
-            ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI>, ssm);
-            k_gs_strip<SH, GH, PC, EPI><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes, xin, xout, b,
-                                                                            ec, zero ? 1 : 0, ccode, dc, L.stop);
+            if (L.planes > 1) {
+                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, true>, ssm);
+                k_gs_strip<SH, GH, PC, EPI, true><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes,
+                                                                                      xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
+            } else {
+                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, false>, ssm);
+                k_gs_strip<SH, GH, PC, EPI, false><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, 1,
+                                                                                       xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
+            }
             if (L.counter) *L.counter += 1;
         }
         return;

@@ -81,7 +81,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <int NTHREADS>
 __device__ __forceinline__ void bar_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
 
-template <int H, bool PC, int EPI, bool GEN>
+template <int H, bool PC, int EPI, bool GEN, bool MP>
 __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __restrict__ smeta, int nlist, int planes, const VecRef& xin_r,
                                            const VecRef& xout_r, const VecRef& b_r, const double* __restrict__ ec0, int xin_zero,
                                            const uint16_t* __restrict__ ccode, double* __restrict__ dc0, const int* __restrict__ stop, int cta,
@@ -114,7 +114,8 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
         q.dc = DR ? dc0 + pco : (AP ? dc0 + po : nullptr);
         return q;
     };
-    const int nitems = nlist * planes;
+    const int nitems = MP ? nlist * planes : nlist;       // MP: several planes in the launch (pointers per work item)
+    const PP one = plane_ptrs(0);
     if (cta >= nitems) return;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // ---- the strip of this thread: pair column p, rows ry0 .. ry0 + R - 1 of the region
@@ -140,8 +141,8 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
 
     // asynchronous copies of this thread's strip of the tile described by m[] into its staging slots
     auto prefetch = [&](const int* m) {
-        if (m[22]) { cp_async_commit(); return; }            // the plane of that item has ended its cycle: nothing to do
-        const PP q = plane_ptrs(m[21]);
+        if (MP && m[22]) { cp_async_commit(); return; }      // the plane of that item has ended its cycle: nothing to do
+        const PP q = MP ? plane_ptrs(m[21]) : one;
 #pragma unroll
         for (int r = 0; r < R; r++) {
             const int ly = ry0 + r - H;
@@ -177,9 +178,9 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
     };
     // table entry `tid` of work item `item`: the list entry's tables, [21] its plane, [22] whether that plane has stopped
     auto meta_of = [&](int item) {
-        const int pl = item / nlist, e = item - pl * nlist;
+        const int pl = MP ? item / nlist : 0, e = item - pl * nlist;
         if (tid == 21) return pl;
-        if (tid == 22) return stopped(stop, pl) ? 1 : 0;
+        if (tid == 22) return (MP && stopped(stop, pl)) ? 1 : 0;
         return __ldg(smeta + (int64_t)e * SMETA + tid);
     };
 
@@ -201,14 +202,14 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
         if (tid < SMETA && more2) mnext = meta_of(it + 2 * G0);    // tables two tiles ahead
         // ---- the strip: staging slots -> registers (pairs)
         cp_async_wait_all();
-        if (m[22]) {                                          // this plane's cycle has ended: keep the pipeline moving, skip the tile
+        if (MP && m[22]) {                                    // this plane's cycle has ended: keep the pipeline moving, skip the tile
             if (it + G0 < nitems) prefetch(M + (ib == 2 ? 0 : ib + 1) * SMETA);
             if (tid < SMETA && more2) M[(ib == 0 ? 2 : ib - 1) * SMETA + tid] = mnext;
             ib = ib == 2 ? 0 : ib + 1;
             bar_sync<NT>();
             continue;
         }
-        const PP cur = plane_ptrs(m[21]);
+        const PP cur = MP ? plane_ptrs(m[21]) : one;
         const double* __restrict__ b = cur.b;
         double* __restrict__ xout = cur.xout;
         double* __restrict__ dc = cur.dc;
@@ -522,15 +523,15 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
 
 // One launch, two geometries: CTAs [0, ggen) run the general tiles (list smeta_g), the others the interior tiles
 // (list smeta_i); both persistent, both with their own thread count (the block carries the larger one).
-template <int HI, int HG, bool PC, int EPI>
+template <int HI, int HG, bool PC, int EPI, bool MP>
 __global__ void __launch_bounds__((SGeo<HI>::NT > SGeo<HG>::NT ? SGeo<HI>::NT : SGeo<HG>::NT), 1)
     k_gs_strip(LevelDev lv, const int* __restrict__ smeta_i, int nint, const int* __restrict__ smeta_g, int ngen, int ggen, int planes, VecRef xin_r,
                VecRef xout_r, VecRef b_r, const double* __restrict__ ec, int xin_zero, const uint16_t* __restrict__ ccode,
                double* __restrict__ dc, const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char strip_smem[];
-    if (planes == 1 && stopped(stop, 0)) return;
-    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
-    else strip_body<HI, PC, EPI, false>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
+    if (!MP && stopped(stop, 0)) return;
+    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true, MP>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
+    else strip_body<HI, PC, EPI, false, MP>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
 }
 
 }  // namespace

@@ -64,3 +64,22 @@ def test_config5_step_sequence_is_seeded_and_chained():
     c = W.next_step(b1, 1)
     assert np.all(np.abs(b1.lam / a.lam - 1.0) <= 0.05 + 1e-12) and np.all(np.abs(c.c / b1.c - 1.0) <= 0.05 + 1e-12)
     assert not np.array_equal(c.f, b1.f) and np.array_equal(c.i, a.i)
+
+
+def test_bench_gpus_n_spawns_its_own_ranks():
+    """`python bench.py --gpus 2` with no launcher re-executes itself under torchrun (one rank per GPU, 127.0.0.1
+    rendezvous) — the driver's command shape for the scaling runs.  Dry mode: gloo on the CPU, no GPU work."""
+    import json
+    import subprocess
+    env = dict(os.environ, MG_BENCH_DRY="1")
+    for k in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT"):
+        env.pop(k, None)
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--config", "3", "--steps", "2", "--warmup", "1"],
+                         env=env, capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["ms_per_step"] == 10.0      # max over ranks: 20 ms / 2 steps
+    import bench
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "3"], port=29511)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=4" in cmd and cmd[-4:] == ["--gpus", "4", "--steps", "3"]
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
