@@ -730,4 +730,90 @@ int orc_solve(void* h, const double* f, const double* x0, double* x, double rtol
     return orc_solve_ex(h, f, x0, x, rtol, 0, iters, relres, nullptr, nullptr, nullptr, nullptr, nullptr);
 }
 
+// BiCGStab (van der Vorst) with the same V-cycle as RIGHT preconditioner — the alternative outer solver the paper names as
+// future work (section 6).  Notation of the textbook algorithm (Saad, Iterative Methods, Alg. 7.7, preconditioned
+// on the right: y = M p, z = M s):
+//     r0 = b - A x0, rhat = r0, rho = alpha = omega = 1, v = p = 0
+//     rho' = (rhat, r); beta = (rho'/rho)(alpha/omega); p = r + beta (p - omega v)
+//     y = M p; v = A y; alpha = rho' / (rhat, v); s = r - alpha v            [|s|/|b| < rtol: x += alpha y, stop]
+//     z = M s; t = A z; omega = (t, s)/(t, t); x += alpha y + omega z; r = s - omega t     [|r|/|b| < rtol: stop]
+// Stop test and restarts follow rules K1, K3, K5 of the fGMRES solve: Eq. 23 on the recurrence residual inside,
+// the recomputed true residual decides at the end; if it is still >= rtol the iteration restarts from it (rhat = r = b - A x).
+// iters counts preconditioner applications (two per full step), as orc_solve_ex does.  precond as there (0 cycle, 1 identity,
+// 2 dense exact inverse).  hist[k] = recurrence |s| or |r| over |b| after application k+1.
+// Returns 0 converged, 1 max_iters reached, 2 breakdown (rho, (rhat, v) or (t, t) vanished), <0 error.
+int orc_solve_bicgstab(void* h, const double* f_user, const double* x0_user, double* x_user, double rtol, int precond,
+                       int* iters_out, double* relres_out, double* hist) {
+    Oracle* o = (Oracle*)h;
+    if (!o->have_coeffs) { g_err = "solve before update"; return -3; }
+    Level& lv = o->lev[0];
+    const int64_t n = lv.n;
+    std::vector<double> b(n), x(n), r(n), rhat(n), p(n, 0.0), v(n, 0.0), y(n), s(n), z(n), t(n);
+    for (int64_t k = 0; k < n; k++) { b[o->user2canon[k]] = f_user[k]; x[o->user2canon[k]] = x0_user[k]; }
+    if (precond == 2 && o->lu0.empty()) { assemble_dense(lv, o->lu0); if (!lu_factor(o->lu0, o->piv0, n)) return -2; }
+    auto M = [&](const std::vector<double>& in, std::vector<double>& out) {
+        if (precond == 0) { std::fill(out.begin(), out.end(), 0.0); mg_cycle(*o, 0, out.data(), in.data(), o->gamma); }
+        else if (precond == 1) out = in;
+        else lu_solve(o->lu0, o->piv0, n, in.data(), out.data());
+    };
+    int iters = 0, status = 1; double relres = 0.0;
+    const double bn = std::sqrt(dot(b.data(), b.data(), n));
+    auto finish = [&](int st) {
+        for (int64_t k = 0; k < n; k++) x_user[k] = x[o->user2canon[k]];
+        if (iters_out) *iters_out = iters;
+        if (relres_out) *relres_out = relres;
+        return st;
+    };
+    if (bn == 0.0) { std::fill(x.begin(), x.end(), 0.0); return finish(0); }                     // K1
+    while (true) {
+        apply(lv, x.data(), r.data());
+        for (int64_t k = 0; k < n; k++) r[k] = b[k] - r[k];                                      // D4
+        relres = std::sqrt(dot(r.data(), r.data(), n)) / bn;
+        if (relres < rtol) { status = 0; break; }                                                // K1 / K5
+        if (iters >= o->max_iters) { status = 1; break; }
+        rhat = r;
+        std::fill(p.begin(), p.end(), 0.0); std::fill(v.begin(), v.end(), 0.0);
+        double rho = 1.0, alpha = 1.0, omega = 1.0;
+        bool breakdown = false;
+        while (iters < o->max_iters) {
+            const double rho1 = dot(rhat.data(), r.data(), n);
+            if (rho1 == 0.0 || omega == 0.0) { breakdown = true; break; }
+            const double beta = (rho1 / rho) * (alpha / omega);
+            for (int64_t k = 0; k < n; k++) p[k] = r[k] + beta * (p[k] - omega * v[k]);
+            M(p, y);
+            apply(lv, y.data(), v.data());
+            const double rv = dot(rhat.data(), v.data(), n);
+            if (rv == 0.0) { breakdown = true; break; }
+            alpha = rho1 / rv;
+            for (int64_t k = 0; k < n; k++) s[k] = r[k] - alpha * v[k];
+            iters++;
+            const double sn = std::sqrt(dot(s.data(), s.data(), n)) / bn;
+            if (hist) hist[iters - 1] = sn;
+            if (sn < rtol || iters >= o->max_iters) {                                             // K3 at the half step
+                for (int64_t k = 0; k < n; k++) x[k] += alpha * y[k];
+                break;
+            }
+            M(s, z);
+            apply(lv, z.data(), t.data());
+            const double tt = dot(t.data(), t.data(), n);
+            if (tt == 0.0) { for (int64_t k = 0; k < n; k++) x[k] += alpha * y[k]; breakdown = true; break; }
+            omega = dot(t.data(), s.data(), n) / tt;
+            for (int64_t k = 0; k < n; k++) { x[k] += alpha * y[k] + omega * z[k]; r[k] = s[k] - omega * t[k]; }
+            iters++;
+            rho = rho1;
+            const double rn = std::sqrt(dot(r.data(), r.data(), n)) / bn;
+            if (hist) hist[iters - 1] = rn;
+            if (rn < rtol) break;                                                                 // K3
+        }
+        if (breakdown) {
+            apply(lv, x.data(), r.data());
+            for (int64_t k = 0; k < n; k++) r[k] = b[k] - r[k];
+            relres = std::sqrt(dot(r.data(), r.data(), n)) / bn;
+            status = relres < rtol ? 0 : 2;
+            break;
+        }
+    }                                                                                             // K5: loop = restart
+    return finish(status);
+}
+
 }  // extern "C"

@@ -48,7 +48,7 @@ def _declare(_lib):
     for name in ("orc_destroy", "orc_num_levels", "orc_level_n", "orc_level_h", "orc_user_perm",
                  "orc_level_arrays", "orc_transfer_tables", "orc_update", "orc_update3", "orc_level_xi", "orc_level_coeffs",
                  "orc_apply", "orc_smooth", "orc_smooth_group", "orc_restrict", "orc_prolong_correct",
-                 "orc_restrict_coeff", "orc_coarse_solve", "orc_cycle", "orc_solve_ex"):
+                 "orc_restrict_coeff", "orc_coarse_solve", "orc_cycle", "orc_solve_ex", "orc_solve_bicgstab"):
         getattr(_lib, name).argtypes = None
     return _lib
 
@@ -222,3 +222,15 @@ class Oracle:
             k = ncols.value
             res.update(V=V[:k + 1], Z=Z[:k], H=H[:k + 1, :k], ncols=k)
         return res
+
+    def solve_bicgstab(self, f, x0, rtol, precond=0):
+        """BiCGStab with the V-cycle as right preconditioner; iters counts preconditioner applications."""
+        f, x0 = _d(f), _d(x0)
+        x = np.empty(self.n)
+        iters, relres = C.c_int(0), C.c_double(0.0)
+        hist = np.zeros(8192)
+        vp = lambda a: C.c_void_p(a.ctypes.data)
+        st = lib().orc_solve_bicgstab(self._h, vp(f), vp(x0), vp(x), C.c_double(rtol), int(precond), C.byref(iters), C.byref(relres), vp(hist))
+        if st < 0:
+            raise RuntimeError("oracle bicgstab: " + lib().orc_last_error().decode())
+        return dict(x=x, iters=iters.value, relres=relres.value, status=st, hist=hist[:iters.value].copy())
