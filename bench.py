@@ -237,7 +237,7 @@ def run_ours(args):
     uniq = seq if warm else seq[:1]
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, full_cgs2=args.full_cgs2)
+    s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, full_cgs2=args.full_cgs2, solver=args.solver)
     d_in = [(dev(q.lam), dev(q.c), dev(q.f)) for q in uniq]          # resident in HBM before the timed region
     h_in = [(pin(q.lam).numpy(), pin(q.c).numpy(), pin(q.f).numpy()) for q in uniq]
     # --three-field: the paper's lambda phi - xi div(c grad phi) = rho (Eq. 3) with a seeded xi, the same every step
@@ -353,7 +353,7 @@ def run_ours(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": WORKLOADS[args.config] + (f" [geometry on a {args.lattice}^2 lattice]" if args.lattice else ""),
                            "unknowns_per_plane": pl.n, "planes": world, "rtol": args.rtol,
-                           "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels,
+                           "cycle": "V(2,2) RB-B GS", "restart_m": 30, "levels": s.levels, "solver": args.solver,
                            "form": "three-field (lambda, xi, c), PAPER.md Eq. 3" if args.three_field else "two-field (lambda, c), xi = 1",
                            "step": ("mg_update_coeffs3" if args.three_field else "mg_update_coeffs") + " + mg_solve" + (" (time stepping: new coefficients and rhs, warm start)" if warm else ""),
                            "l2_policy": "inputs larger than L2 (no flush)" if pl.n * 8 * 8 > 126e6 else "working set fits L2 (small config)"},
@@ -585,6 +585,7 @@ def main():
                     help="run the paper's annulus MMS scaling experiment over R refinements (6 reaches its 24 M points) instead")
     ap.add_argument("--three-field", action="store_true", help="secondary line: the paper's three-field form with a seeded xi (mg_update_coeffs3)")
     ap.add_argument("--planes", type=int, default=1, help="planes per GPU solved together by one batched handle (secondary line, SURVEY.md 8(f) NEXT-1)")
+    ap.add_argument("--solver", default="fgmres", choices=["fgmres", "bicgstab"], help="outer solver (secondary line: BiCGStab, PAPER.md:342)")
     ap.add_argument("--plane-streams", action="store_true", help="with --planes: one handle + stream + host thread per plane instead of the batched handle")
     args = ap.parse_args()
     respawn(args, sys.argv[1:])

@@ -94,6 +94,11 @@ typedef struct {
                       every kernel launch covers all planes (gridDim.y = P), each plane has its own fGMRES state and
                       stops on its own Eq. 23; results are bit-identical to P separate handles.  The single-step and
                       inspection calls below work on plane 0.                                                   */
+    int solver;    /* outer solver: 0 = fGMRES(restart_m) (the paper's and the benchmarked choice);
+                      1 = BiCGStab with the same cycle as right preconditioner ("BiCGStab ... as alternative");
+                      it keeps no Krylov basis (seven work vectors instead of 2 (m + 1)), restart_m is ignored, iters
+                      counts preconditioner applications (two per step), the stop test and the restart from the
+                      recomputed true residual are those of mg_solve                                             */
 } mg_options;
 
 /* Device-memory allocator used by handles created afterwards (e.g. torch's caching allocator).

@@ -42,7 +42,7 @@ class _Bc(C.Structure):
 
 class _Options(C.Structure):
     _fields_ = [("levels", C.c_int), ("nu_pre", C.c_int), ("nu_post", C.c_int), ("restart_m", C.c_int),
-                ("max_iters", C.c_int), ("flags", C.c_int), ("gamma", C.c_int), ("planes", C.c_int)]
+                ("max_iters", C.c_int), ("flags", C.c_int), ("gamma", C.c_int), ("planes", C.c_int), ("solver", C.c_int)]
 
 
 EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_update_coeffs3", "mg_update_coeffs3_host", "mg_level_xi", "mg_solve", "mg_update_coeffs_host",
@@ -108,7 +108,7 @@ def _dptr(t):
 class Solver:
     """create / update / solve on one mesh."""
 
-    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1, full_cgs2=False, planes=1):
+    def __init__(self, i, j, kind, h, levels=0, nu_pre=2, nu_post=2, restart_m=30, max_iters=200, stream=None, host_only=False, fused_tail=False, gamma=1, full_cgs2=False, planes=1, solver=0):
         import torch
         if not host_only and not torch.cuda.is_available():
             raise RuntimeError("paper_2509_11831_b200 needs a CUDA device (no CPU fallback)")
@@ -122,7 +122,7 @@ class Solver:
         mesh = _Mesh(self.n, i.ctypes.data, j.ctypes.data, float(h))
         bc = _Bc(kind.ctypes.data)
         opt = _Options(int(levels), int(nu_pre), int(nu_post) if int(nu_post) != 0 else -1,   # 0 sweeps = MG_NU_NONE
-                        int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma), int(planes))
+                        int(restart_m), int(max_iters), (1 if host_only else 0) | (2 if fused_tail else 0) | (4 if full_cgs2 else 0), int(gamma), int(planes), {0: 0, 1: 1, 'fgmres': 0, 'bicgstab': 1}[solver])
         hd = C.c_void_p()
         rc = L.mg_setup(C.byref(mesh), C.byref(bc), C.byref(opt), None if host_only else _stream_ptr(stream), C.byref(hd))
         if rc:

@@ -45,6 +45,8 @@ struct LevelBuf {           // device arrays owned per level
 struct mg_handle_s {
     HostHierarchy hh;
     int L = 0;
+    int solver = 0;                       // outer solver: 0 fGMRES(m), 1 BiCGStab
+    double* bv[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // BiCGStab: rhat, p, v, s, t, y, z
     int P = 1;                            // planes solved together on this mesh; vectors are [plane][slot]
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
     int gamma = 1;                        // cycle type: 1 V-cycle, 2 W-cycle, 3 F-cycle
@@ -256,6 +258,22 @@ void enqueue_iteration(mg_handle h, const Launch& L) {
     launch_next_v(L, h->w, h->V, ns, ns, h->st);
 }
 
+// One BiCGStab step (mg_bicgstab.cu): two preconditioner applications, each with its operator apply fused into the
+// cycle's last smoothing launch; the second application is skipped on the device after a half step.
+void enqueue_bicgstab_step(mg_handle h, const Launch& L) {
+    const int64_t ns = h->lev[0].nslots;
+    double *rhat = h->bv[0], *p = h->bv[1], *v = h->bv[2], *sv = h->bv[3], *t = h->bv[4], *y = h->bv[5], *z = h->bv[6];
+    launch_bi_p(L, h->st, h->r, p, v, ns);
+    if (!enqueue_cycle(h, L, 0, vec(y, ns), vec(p, ns), true, v)) launch_apply(L, h->lev[0], vec(y, ns), vec(nullptr), vec(v, ns), 0);
+    launch_bi_alpha(L, h->st, rhat, v, ns, h->partial);
+    launch_bi_s(L, h->st, h->r, v, sv, ns, h->partial);
+    Launch L2 = L;
+    L2.stop = &h->st->b_skip2;                            // z = M s, t = A z: not after a half step
+    if (!enqueue_cycle(h, L2, 0, vec(z, ns), vec(sv, ns), true, t)) launch_apply(L2, h->lev[0], vec(z, ns), vec(nullptr), vec(t, ns), 0);
+    launch_bi_omega(L, h->st, t, sv, ns, h->partial);
+    launch_bi_update(L, h->st, h->xs, h->r, rhat, y, z, sv, t, ns, h->partial);
+}
+
 int build_iter_graph(mg_handle h) {
     if (h->iter_graph) return MG_OK;
     cudaGraph_t g = nullptr;
@@ -263,7 +281,7 @@ int build_iter_graph(mg_handle h) {
     CU(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
     Launch L = LZ(h, h->cap_stream);
     L.stop = &h->st->cycle_end;          // iterations are enqueued one ahead of the convergence test
-    enqueue_iteration(h, L);
+    if (h->solver == 1) enqueue_bicgstab_step(h, L); else enqueue_iteration(h, L);
     CU(cudaStreamEndCapture(h->cap_stream, &g));
     CU(h->tail_err);
     h->iter_graph_kernels = h->launches - before;
@@ -323,7 +341,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     if (!mesh || !bc || !mesh->i || !mesh->j || !bc->kind || mesh->n <= 0 || !(mesh->h > 0.0)) { g_last_error = "null pointer, n <= 0 or h <= 0"; return MG_EINVAL; }
     mg_options o{};
     if (opt) o = *opt;
-    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < MG_NU_NONE || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0 || o.planes < 0 || o.planes > 4096) { g_last_error = "bad option"; return MG_EINVAL; }
+    if (o.levels < 0 || o.nu_pre < 0 || o.nu_post < MG_NU_NONE || o.restart_m < 0 || o.restart_m > MAX_M || o.max_iters < 0 || o.gamma < 0 || o.gamma > 3 || (o.flags & ~7) != 0 || o.planes < 0 || o.planes > 4096 || o.solver < 0 || o.solver > 1) { g_last_error = "bad option"; return MG_EINVAL; }
     const bool host_only = (o.flags & 1) != 0;
     int ndev = 0;
     if (!host_only && (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)) { cudaGetLastError(); g_last_error = "no CUDA device (this library has no CPU fallback)"; return MG_ECUDA; }
@@ -335,6 +353,7 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
     h->max_iters = o.max_iters ? o.max_iters : 200;
     h->gamma = o.gamma > 1 ? o.gamma : 1;
     h->P = o.planes > 1 ? o.planes : 1;
+    h->solver = o.solver;
     h->full_cgs2 = (o.flags & MG_SETUP_FULL_CGS2) != 0;
     h->n = mesh->n;
     h->alloc = g_alloc; h->free_fn = g_free;
@@ -408,8 +427,12 @@ int mg_setup(const mg_mesh* mesh, const mg_bc* bc, const mg_options* opt, void* 
         for (int l = h->L - 1; l >= 0 && h->lev[l].ntiles <= h->tail_cap; l--) h->tail_s0 = l;
     TRY(upload(h, &h->user2slot, h->hh.user2slot, s));
     const size_t v0 = (size_t)h->lev[0].nslots * sizeof(double) * h->P;
-    TRY(dev_alloc(h, (void**)&h->V, v0 * (h->m + 1), s));
-    TRY(dev_alloc(h, (void**)&h->Z, v0 * (h->m + 1), s));
+    if (h->solver == 0) {
+        TRY(dev_alloc(h, (void**)&h->V, v0 * (h->m + 1), s));
+        TRY(dev_alloc(h, (void**)&h->Z, v0 * (h->m + 1), s));
+    } else {
+        for (int k = 0; k < 7; k++) TRY(dev_alloc(h, (void**)&h->bv[k], v0, s));     // no Krylov basis: seven work vectors
+    }
     TRY(dev_alloc(h, (void**)&h->w, v0, s));
     TRY(dev_alloc(h, (void**)&h->r, v0, s));
     TRY(dev_alloc(h, (void**)&h->xs, v0, s));
@@ -520,7 +543,8 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
     for (int cycle = 0; cycle < 1000000; cycle++) {
         launch_apply(L, h->lev[0], vec(h->xs, ns), vec(h->bs, ns), vec(h->r, ns), 1);      // r = b - A x (rule D4)
         launch_norm2(L, h->r, ns, h->st, h->partial, 1);
-        launch_start_cycle(L, h->st, h->r, h->V, ns);
+        if (h->solver == 1) launch_bi_start(L, h->st, h->r, h->bv[0], ns);
+        else launch_start_cycle(L, h->st, h->r, h->V, ns);
         rc = copy_headers(h, 0, s);
         if (rc) return rc;
         if (h->coeffs_unchecked) CU(cudaMemcpyAsync(h->h_flag, h->coeff_bad, sizeof(int), cudaMemcpyDeviceToHost, s));
@@ -534,7 +558,8 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
         // One graph launch per Arnoldi step.  The host stays one step ahead: step `it` is enqueued before
         // the headers of step it-1 are inspected, so the GPU never idles on the round trip; a step enqueued
         // after the cycle has ended finds cycle_end set and every kernel in it returns at once.
-        for (int it = 0; it < h->m; it++) {
+        const int nsteps = h->solver == 1 ? h->max_iters / 2 + 2 : h->m;      // BiCGStab: no restart length, the cap ends the cycle
+        for (int it = 0; it < nsteps; it++) {
             CU(cudaGraphLaunch(h->iter_graph, s));
             h->launches += h->iter_graph_kernels;
             rc = copy_headers(h, it & 1, s);
@@ -545,7 +570,7 @@ int mg_solve(mg_handle h, const double* d_f, const double* d_x0, double* d_x, do
                 if (all_ended(h, (it - 1) & 1)) break;
             }
         }
-        launch_update_x(L, h->xs, h->Z, ns, ns, h->st);               // K4
+        if (h->solver == 0) launch_update_x(L, h->xs, h->Z, ns, ns, h->st);               // K4 (BiCGStab updates x in place)
     }
     launch_zero_rhs_planes(L, h->xs, ns, h->st);                      // K1: zero right-hand side -> x = 0
     launch_scatter(L, h->xs, h->user2slot, d_x, h->n, ns);            // B1: tile layout -> user order

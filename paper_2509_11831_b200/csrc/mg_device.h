@@ -67,6 +67,12 @@ struct GmresState {
     double g[MAX_M + 1], cs[MAX_M], sn[MAX_M], y[MAX_M];
     double hist[512];               // |g_{k+1}| / bn per iteration
     double orth[512];               // ||V^T w'|| / ||w'|| after the first Gram-Schmidt projection, per iteration (fused path)
+    // BiCGStab (mg_options.solver = 1, mg_bicgstab.cu): the scalars of the recurrence and the flags of the running step
+    double b_rho, b_rho1, b_alpha, b_omega;
+    int b_first;                    // first step after a (re)start: p = r
+    int b_half;                     // the step ends after its first half (|s| below rtol, iteration cap, or (t, t) = 0)
+    int b_skip2;                    // second preconditioner application of the step not needed (b_half or cycle_end)
+    int b_pad;
 };
 
 // Planes (one elliptic solve per poloidal plane, all on the same mesh).  A handle created
@@ -206,6 +212,14 @@ void launch_final_v(const Launch& L, const double* w, double* V, int64_t stride,
 void launch_next_v(const Launch& L, const double* w, double* V, int64_t stride, int64_t n, GmresState* st);
 void launch_update_x(const Launch& L, double* x, const double* Z, int64_t stride, int64_t n, GmresState* st);
 void launch_zero_rhs_planes(const Launch& L, double* x, int64_t n, const GmresState* st);
+// ---- BiCGStab vector kernels (mg_bicgstab.cu); all vectors level-0 tile layout, n = nslots, plane stride n
+void launch_bi_start(const Launch& L, GmresState* st, const double* r, double* rhat, int64_t n);
+void launch_bi_p(const Launch& L, GmresState* st, const double* r, double* p, const double* v, int64_t n);
+void launch_bi_alpha(const Launch& L, GmresState* st, const double* rhat, const double* v, int64_t n, double* partial);
+void launch_bi_s(const Launch& L, GmresState* st, const double* r, const double* v, double* s, int64_t n, double* partial);
+void launch_bi_omega(const Launch& L, GmresState* st, const double* t, const double* s, int64_t n, double* partial);
+void launch_bi_update(const Launch& L, GmresState* st, double* x, double* r, const double* rhat, const double* y, const double* z,
+                      const double* s, const double* t, int64_t n, double* partial);
 void launch_init_state(const Launch& L, GmresState* st, int m, int max_iters, double rtol, bool full_cgs2);
 
 }  // namespace mgb
