@@ -33,7 +33,7 @@ inline int64_t floordiv(int64_t a, int64_t b) { return (a >= 0) ? a / b : -((-a 
 struct HostLevel {
     double h = 0;
     int32_t ntiles = 0;
-    std::vector<int32_t> tI, tJ;        // tile coordinates, sorted by (TJ, TI)
+    std::vector<int32_t> tI, tJ;        // tile coordinates per tile id (ids in (TJ, TI) order unless MG_B200_TILE_ORDER says otherwise)
     std::vector<uint16_t> code;         // (ntiles + 1) * TS
     std::vector<int32_t> tnb;           // 9 * ntiles: neighbour tile ids, (dy+1)*3 + (dx+1); missing -> ntiles
     std::vector<int32_t> ctab;          // on a COARSE level: 9 * ntiles ids of the FINE tiles (2TJ-1..2TJ+1) x (2TI-1..2TI+1)
@@ -48,6 +48,8 @@ struct HostLevel {
     int64_t nslots() const { return (int64_t)(ntiles + 1) * TS; }
     // lookup
     std::vector<int64_t> keys;          // sorted tile keys for binary search
+    std::vector<int32_t> id_of_key;     // position in `keys` -> tile id (the tile ORDER is a layout choice: row-major by default,
+                                        // Morton or parent-grouped for the ordering study, MG_B200_TILE_ORDER)
     int32_t find_tile(int64_t TI, int64_t TJ) const;
     uint16_t get(int64_t I, int64_t J) const;     // code at lattice point, 0 if absent
     int64_t slot_of(int64_t I, int64_t J) const;  // -1 if the tile is not active

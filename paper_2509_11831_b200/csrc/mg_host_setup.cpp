@@ -5,7 +5,9 @@
 #include "mg_common.h"
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
+#include <numeric>
 
 #include "../../include/mg_b200.h"
 
@@ -19,7 +21,7 @@ int32_t HostLevel::find_tile(int64_t TI, int64_t TJ) const {
     const int64_t k = tile_key(TI, TJ);
     auto it = std::lower_bound(keys.begin(), keys.end(), k);
     if (it == keys.end() || *it != k) return -1;
-    return (int32_t)(it - keys.begin());
+    return id_of_key[it - keys.begin()];
 }
 
 int64_t HostLevel::slot_of(int64_t I, int64_t J) const {
@@ -48,15 +50,33 @@ bool fill_level(HostLevel& lv, const std::vector<Pt>& pts, std::vector<int32_t>*
     lv.keys.erase(std::unique(lv.keys.begin(), lv.keys.end()), lv.keys.end());
     lv.ntiles = (int32_t)lv.keys.size();
     lv.tI.resize(lv.ntiles); lv.tJ.resize(lv.ntiles);
-    for (int32_t t = 0; t < lv.ntiles; t++) {
-        lv.tJ[t] = (int32_t)((lv.keys[t] >> 31) - (int64_t(1) << 30));
-        lv.tI[t] = (int32_t)((lv.keys[t] & 0x7fffffffLL) - (int64_t(1) << 30));
+    // Tile order = order of the tile ids in memory and in the smoother's work lists.  0: (TJ, TI) row-major (default);
+    // 1: Morton (Z-curve) over the tile coordinates; 2: parent-grouped — the 2 x 2 tiles under one coarse tile adjacent,
+    // parents row-major.  The paper's ordering study at tile granularity: profiles/r02_layout.md.
+    static const int order = getenv("MG_B200_TILE_ORDER") ? atoi(getenv("MG_B200_TILE_ORDER")) : 0;
+    std::vector<int32_t> cI(lv.ntiles), cJ(lv.ntiles), pos(lv.ntiles);
+    for (int32_t q = 0; q < lv.ntiles; q++) {
+        cJ[q] = (int32_t)((lv.keys[q] >> 31) - (int64_t(1) << 30));
+        cI[q] = (int32_t)((lv.keys[q] & 0x7fffffffLL) - (int64_t(1) << 30));
     }
+    std::iota(pos.begin(), pos.end(), 0);
+    if (order != 0 && lv.ntiles > 0) {
+        const int32_t i0 = *std::min_element(cI.begin(), cI.end()) & ~1, j0 = *std::min_element(cJ.begin(), cJ.end()) & ~1;
+        auto spread = [](uint64_t v) { uint64_t r = 0; for (int b = 0; b < 28; b++) r |= ((v >> b) & 1ull) << (2 * b); return r; };
+        std::vector<uint64_t> sk(lv.ntiles);
+        for (int32_t q = 0; q < lv.ntiles; q++) {
+            const uint64_t a = (uint64_t)(cI[q] - i0), b = (uint64_t)(cJ[q] - j0);
+            sk[q] = order == 1 ? (spread(a) | (spread(b) << 1)) : ((((b >> 1) << 28 | (a >> 1)) << 2) | ((b & 1) << 1) | (a & 1));
+        }
+        std::stable_sort(pos.begin(), pos.end(), [&](int32_t x, int32_t y) { return sk[x] < sk[y]; });
+    }
+    lv.id_of_key.assign(lv.ntiles, 0);
+    for (int32_t id = 0; id < lv.ntiles; id++) { lv.id_of_key[pos[id]] = id; lv.tI[id] = cI[pos[id]]; lv.tJ[id] = cJ[pos[id]]; }
     lv.code.assign((size_t)lv.nslots(), C_ABSENT);
     if (slot_out) slot_out->resize(pts.size());
     lv.n = (int64_t)pts.size(); lv.n_inner = 0;
     for (size_t p = 0; p < pts.size(); p++) {
-        const int32_t t = (int32_t)(std::lower_bound(lv.keys.begin(), lv.keys.end(), k[p]) - lv.keys.begin());
+        const int32_t t = lv.id_of_key[std::lower_bound(lv.keys.begin(), lv.keys.end(), k[p]) - lv.keys.begin()];
         const int64_t s = (int64_t)t * TS + (pts[p].J - (int64_t)lv.tJ[t] * TY) * TX + (pts[p].I - (int64_t)lv.tI[t] * TX);
         if (lv.code[s] != C_ABSENT) return false;
         lv.code[s] = (uint16_t)(pts[p].kind + 1);
@@ -151,12 +171,13 @@ void build_tile_tables(HostLevel& lv) {
     }
     // canonical order: ascending (J, I)
     lv.canon2slot.clear(); lv.canon2slot.reserve((size_t)lv.n);
-    int32_t t0 = 0;
+    int32_t t0 = 0;                                  // positions in `keys` (sorted by (TJ, TI)): one tile row at a time
     while (t0 < lv.ntiles) {
         int32_t t1 = t0;
-        while (t1 < lv.ntiles && lv.tJ[t1] == lv.tJ[t0]) t1++;
+        while (t1 < lv.ntiles && (lv.keys[t1] >> 31) == (lv.keys[t0] >> 31)) t1++;
         for (int ly = 0; ly < TY; ly++)
-            for (int32_t t = t0; t < t1; t++) {
+            for (int32_t q = t0; q < t1; q++) {
+                const int32_t t = lv.id_of_key[q];
                 const uint16_t* c = &lv.code[(size_t)t * TS + ly * TX];
                 for (int lx = 0; lx < TX; lx++)
                     if (c[lx] != C_ABSENT) lv.canon2slot.push_back((int32_t)((int64_t)t * TS + ly * TX + lx));

@@ -104,6 +104,12 @@ void launch_ns(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, Vec
     static const bool no_sub = getenv("MG_B200_NO_SUBBLOCKS") != nullptr;
     const int sms = dev_info().sms;
     const int SUB_MAX_TILES = sms * 10 / 37, MID_MAX_TILES = sms / 2, HALF_MAX_TILES = sms;
+    // layout study (profiles/r02_layout.md): MG_B200_FORCE_BLOCK = 1 / 2 / 3 / 4 forces 16x16 / 32x16 / 64x16 / whole-tile CTAs of the
+    // shared-memory tile code on every level
+    static const int force = getenv("MG_B200_FORCE_BLOCK") ? atoi(getenv("MG_B200_FORCE_BLOCK")) : 0;
+    if (force == 1) return launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    if (force == 2) return launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
+    if (force == 3) return launch_blk<NS, PC, EPI, HBX, HBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     const int64_t nt = (int64_t)lv.ntiles * L.planes;       // tiles of all planes: what fills the machine
     if (nt <= SUB_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, SBX, SBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
     else if (nt <= MID_MAX_TILES && !no_sub) launch_blk<NS, PC, EPI, MBX, MBY>(L, lv, xin, xout, b, ec, zero, ccode, dc);
