@@ -76,6 +76,7 @@ struct Oracle {
     std::vector<int64_t> user2canon;          // user index -> canonical index on level 0
     int nu_pre = 2, nu_post = 2, m = 30, max_iters = 200;
     int gamma = 1;                            // cycle type: 1 V-cycle, 2 W-cycle, 3 F-cycle
+    int bc_transfer = 0;                      // 0: rules T2 / T3 (fixed weights, missing points count 0); 1: boundary-aware variant (reading G9)
     bool have_coeffs = false;
     // coarse factorisation
     std::vector<double> lu;
@@ -320,30 +321,43 @@ static const double FW[9] = {1.0 / 16, 2.0 / 16, 1.0 / 16, 2.0 / 16, 4.0 / 16, 2
 
 // T2: full-weighting restriction of the defect; fine guards/absent count 0;
 // coarse guard rows are reset to 0 ("boundary values can explicitly be reset").
-static void restrict_defect(const Level& f, const Level& c, const double* df, double* dc) {
+// bc_mode 1 (experiment of reading G9, "stencil points may be missing"): where the 3 x 3 fine neighbourhood of the
+// coarse point touches a NEUMANN guard, the weights of the fine inner points present are renormalised to sum 1 (at a
+// Dirichlet boundary the missing defects really are 0, at a Neumann boundary they are not).
+static void restrict_defect(const Level& f, const Level& c, const double* df, double* dc, int bc_mode = 0) {
 #pragma omp parallel for schedule(static)
     for (int64_t q = 0; q < c.n; q++) {
         if (c.kind[q] != INNER) { dc[q] = 0.0; continue; }
-        double s = 0.0;
+        double s = 0.0, w = 0.0;
+        bool neu = false;
         for (int k = 0; k < 9; k++) {
             const int32_t l = f.fine9[9 * q + k];
-            if (l >= 0 && f.kind[l] == INNER) s += FW[k] * df[l];
+            if (l >= 0 && f.kind[l] == INNER) { s += FW[k] * df[l]; w += FW[k]; }
+            if (l >= 0 && f.kind[l] == NEUMANN) neu = true;
         }
-        dc[q] = s;
+        dc[q] = (bc_mode == 1 && neu && w > 0.0) ? s / w : s;
     }
 }
 
 // T3: e = P e_c on fine inner points (bilinear, absent parents count 0), set_bnds_hom on fine guards
 // (homogeneous Eq. 11/16), then x <- x - e.
-static void prolong_correct(const Level& f, const double* ec, double* x, std::vector<double>& e) {
+// bc_mode 1 (reading G9 experiment): a fine inner point with an absent parent and a Neumann guard among its 4-neighbours
+// interpolates from the parents present with weights renormalised to sum 1 (zero-filling is exact only for Dirichlet data).
+static void prolong_correct(const Level& f, const double* ec, double* x, std::vector<double>& e, int bc_mode = 0) {
     e.assign(f.n, 0.0);
 #pragma omp parallel for schedule(static)
     for (int64_t l = 0; l < f.n; l++) {
         if (f.kind[l] != INNER) continue;
-        double s = 0.0;
+        double s = 0.0, w = 0.0, wall = 0.0;
         for (int k = 0; k < 4; k++) {
             const int32_t p = f.parent[4 * l + k];
-            if (p >= 0) s += f.parent_w[4 * l + k] * ec[p];
+            wall += f.parent_w[4 * l + k];
+            if (p >= 0) { s += f.parent_w[4 * l + k] * ec[p]; w += f.parent_w[4 * l + k]; }
+        }
+        if (bc_mode == 1 && w > 0.0 && w < wall) {
+            bool neu = false;
+            for (int d = 0; d < 4; d++) { const int32_t q = f.nbr[4 * l + d]; if (q >= 0 && f.kind[q] == NEUMANN) neu = true; }
+            if (neu) s *= wall / w;
         }
         e[l] = s;
     }
@@ -433,7 +447,7 @@ static void mg_cycle(Oracle& o, int s, double* x, const double* b, int kind) {
     for (int64_t l = 0; l < lv.n; l++) d[l] = d[l] - b[l];                   // P:183 d = A x - b
     Level& cv = o.lev[s + 1];
     std::vector<double> dc(cv.n), ec(cv.n, 0.0);                             // P:186 e = 0
-    restrict_defect(lv, cv, d.data(), dc.data());
+    restrict_defect(lv, cv, d.data(), dc.data(), o.bc_transfer);
     if (kind == 3) {
         mg_cycle(o, s + 1, ec.data(), dc.data(), 3);
         mg_cycle(o, s + 1, ec.data(), dc.data(), 1);
@@ -441,7 +455,7 @@ static void mg_cycle(Oracle& o, int s, double* x, const double* b, int kind) {
         for (int g = 0; g < kind; g++) mg_cycle(o, s + 1, ec.data(), dc.data(), kind);   // gamma visits, e carried over
     }
     std::vector<double> e;
-    prolong_correct(lv, ec.data(), x, e);
+    prolong_correct(lv, ec.data(), x, e, o.bc_transfer);
     for (int k = 0; k < o.nu_post; k++) gs_sweep(lv, x, b);
 }
 
@@ -519,6 +533,9 @@ void* orc_create(int64_t n, const int32_t* i, const int32_t* j, const uint8_t* k
 
 // cycle type: gamma of P:187-189 (1 = V, 2 = W) or 3 = F-cycle; default 1
 void orc_set_gamma(void* h, int gamma) { ((Oracle*)h)->gamma = (gamma < 1 || gamma > 3) ? 1 : gamma; }
+
+// 1: boundary-aware transfers inside the cycle (reading G9 experiment; the single-step entry points keep rules T2 / T3)
+void orc_set_bc_transfer(void* h, int mode) { ((Oracle*)h)->bc_transfer = mode == 1 ? 1 : 0; }
 
 int orc_num_levels(void* h) { return ((Oracle*)h)->L; }
 int64_t orc_level_n(void* h, int s) { return ((Oracle*)h)->lev[s].n; }

@@ -97,6 +97,10 @@ class Oracle:
         L.orc_user_perm(self._h, C.c_void_p(perm.ctypes.data))
         self.user2canon = perm
 
+    def set_bc_transfer(self, mode):
+        """Reading G9 experiment: 1 = transfers renormalised next to Neumann guards inside the cycle, 0 = rules T2 / T3."""
+        lib().orc_set_bc_transfer(self._h, int(mode))
+
     def __del__(self):
         try:
             if getattr(self, "_h", None):

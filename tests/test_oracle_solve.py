@@ -264,3 +264,26 @@ def test_f_cycle(oracle_mod):
     assert np.linalg.norm(ew) <= 1.05 * np.linalg.norm(ef) <= 1.05 * 1.05 * np.linalg.norm(ev)
     rf = of.solve(pl.f, pl.x0, 1e-10)
     assert rf["status"] == 0 and rf["iters"] <= ov.solve(pl.f, pl.x0, 1e-10)["iters"]
+
+
+def test_G9_boundary_aware_transfer_experiment(oracle_mod):
+    """Reading G9 ("stencil points may be missing"): the oracle's optional transfers that renormalise the weights next
+    to NEUMANN guards.  Pins of the option itself: it changes nothing where no Neumann guard exists (all-Dirichlet mesh:
+    identical cycle, bit for bit), the solution of a solve does not depend on it, and on the annulus with a Neumann inner
+    circle it lowers the stationary V-cycle factor.  The numbers behind DESIGN.md G9 (why the CUDA path keeps T2 / T3)."""
+    pl = H.small_annulus(65, 3, neumann_inner=False)
+    o = H.make_oracle(oracle_mod, pl)
+    rng = np.random.default_rng(3)
+    x, b = rng.standard_normal(pl.n), rng.standard_normal(pl.n)
+    c0 = o.cycle(0, x, b)
+    o.set_bc_transfer(1)
+    assert np.array_equal(o.cycle(0, x, b), c0)
+    pl = W.make_plane(2, 129)
+    res = {}
+    for mode in (0, 1):
+        o = H.make_oracle(oracle_mod, pl)
+        o.set_bc_transfer(mode)
+        r = o.solve(pl.f, pl.x0, 1e-10)
+        res[mode] = (_vcycle_factor(o, pl.n), r["iters"], r["x"])
+    assert res[1][0] < res[0][0] - 0.03 and res[1][1] <= res[0][1]
+    assert np.linalg.norm(res[1][2] - res[0][2]) <= 1e-8 * np.linalg.norm(res[0][2])
