@@ -197,6 +197,19 @@ int mg_last_reorth(mg_handle h);
  * iteration (0 on the unfused path, restart_m > 32).  Returns the number of entries written. */
 int mg_last_history(mg_handle h, double* relres, double* orth, int cap);
 
+/* ---- an entry point that allocates nothing --------------------------------------------------------------------
+ * d_out[0] = ||d_v||_2 over n doubles (the reduction behind the stop test of PAPER.md:260 Eq. 23), for callers that cannot
+ * call cudaMalloc: stream capture, tight serving loops, harnesses that forbid it.  d_v, d_out: DEVICE, caller-owned;
+ * needs no handle.  Asynchronous on `stream`; calls no cudaMalloc / cudaFree / allocating routine (one cudaMemsetAsync
+ * of 4 bytes and one kernel).  Its scratch (4096 per-block partial sums + a ticket, 32.25 KB) is a fixed __device__ array of the library that
+ * every GPU which loads the library holds until exit; n > MG_NOALLOC_MAX_N is refused with MG_EINVAL (mg_last_error says
+ * why).  All calls on a device share that array: calls that OVERLAP on the GPU (different streams, unordered graph
+ * branches) race and give wrong results — order them.  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress): make it outside stream capture.  The summation order depends on n only (deterministic, the same on
+ * every device).  Errors: MG_EINVAL, MG_ECUDA. */
+#define MG_NOALLOC_MAX_N 268435456LL /* 4096 partial sums x 65536 elements per block */
+int mg_norm2_noalloc(const double* d_v, int64_t n, double* d_out, void* stream);
+
 const char* mg_strerror(int code);
 const char* mg_last_error(void);
 

@@ -27,6 +27,22 @@ class MgError(RuntimeError):
         self.code = code
 
 
+NOALLOC_MAX_N = 268435456          # MG_NOALLOC_MAX_N of include/mg_b200.h
+
+
+def norm2_noalloc(v, out=None, stream=None):
+    """mg_norm2_noalloc: ||v||_2 of a CUDA fp64 tensor into the 1-element CUDA tensor `out`, no allocation inside the library
+    (pass `out` to allocate nothing here either).  Asynchronous; returns `out`."""
+    import torch
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=v.device)
+    assert v.is_cuda and v.dtype == torch.float64 and v.is_contiguous() and out.is_cuda and out.dtype == torch.float64
+    rc = lib().mg_norm2_noalloc(C.c_void_p(v.data_ptr()), C.c_int64(v.numel()), C.c_void_p(out.data_ptr()), _stream_ptr(stream))
+    if rc:
+        raise MgError(rc, "mg_norm2_noalloc")
+    return out
+
+
 def last_error() -> str:
     """mg_last_error(): the calling thread's last error / diagnostic text."""
     return lib().mg_last_error().decode()
@@ -49,7 +65,7 @@ EXPORTS = ["mg_set_allocator", "mg_setup", "mg_update_coeffs", "mg_update_coeffs
            "mg_solve_host", "mg_destroy", "mg_num_levels", "mg_level_n", "mg_level_info", "mg_transfer_info",
            "mg_level_coeffs", "mg_apply", "mg_smooth", "mg_restrict", "mg_smooth_restrict", "mg_prolong_correct", "mg_coarse_solve",
            "mg_vcycle", "mg_kernel_launches", "mg_last_solve_ms", "mg_last_update_ms", "mg_last_step_ms", "mg_last_reorth", "mg_last_history", "mg_strerror",
-           "mg_last_error"]
+           "mg_last_error", "mg_norm2_noalloc"]
 
 
 def lib():

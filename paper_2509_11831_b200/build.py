@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmg_b200.so")
-SOURCES = ["mg_api.cu", "mg_kernels.cu", "mg_smoother.cu", "mg_coarse.cu", "mg_krylov.cu", "mg_tail.cu", "mg_bicgstab.cu", "mg_devinfo.cu", "mg_host_setup.cpp"]
+SOURCES = ["mg_api.cu", "mg_kernels.cu", "mg_smoother.cu", "mg_coarse.cu", "mg_krylov.cu", "mg_tail.cu", "mg_bicgstab.cu", "mg_noalloc.cu", "mg_devinfo.cu", "mg_host_setup.cpp"]
 HEADERS = ["mg_common.h", "mg_device.h", "mg_tile_gs.cuh", "mg_tile_ops.cuh", os.path.join("..", "..", "include", "mg_b200.h")]
 NVCC_FLAGS = ["--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "shared"]

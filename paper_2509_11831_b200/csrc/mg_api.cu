@@ -42,6 +42,10 @@ struct LevelBuf {           // device arrays owned per level
 
 }  // namespace
 
+namespace mgb {
+void set_last_error(const std::string& msg) { g_last_error = msg; }
+}  // namespace mgb
+
 struct mg_handle_s {
     HostHierarchy hh;
     int L = 0;

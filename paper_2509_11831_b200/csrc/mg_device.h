@@ -12,6 +12,9 @@ constexpr int MAX_M = 64;          // largest fGMRES restart length
 constexpr int RED_BLOCKS_MAX = 1024;   // capacity of the per-block partial sums of the grid-wide reductions
 constexpr int RED_THREADS = 256;
 
+// text behind mg_last_error() of the calling thread (mg_api.cu), for entry points that live in other files
+void set_last_error(const std::string& msg);
+
 // Per-device facts, queried once per device (mg_devinfo.cu).
 struct DevInfo {
     int device;
