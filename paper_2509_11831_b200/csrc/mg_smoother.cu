@@ -43,7 +43,18 @@ constexpr int SBX = 16, SBY = 16;      // 8 CTAs per tile: levels of at most 40 
 constexpr int MBX = 32, MBY = 16;      // 4 CTAs per tile: at most one wave at 2 CTAs per SM (tiles <= sms / 2)
 constexpr int HBX = 64, HBY = 16;      // 2 CTAs per tile: one wave up to `sms` tiles
 
-inline double strip_gen_cost() { static const double v = getenv("MG_B200_STRIP_GEN_COST") ? atof(getenv("MG_B200_STRIP_GEN_COST")) : 2.5; return v; }
+// cost of a general tile in units of an interior tile, per fused variant (measured on config 4, B200): k = 0 sweeps + defect + restriction,
+// 1 correction + sweeps, 2 correction + sweeps + apply, 3 plain sweeps.  MG_B200_STRIP_GEN_COST_<k> overrides (tuning runs).
+inline double strip_gen_cost(int k) {
+    static double v[4] = {-1.0, -1.0, -1.0, -1.0};
+    static const double dflt[4] = {2.5, 2.5, 2.5, 2.5};
+    if (v[k] < 0.0) {
+        const char* names[4] = {"MG_B200_STRIP_GEN_COST_0", "MG_B200_STRIP_GEN_COST_1", "MG_B200_STRIP_GEN_COST_2", "MG_B200_STRIP_GEN_COST_3"};
+        const char* e = getenv(names[k]);
+        v[k] = e ? atof(e) : dflt[k];
+    }
+    return v[k];
+}
 inline bool no_strips() { static const bool v = getenv("MG_B200_NO_STRIPS") != nullptr; return v; }
 
 template <int NS, bool PC, int EPI, int BX, int BY, int XIM>
@@ -68,7 +79,7 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
             const int grid = (int)std::min<int64_t>(sms, (int64_t)(nint + ngen) * L.planes);
             int ggen = 0;
             if (ngen > 0) {
-                const double wg = ngen * strip_gen_cost();
+                const double wg = ngen * strip_gen_cost(EPI == 1 ? 0 : (PC ? (EPI == 2 ? 2 : 1) : 3));
                 ggen = std::max(1, std::min(ngen * L.planes, (int)(grid * wg / (wg + nint) + 0.5)));
                 if (nint > 0) ggen = std::min(ggen, grid - 1);
             }
