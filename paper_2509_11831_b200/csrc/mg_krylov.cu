@@ -615,7 +615,10 @@ inline void count(const Launch& L, int k = 1) { if (L.counter) *L.counter += k; 
 // CTAs per plane of the TMA-staged passes: one per SM, fewer for short vectors so that every CTA streams at least four
 // chunks through its pipeline.  A function of the vector length only — not of the number of planes — because the
 // block count fixes the summation tree: a batched handle must reduce exactly like a single-plane one.
-inline int tma_blocks(int64_t n, int sms) { return (int)std::max<int64_t>(1, std::min<int64_t>(sms, n / (UDT_THREADS * 4) / 4)); }
+inline int tma_blocks(int64_t n, int sms) {
+    static const int div = getenv("MG_B200_TMA_DIV") ? atoi(getenv("MG_B200_TMA_DIV")) : 4;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(sms, n / (UDT_THREADS * 4) / div));
+}
 
 }  // namespace
 
