@@ -95,3 +95,40 @@ def test_hierarchy_bit_exact_vs_oracle(oracle_mod, case):
         exp = np.where(a["parent_w"] > 0, a["parent"], -1)
         assert np.array_equal(exp, g["parent"])
     s.close()
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_tile_order_is_a_layout_choice_only(order):
+    """MG_B200_TILE_ORDER (Morton / parent-grouped tile ids; the ordering study of profiles/r02_layout.md) changes where a tile
+    lives in memory, nothing else: every canonical index array stays bit-exact against the oracle and the slot map stays a
+    permutation.  The variable is read once per process, hence the subprocess."""
+    import subprocess
+    import sys
+    code = (
+        "import numpy as np\n"
+        "from oracle import oracle as om\n"
+        "from paper_2509_11831_b200 import binding as B, workloads as W\n"
+        "from tests import helpers as H\n"
+        "for pl in (W.make_plane(3, 257), H.random_blob_plane(103), H.small_annulus(65, 4, i0=-37, j0=-22)):\n"
+        "    o = om.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels)\n"
+        "    s = B.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, host_only=True)\n"
+        "    assert s.levels == o.levels\n"
+        "    slots = []\n"
+        "    for lv in range(o.levels):\n"
+        "        a, g = o.level_arrays(lv), s.level_info(lv)\n"
+        "        for k in ('I', 'J', 'kind', 'colour', 'nbr', 'ns_fallback'):\n"
+        "            assert np.array_equal(a[k], g[k]), (lv, k)\n"
+        "        assert len(np.unique(g['slot'])) == len(g['slot'])\n"
+        "        slots.append(g['slot'])\n"
+        "    assert np.array_equal(o.user2canon, s.level_info(0)['user2canon'])\n"
+        "    for lv in range(o.levels - 1):\n"
+        "        a, g = o.transfer_tables(lv), s.transfer_info(lv)\n"
+        "        assert np.array_equal(a['fine9'], g['fine9']) and np.array_equal(a['ptype'], g['ptype'])\n"
+        "print('ok', sum(int(x.sum()) for x in slots))\n")
+    outs = {}
+    for o in (0, order):
+        env = dict(os.environ, MG_B200_TILE_ORDER=str(o))
+        r = subprocess.run([sys.executable, "-c", code], env=env, cwd=ROOT, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0 and r.stdout.startswith("ok"), r.stderr[-2000:]
+        outs[o] = r.stdout
+    assert outs[0] != outs[order]          # the slots really moved (last mesh has several tiles on level 0)
