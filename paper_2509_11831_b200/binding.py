@@ -88,23 +88,32 @@ def lib():
 
 
 def use_torch_allocator():
-    """Route the library's device allocations through torch's CUDA caching allocator."""
+    """Route the library's device allocations through torch's CUDA caching allocator.  The callback objects are created once and
+    kept for the life of the process: a handle keeps the function pointers it was created with (mg_set_allocator)."""
     global _alloc_cb, _free_cb
     import torch
-    AF = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
-    FF = C.CFUNCTYPE(None, C.c_void_p)
+    if _alloc_cb is None:
+        AF = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
+        FF = C.CFUNCTYPE(None, C.c_void_p)
 
-    def _alloc(nbytes, stream):
-        try:
-            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
-        except Exception:
-            return None
+        def _alloc(nbytes, stream):
+            try:
+                return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+            except Exception:
+                return None
 
-    def _free(ptr):
-        torch.cuda.caching_allocator_delete(ptr)
+        def _free(ptr):
+            torch.cuda.caching_allocator_delete(ptr)
 
-    _alloc_cb, _free_cb = AF(_alloc), FF(_free)
+        _alloc_cb, _free_cb = AF(_alloc), FF(_free)
     rc = lib().mg_set_allocator(_alloc_cb, _free_cb)
+    if rc:
+        raise MgError(rc, "mg_set_allocator")
+
+
+def use_default_allocator():
+    """Back to cudaMalloc / cudaFree for handles created from now on (existing handles keep the allocator they were created with)."""
+    rc = lib().mg_set_allocator(None, None)
     if rc:
         raise MgError(rc, "mg_set_allocator")
 

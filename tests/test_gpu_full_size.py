@@ -198,3 +198,31 @@ def test_register_tiled_smoother_on_ragged_large_meshes(gpu, oracle_mod, seed, l
     print(f"blob {seed} {lattice}: n={pl.n} levels={o.levels} iters gpu/oracle={iters}/{ro['iters']} rel.err={rel(host(xs), ro['x']):.2e}")
     assert rc == ro["status"] == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xs), ro["x"]) <= TOL_SOLVE
     s.close()
+
+
+def test_allocator_is_captured_per_handle(gpu, oracle_mod):
+    """a handle allocates and frees with the allocator pair that was installed when it was created, whatever
+    mg_set_allocator is called with in between — also for its late allocations (host-buffer staging, the xi arrays of the first
+    three-field update)."""
+    import torch
+    pl = H.small_annulus(65, 3)
+    o = H.make_oracle(oracle_mod, pl)
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    gpu.use_torch_allocator()
+    a = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=3)               # torch's caching allocator
+    gpu.use_default_allocator()
+    b = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=3)               # cudaMalloc
+    gpu.use_torch_allocator()
+    for s in (a, b):
+        s.update_coeffs_host(pl.lam, pl.c)                            # late allocation: staging buffers
+        x, iters, relres, rc = s.solve_host(pl.f, pl.x0, 1e-10)
+        assert rc == 0 and abs(iters - ro["iters"]) <= 1 and rel(x, ro["x"]) <= TOL_SOLVE
+        s.update_coeffs3(dev(pl.lam), dev(np.ones(pl.n)), dev(pl.c))  # late allocation: xi on every level
+        x3, it3, _, rc3 = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+        assert rc3 == 0 and rel(host(x3), ro["x"]) <= TOL_SOLVE
+    gpu.use_default_allocator()
+    a.close()                                                         # frees torch-cached pointers through torch although cudaFree is installed now
+    gpu.use_torch_allocator()
+    b.close()                                                         # and the other way round
+    torch.cuda.synchronize()
+    assert torch.zeros(4, device="cuda").sum().item() == 0.0          # the context is healthy
