@@ -62,8 +62,8 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
                   const uint16_t* ccode, double* dc) {
     constexpr size_t smem = Geo<NS, PC, EPI, BX, BY>::SMEM;
     ensure_dyn_smem((const void*)k_gs<NS, PC, EPI, BX, BY, XIM>, smem);
-    if (NS == 2 && XIM == 0 && BX == TX && BY == TY && !no_strips()) {
-        // large level, two-field form: interior tiles by the register-tiled kernel, the rest by the general tile code
+    if (NS == 2 && XIM != 2 && BX == TX && BY == TY && !no_strips()) {
+        // large level, two sweeps: interior and general tiles by the register-tiled kernel, guard-list overflow tiles by the tile code
         constexpr int K = EPI ? 1 : 0, SH = EPI ? 6 : 4, GH = (EPI || PC) ? 8 : 6;
         const int nint = lv.nint[K], ngen = lv.ngen[K], novf = lv.ntiles - nint - ngen, sms = dev_info().sms;
         if (novf > 0) {
@@ -84,12 +84,12 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
                 if (nint > 0) ggen = std::min(ggen, grid - 1);
             }
             if (L.planes > 1) {
-                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, true>, ssm);
-                k_gs_strip<SH, GH, PC, EPI, true><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes,
+                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, true, XIM == 1>, ssm);
+                k_gs_strip<SH, GH, PC, EPI, true, XIM == 1><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes,
                                                                                       xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
             } else {
-                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, false>, ssm);
-                k_gs_strip<SH, GH, PC, EPI, false><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, 1,
+                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, false, XIM == 1>, ssm);
+                k_gs_strip<SH, GH, PC, EPI, false, XIM == 1><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, 1,
                                                                                        xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
             }
             if (L.counter) *L.counter += 1;

@@ -81,7 +81,9 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <int NTHREADS>
 __device__ __forceinline__ void bar_sync() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
 
-template <int H, bool PC, int EPI, bool GEN, bool MP>
+// XI: the three-field form (Eq. 3): the smoother works on the row divided by xi — it holds b / xi, and 1/a_ll is
+// xi / a_ll (k_diag) — and the epilogues scale kappa by xi of the row's point, exactly as mg_tile_gs.cuh does.
+template <int H, bool PC, int EPI, bool GEN, bool MP, bool XI>
 __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __restrict__ smeta, int nlist, int planes, const VecRef& xin_r,
                                            const VecRef& xout_r, const VecRef& b_r, const double* __restrict__ ec0, int xin_zero,
                                            const uint16_t* __restrict__ ccode, double* __restrict__ dc0, const int* __restrict__ stop, int cta,
@@ -104,11 +106,11 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
     __shared__ int gcount;
     double* sxp = sx + RWC;                                 // mirror as neumann_smem / cidx<G> address it (region row 0 = padded row 1)
     // work items: (plane, list entry) pairs, plane-major; the vectors of plane pl (one solve per plane, same mesh)
-    struct PP { const double *c, *rd, *lam, *b, *xin, *ec; double *xout, *dc; };
+    struct PP { const double *c, *rd, *lam, *xi, *b, *xin, *ec; double *xout, *dc; };
     auto plane_ptrs = [&](int pl) {
         const int64_t po = (int64_t)pl * lv.nslots, pco = (int64_t)pl * (lv.ntiles_coarse + 1) * TS;
         PP q;
-        q.c = lv.c + po; q.rd = lv.rd + po; q.lam = lv.lam + po;
+        q.c = lv.c + po; q.rd = lv.rd + po; q.lam = lv.lam + po; q.xi = XI ? lv.xi + po : nullptr;
         q.b = resolve(b_r, pl); q.xin = resolve(xin_r, pl); q.xout = resolve(xout_r, pl);
         q.ec = PC ? ec0 + pco : nullptr;
         q.dc = DR ? dc0 + pco : (AP ? dc0 + po : nullptr);
@@ -152,9 +154,10 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
             if (!xin_zero) cp_async16(&stg[(1 * R + r) * NT + tid], q.xin + gs);
             if (GEN) cp_async4(&cstg[r * NT + tid], lv.code + gs);
         }
-        if (tid < 2 + (EPI ? 1 : 0)) {                       // b, 1/a_ll, lambda of that tile: into L2 now, into registers when its turn comes
+        if (tid < 4) {                                       // b, 1/a_ll, lambda, xi of that tile: into L2 now, into registers when its turn comes
             const int64_t o = (int64_t)m[20] * TS;
-            prefetch_l2_bulk(tid == 0 ? q.b + o : (tid == 1 ? q.rd + o : q.lam + o), TS * sizeof(double));
+            const double* src = tid == 0 ? q.b + o : (tid == 1 ? q.rd + o : (tid == 2 ? (EPI ? q.lam + o : nullptr) : (XI ? q.xi + o : nullptr)));
+            if (src != nullptr) prefetch_l2_bulk(src, TS * sizeof(double));
         }
         if (PC) {
             // coarse parents of the strip (bilinear prolongation): columns cx, cx + 1, rows cy0 .. cy0 + 2
@@ -253,6 +256,11 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
             const int64_t gs = (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm;
             const double2 bv = ldg2(b + gs), dv = ldg2(cur.rd + gs);
             br[r][0] = bv.x; br[r][1] = bv.y; rd[r][0] = dv.x; rd[r][1] = dv.y;
+            if (XI) {                                         // inner rows are divided by xi; guards keep their b
+                const double2 xv2 = ldg2(cur.xi + gs);
+                if (!GEN || ((imask >> (2 * r)) & 1u)) br[r][0] = __ddiv_rn(br[r][0], xv2.x);
+                if (!GEN || ((imask >> (2 * r + 1)) & 1u)) br[r][1] = __ddiv_rn(br[r][1], xv2.y);
+            }
             if (EPI && !GEN) { const double2 lv2 = ldg2(cur.lam + gs); lam[r][0] = lv2.x; lam[r][1] = lv2.y; }
         }
         double e[3][2];
@@ -409,6 +417,16 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                 lam[r][0] = lv2.x; lam[r][1] = lv2.y;
             }
         }
+        double xi2[R][2];
+        if (XI && EPI) {                                      // xi of the strip again for the epilogue (in L2; no register held it through the sweeps)
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const int ly = ry0 + r - H;
+                const int oy = (ly < 0) ? -1 : (ly >= TY ? 1 : 0);
+                const double2 xv2 = ldg2(cur.xi + (int64_t)m[(oy + 1) * 3 + ox + 1] * TS + (ly - oy * TY) * TX + lxm);
+                xi2[r][0] = xv2.x; xi2[r][1] = xv2.y;
+            }
+        }
         // ---- write the tile rows of the main strips
         if (main_w) {
 #pragma unroll
@@ -433,9 +451,11 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                         const double xl = x[r][pos];
                         const double xW = pos == 0 ? sx[SIDX(1, r) - 1] : x[r][0], xE = pos == 0 ? x[r][1] : sx[SIDX(0, r) + 1];
                         const double xS = r == 0 ? xsd[pos] : x[r - 1][pos], xN = r == R - 1 ? xnd[pos] : x[r + 1][pos];
-                        const double aW = kappa * (pos == 0 ? hW[r] : hM[r]), aE = kappa * (pos == 0 ? hM[r] : hE[r]);
-                        const double aS = kappa * v[r][pos], aN = kappa * v[r + 1][pos];
-                        d = __dsub_rn(row_d1(lam[r][pos], xl, aW, xW, aE, xE, aS, xS, aN, xN), br[r][pos]);
+                        // __dmul_rn: never contracted, so that this kernel and mg_tile_gs.cuh round identically
+                        const double kap = XI ? __dmul_rn(kappa, xi2[r][pos]) : kappa, bl = XI ? __dmul_rn(br[r][pos], xi2[r][pos]) : br[r][pos];
+                        const double aW = kap * (pos == 0 ? hW[r] : hM[r]), aE = kap * (pos == 0 ? hM[r] : hE[r]);
+                        const double aS = kap * v[r][pos], aN = kap * v[r + 1][pos];
+                        d = __dsub_rn(row_d1(lam[r][pos], xl, aW, xW, aE, xE, aS, xS, aN, xN), bl);
                     }
                     sc[SIDX(pos, r)] = d;
                 }
@@ -486,8 +506,9 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
                         const double xW = sx[SIDX(1, r) - 1], xE = sx[SIDX(0, r) + 1];
                         const double s0 = r == 0 ? xs0 : x[r - 1][0], n0 = r == R - 1 ? xn0 : x[r + 1][0];
                         const double s1 = r == 0 ? xs1 : x[r - 1][1], n1 = r == R - 1 ? xn1 : x[r + 1][1];
-                        const double w0 = row_d1(lam[r][0], x0, kappa * hW[r], xW, kappa * hM[r], x1, kappa * v[r][0], s0, kappa * v[r + 1][0], n0);
-                        const double w1 = row_d1(lam[r][1], x1, kappa * hM[r], x0, kappa * hE[r], xE, kappa * v[r][1], s1, kappa * v[r + 1][1], n1);
+                        const double k0 = XI ? __dmul_rn(kappa, xi2[r][0]) : kappa, k1 = XI ? __dmul_rn(kappa, xi2[r][1]) : kappa;
+                        const double w0 = row_d1(lam[r][0], x0, k0 * hW[r], xW, k0 * hM[r], x1, k0 * v[r][0], s0, k0 * v[r + 1][0], n0);
+                        const double w1 = row_d1(lam[r][1], x1, k1 * hM[r], x0, k1 * hE[r], xE, k1 * v[r][1], s1, k1 * v[r + 1][1], n1);
                         *reinterpret_cast<double2*>(dc + (int64_t)t * TS + ly * TX + 2 * lane) =
                             make_double2((!GEN || ((imask >> (2 * r)) & 1u)) ? w0 : 0.0, (!GEN || ((imask >> (2 * r + 1)) & 1u)) ? w1 : 0.0);
                     }
@@ -523,15 +544,15 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
 
 // One launch, two geometries: CTAs [0, ggen) run the general tiles (list smeta_g), the others the interior tiles
 // (list smeta_i); both persistent, both with their own thread count (the block carries the larger one).
-template <int HI, int HG, bool PC, int EPI, bool MP>
+template <int HI, int HG, bool PC, int EPI, bool MP, bool XI>
 __global__ void __launch_bounds__((SGeo<HI>::NT > SGeo<HG>::NT ? SGeo<HI>::NT : SGeo<HG>::NT), 1)
     k_gs_strip(LevelDev lv, const int* __restrict__ smeta_i, int nint, const int* __restrict__ smeta_g, int ngen, int ggen, int planes, VecRef xin_r,
                VecRef xout_r, VecRef b_r, const double* __restrict__ ec, int xin_zero, const uint16_t* __restrict__ ccode,
                double* __restrict__ dc, const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char strip_smem[];
     if (!MP && stopped(stop, 0)) return;
-    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true, MP>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
-    else strip_body<HI, PC, EPI, false, MP>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
+    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true, MP, XI>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
+    else strip_body<HI, PC, EPI, false, MP, XI>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
 }
 
 }  // namespace

@@ -297,3 +297,43 @@ def test_paper_annulus_mms_v55_three_fields_as_printed(gpu, oracle_mod, neumann)
     err = np.linalg.norm(host(xg)[m] - pl.meta["phi"][m]) / np.linalg.norm(pl.meta["phi"][m])
     assert err < (1.2e-2 if neumann else 1e-4)              # O(h) / O(h^2) at h = 2e-3
     s.close()
+
+
+@pytest.mark.parametrize("seed,lattice", [(311, 1025), (312, 769)])
+def test_three_field_on_the_register_tiled_smoother(gpu, oracle_mod, seed, lattice):
+    """The three-field form (Eq. 3) on levels large enough for the register-tiled smoother kernels (k_gs_strip with xi:
+    b / xi in registers, kappa xi in the epilogues): ragged domain with mixed guards, every fused variant, the cycle and the solve
+    against the oracle's three-field path; and bit-identity with the shared-memory tile code (MG_B200_NO_STRIPS is read once per
+    process, so that comparison goes through the oracle bar only here)."""
+    pl = H.random_blob_plane(seed, lattice)
+    xi = W.xi_field(pl, seed=seed)
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, max_iters=90)
+    o.update3(pl.lam, xi, pl.c)
+    s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, max_iters=90)
+    s.update_coeffs3(dev(pl.lam), dev(xi), dev(pl.c))
+    rng = np.random.default_rng(seed)
+    for lv in (0, 1):
+        n = o.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        assert rel(host(s.apply(lv, dev(x))), o.apply(lv, x)) <= TOL_STEP
+        for sweeps in (2, 3):
+            assert rel(host(s.smooth(lv, dev(x), dev(b), sweeps)), o.smooth(lv, x, b, sweeps)) <= TOL_STEP
+        xo = o.smooth(lv, x, b, 2)
+        do = o.restrict(lv, o.apply(lv, xo) - b)
+        xg, dg = s.smooth_restrict(lv, dev(x), dev(b), 2)
+        scale = np.linalg.norm(o.restrict(lv, np.abs(o.apply(lv, xo)) + np.abs(b)))
+        assert rel(host(xg), xo) <= TOL_STEP and np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
+        assert rel(host(s.vcycle(lv, dev(x), dev(b))), o.cycle(lv, x, b)) <= 1e-12
+    ro = o.solve(pl.f, pl.x0, 1e-10)
+    xs, iters, relres, rc = s.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    print(f"three-field blob {seed} {lattice}: n={pl.n} iters gpu/oracle={iters}/{ro['iters']} status {rc}/{ro['status']} rel.err={rel(host(xs), ro['x']):.2e}")
+    # (a ragged domain with a xi of contrast 30 may need more than the 90 iterations allowed here: then both sides stop at the cap
+    # with the same iterate)
+    assert rc == ro["status"] and abs(iters - ro["iters"]) <= 1 and rel(host(xs), ro["x"]) <= (TOL_SOLVE if rc == 0 else 1e-6)
+    # back to the two-field form on the same handle: the kernels without xi again
+    o.update(pl.lam, pl.c)
+    s.update_coeffs(dev(pl.lam), dev(pl.c))
+    n = o.level_n(0)
+    x, b = rng.standard_normal(n), rng.standard_normal(n)
+    assert rel(host(s.vcycle(0, dev(x), dev(b))), o.cycle(0, x, b)) <= 1e-12
+    s.close()
