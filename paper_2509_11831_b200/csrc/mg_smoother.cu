@@ -62,9 +62,13 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
                   const uint16_t* ccode, double* dc) {
     constexpr size_t smem = Geo<NS, PC, EPI, BX, BY>::SMEM;
     ensure_dyn_smem((const void*)k_gs<NS, PC, EPI, BX, BY, XIM>, smem);
-    if (NS == 2 && XIM != 2 && BX == TX && BY == TY && !no_strips()) {
-        // large level, two sweeps: interior and general tiles by the register-tiled kernel, guard-list overflow tiles by the tile code
-        constexpr int K = EPI ? 1 : 0, SH = EPI ? 6 : 4, GH = (EPI || PC) ? 8 : 6;
+    if (XIM != 2 && BX == TX && BY == TY && !no_strips()) {
+        // large level: interior and general tiles by the register-tiled kernel, guard-list overflow tiles by the tile code.  Halos
+        // (even: column pairs): interior 2 NS + epilogue (2 defect restriction, 1 apply), general 3 NS + 1 (correction) + epilogue
+        constexpr int EH = EPI == 1 ? 2 : (EPI == 2 ? 1 : 0);
+        constexpr int SH = (2 * NS + EH + 1) / 2 * 2, GH = (3 * NS + (PC ? 1 : 0) + EH + 1) / 2 * 2;
+        constexpr int K = SH <= 4 ? 0 : 1;                  // work lists: interior = all inner within 4 (K = 0) / 6 (K = 1) cells of the tile
+        static_assert(SH <= 6 && GH <= 8, "work lists and the overflow rule cover halos up to 6 / 8");
         const int nint = lv.nint[K], ngen = lv.ngen[K], novf = lv.ntiles - nint - ngen, sms = dev_info().sms;
         if (novf > 0) {
             k_gs<NS, PC, EPI, BX, BY, XIM><<<dim3(novf, L.planes), GT, smem, L.stream>>>(lv, xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop, lv.tlist[K] + nint + ngen);
@@ -84,12 +88,12 @@ void launch_blk_x(const Launch& L, const LevelDev& lv, VecRef xin, VecRef xout, 
                 if (nint > 0) ggen = std::min(ggen, grid - 1);
             }
             if (L.planes > 1) {
-                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, true, XIM == 1>, ssm);
-                k_gs_strip<SH, GH, PC, EPI, true, XIM == 1><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes,
+                ensure_dyn_smem((const void*)k_gs_strip<NS, SH, GH, PC, EPI, true, XIM == 1>, ssm);
+                k_gs_strip<NS, SH, GH, PC, EPI, true, XIM == 1><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, L.planes,
                                                                                       xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
             } else {
-                ensure_dyn_smem((const void*)k_gs_strip<SH, GH, PC, EPI, false, XIM == 1>, ssm);
-                k_gs_strip<SH, GH, PC, EPI, false, XIM == 1><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, 1,
+                ensure_dyn_smem((const void*)k_gs_strip<NS, SH, GH, PC, EPI, false, XIM == 1>, ssm);
+                k_gs_strip<NS, SH, GH, PC, EPI, false, XIM == 1><<<grid, nthreads, ssm, L.stream>>>(lv, lv.smeta[K], nint, lv.smeta[K] + (size_t)SMETA * nint, ngen, ggen, 1,
                                                                                        xin, xout, b, ec, zero ? 1 : 0, ccode, dc, L.stop);
             }
             if (L.counter) *L.counter += 1;

@@ -75,7 +75,7 @@ __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterp
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// x_out = S^2 (x_in - [PC] P e_c) on the nlist interior tiles described by smeta; EPI as in k_gs (1: d_c = R (A x_out - b), 2: w = A x_out).
+// x_out = S^NS (x_in - [PC] P e_c), NS = 1 or 2 sweeps, on the nlist tiles described by smeta; EPI as in k_gs (1: d_c = R (A x_out - b), 2: w = A x_out).
 // CTA `cta` of `ncta` walks the list entries cta, cta + ncta, ...; barriers count the NT threads of this geometry only
 // (the launch may carry more: the two geometries of k_gs_strip share one grid).
 template <int NTHREADS>
@@ -83,7 +83,7 @@ __device__ __forceinline__ void bar_sync() { asm volatile("bar.sync 0, %0;" ::"n
 
 // XI: the three-field form (Eq. 3): the smoother works on the row divided by xi — it holds b / xi, and 1/a_ll is
 // xi / a_ll (k_diag) — and the epilogues scale kappa by xi of the row's point, exactly as mg_tile_gs.cuh does.
-template <int H, bool PC, int EPI, bool GEN, bool MP, bool XI>
+template <int NS, int H, bool PC, int EPI, bool GEN, bool MP, bool XI>
 __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __restrict__ smeta, int nlist, int planes, const VecRef& xin_r,
                                            const VecRef& xout_r, const VecRef& b_r, const double* __restrict__ ec0, int xin_zero,
                                            const uint16_t* __restrict__ ccode, double* __restrict__ dc0, const int* __restrict__ stop, int cta,
@@ -92,7 +92,8 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
     constexpr int R = G::R, RWC = G::RWC, NCP = G::NCP, NRB = G::NRB, RBL = G::RBL, NT = G::NT;
     constexpr bool DR = EPI == 1, AP = EPI == 2;
     constexpr int NA = SGeo<H>::NA;                         // staged arrays: c, x (b, 1/a_ll, lambda: loaded directly, after an L2 prefetch)
-    static_assert(H >= (GEN ? 6 + (PC ? 1 : 0) : 4) + (DR ? 2 : (AP ? 1 : 0)), "halo too small for two sweeps and the epilogue");
+    // the valid region shrinks by one cell per phase: two per sweep on interior tiles, three (red, black, boundary) on general ones
+    static_assert(H >= (GEN ? 3 * NS + (PC ? 1 : 0) : 2 * NS) + (DR ? 2 : (AP ? 1 : 0)), "halo too small for NS sweeps and the epilogue");
     if ((int)threadIdx.x >= NT) return;
     double* sx = reinterpret_cast<double*>(smem_raw);       // [2][RH + 2][RWC] colour-split mirror of x
     double* sc = sx + 2 * NCP;                              // same for c; dead after the face sums: scratch of the epilogues
@@ -356,7 +357,7 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
         }
         // ---- two sweeps: red (colour 0), black (colour 1); the cell of colour col in row r is at position (r + col) & 1
 #pragma unroll
-        for (int ph = 0; ph < 4; ph++) {
+        for (int ph = 0; ph < 2 * NS; ph++) {
             const int col = ph & 1;
             const double xs = sx[SIDX(col, -1)];             // S neighbour of the updated cell of row 0 (position col)
             const double xn = sx[SIDX(1 - col, R)];          // N neighbour of the updated cell of row R - 1 (R even: position 1 - col)
@@ -544,15 +545,15 @@ __device__ __forceinline__ void strip_body(const LevelDev& lv, const int* __rest
 
 // One launch, two geometries: CTAs [0, ggen) run the general tiles (list smeta_g), the others the interior tiles
 // (list smeta_i); both persistent, both with their own thread count (the block carries the larger one).
-template <int HI, int HG, bool PC, int EPI, bool MP, bool XI>
+template <int NS, int HI, int HG, bool PC, int EPI, bool MP, bool XI>
 __global__ void __launch_bounds__((SGeo<HI>::NT > SGeo<HG>::NT ? SGeo<HI>::NT : SGeo<HG>::NT), 1)
     k_gs_strip(LevelDev lv, const int* __restrict__ smeta_i, int nint, const int* __restrict__ smeta_g, int ngen, int ggen, int planes, VecRef xin_r,
                VecRef xout_r, VecRef b_r, const double* __restrict__ ec, int xin_zero, const uint16_t* __restrict__ ccode,
                double* __restrict__ dc, const int* __restrict__ stop) {
     extern __shared__ __align__(16) unsigned char strip_smem[];
     if (!MP && stopped(stop, 0)) return;
-    if ((int)blockIdx.x < ggen) strip_body<HG, PC, EPI, true, MP, XI>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
-    else strip_body<HI, PC, EPI, false, MP, XI>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
+    if ((int)blockIdx.x < ggen) strip_body<NS, HG, PC, EPI, true, MP, XI>(lv, smeta_g, ngen, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x, ggen, strip_smem);
+    else strip_body<NS, HI, PC, EPI, false, MP, XI>(lv, smeta_i, nint, planes, xin_r, xout_r, b_r, ec, xin_zero, ccode, dc, stop, blockIdx.x - ggen, gridDim.x - ggen, strip_smem);
 }
 
 }  // namespace

@@ -198,6 +198,25 @@ def test_register_tiled_smoother_on_ragged_large_meshes(gpu, oracle_mod, seed, l
     print(f"blob {seed} {lattice}: n={pl.n} levels={o.levels} iters gpu/oracle={iters}/{ro['iters']} rel.err={rel(host(xs), ro['x']):.2e}")
     assert rc == ro["status"] == 0 and abs(iters - ro["iters"]) <= 1 and rel(host(xs), ro["x"]) <= TOL_SOLVE
     s.close()
+    # odd sweep counts: the single-sweep forms of the same kernels (sweep + restricted defect, correction + sweep, correction + sweep +
+    # apply) — V(3,1): pre-smoothing 2 + 1, post-smoothing 1
+    o31 = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=3, nu_post=1)
+    o31.update(pl.lam, pl.c)
+    s31 = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=3, nu_post=1)
+    s31.update_coeffs(dev(pl.lam), dev(pl.c))
+    for lv in (0, 1):
+        n = o31.level_n(lv)
+        x, b = rng.standard_normal(n), rng.standard_normal(n)
+        xo = o31.smooth(lv, x, b, 1)
+        do = o31.restrict(lv, o31.apply(lv, xo) - b)
+        xg, dg = s31.smooth_restrict(lv, dev(x), dev(b), 1)
+        scale = np.linalg.norm(o31.restrict(lv, np.abs(o31.apply(lv, xo)) + np.abs(b)))
+        assert rel(host(xg), xo) <= TOL_STEP and np.linalg.norm(host(dg) - do) <= TOL_STEP * max(scale, np.linalg.norm(do))
+        assert rel(host(s31.vcycle(lv, dev(x), dev(b))), o31.cycle(lv, x, b)) <= 1e-12
+    r31 = o31.solve(pl.f, pl.x0, 1e-10)
+    x31, it31, _, rc31 = s31.solve(dev(pl.f), dev(pl.x0), 1e-10)
+    assert rc31 == r31["status"] == 0 and abs(it31 - r31["iters"]) <= 1 and rel(host(x31), r31["x"]) <= TOL_SOLVE
+    s31.close()
 
 
 def test_allocator_is_captured_per_handle(gpu, oracle_mod):
