@@ -81,7 +81,8 @@ typedef struct {
                       inspection calls mg_num_levels / mg_level_n / mg_level_info / mg_transfer_info work,
                       every compute call returns MG_ECUDA.
                       bit 1 (MG_SETUP_FUSED_TAIL): run the cycle steps of the small levels (<= 148 tiles) in one
-                      cooperative kernel instead of one kernel per step (bit-identical results; off by default).
+                      cooperative kernel instead of one kernel per step (bit-identical results; off by default; ignored
+                      when planes > 1).
                       bit 2 (MG_SETUP_FULL_CGS2): always run the second Gram-Schmidt update of the Arnoldi step;
                       by default it is skipped in the steps where the measured defect ||V^T w'|| is already
                       <= 1e-13 ||w'|| (G23; same iterates to that level).
