@@ -124,3 +124,43 @@ def test_batched_planes_three_field_form(gpu, oracle_mod):
     ro = o.solve(f[1], x0[1], 1e-10)
     assert abs(its[1] - ro["iters"]) <= 1 and rel(host(xb)[1], ro["x"]) <= TOL_SOLVE
     sb.close()
+
+
+@pytest.mark.parametrize("seed", list(range(230, 238)))
+def test_random_mesh_options_planes_and_solvers(gpu, oracle_mod, seed):
+    """Seeded sweep: ragged random domain x V(nu1,nu2) x V/W/F cycle x restart length x outer solver (fGMRES / BiCGStab) x 2-4 planes
+    with per-plane coefficients and right-hand sides.  Batched == separate handles bit for bit; every plane against the oracle
+    (fGMRES: iterations +-1; BiCGStab: applications +-2, see tests/test_gpu_bicgstab.py)."""
+    rng = np.random.default_rng(seed)
+    n = int(rng.choice([97, 129, 193, 257]))
+    nu1, nu2 = max(1, int(rng.integers(0, 4))), int(rng.integers(0, 4))
+    gamma, m = int(rng.choice([1, 1, 2, 3])), int(rng.choice([5, 12, 30]))
+    solver, P = int(rng.integers(0, 2)), int(rng.integers(2, 5))
+    pl = H.random_blob_plane(seed, n)
+    lam = np.stack([pl.lam * (1.0 + 0.3 * rng.uniform(-1, 1, pl.n)) for _ in range(P)])
+    c = np.stack([pl.c * np.exp(0.3 * rng.standard_normal(pl.n)) for _ in range(P)])
+    f = np.stack([pl.f if p == 0 else rng.standard_normal(pl.n) for p in range(P)])
+    x0 = np.zeros((P, pl.n))
+    kw = dict(levels=pl.levels, nu_pre=nu1, nu_post=nu2, restart_m=m, gamma=gamma, max_iters=150, solver=solver)
+    seq = []
+    for p in range(P):
+        s = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, **kw)
+        s.update_coeffs(dev(lam[p]), dev(c[p]))
+        x, it, rr, rc = s.solve(dev(f[p]), dev(x0[p]), 1e-10)
+        seq.append((host(x), it, rr, rc))
+        s.close()
+    sb = gpu.Solver(pl.i, pl.j, pl.kind, pl.h, planes=P, **kw)
+    sb.update_coeffs(dev(lam), dev(c))
+    xb, its, rrs, rcb = sb.solve(dev(f), dev(x0), 1e-10)
+    sb.close()
+    assert rcb == max(q[3] for q in seq)
+    for p in range(P):
+        assert its[p] == seq[p][1] and rrs[p] == seq[p][2] and np.array_equal(host(xb)[p], seq[p][0]), (p, its, [q[1] for q in seq])
+    o = oracle_mod.Oracle(pl.i, pl.j, pl.kind, pl.h, levels=pl.levels, nu_pre=nu1, nu_post=nu2, m=m, gamma=gamma, max_iters=150)
+    for p in (0, P - 1):
+        o.update(lam[p], c[p])
+        ro = o.solve_bicgstab(f[p], x0[p], 1e-10) if solver else o.solve(f[p], x0[p], 1e-10)
+        if ro["status"] == 0 and seq[p][3] == 0:
+            assert abs(its[p] - ro["iters"]) <= (2 if solver else 1) and rel(host(xb)[p], ro["x"]) <= TOL_SOLVE, (p, its[p], ro["iters"])
+        else:
+            assert ro["status"] == seq[p][3] or solver == 1, (ro["status"], seq[p][3])
