@@ -359,6 +359,9 @@ __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, cons
         for (int c = 0; c < nv; c++) bulk_g2s(sv + c * K, V + (int64_t)c * stride + ci * K, K * sizeof(double), &bars[sg]);
         bulk_g2s(sv + NV * K, w + ci * K, K * sizeof(double), &bars[sg]);
     };
+    double hr[NV];                                          // the projection coefficients in registers (read once, not once per element)
+#pragma unroll
+    for (int c = 0; c < NV; c++) hr[c] = (UPDATE && c < nv) ? hh[c] : 0.0;
     for (int i = 0; i < UDT_STAGES; i++) issue(i);           // all stages in flight; a stage is refilled as soon as it is consumed
     for (int64_t i = 0; (int64_t)blockIdx.x + i * gridDim.x < nchunks; i++) {
         const int64_t ci = (int64_t)blockIdx.x + i * gridDim.x;
@@ -372,7 +375,7 @@ __device__ __forceinline__ void update_dot_tma_body(double* __restrict__ w, cons
             if (UPDATE) {
 #pragma unroll
                 for (int c = 0; c < NV; c++)
-                    if (c < nv) s -= hh[c] * sv[c * K + k];
+                    if (c < nv) s -= hr[c] * sv[c * K + k];
                 w[ci * K + k] = s;
                 accn += s * s;
             }
