@@ -24,7 +24,7 @@ def _stack(pls, name):
 
 
 @pytest.mark.parametrize("cfg,lattice,P,kw", [(2, 257, 5, {}), (3, 257, 3, dict(nu_pre=3, nu_post=1, restart_m=8)),
-                                              (3, 1025, 2, {}), (2, 129, 16, dict(gamma=2))])
+                                              (3, 1025, 2, {}), (2, 129, 16, dict(gamma=2)), (3, 257, 3, dict(restart_m=40))])
 def test_batched_planes_equal_separate_handles(gpu, oracle_mod, cfg, lattice, P, kw):
     import torch
     pls = _planes(cfg, lattice, P)
