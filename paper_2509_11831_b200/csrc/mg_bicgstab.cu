@@ -62,6 +62,11 @@ __device__ __forceinline__ bool gsum2(GmresState* st, double* __restrict__ parti
     return threadIdx.x == 0;
 }
 
+// The vectors have a multiple of 2048 entries (tile layout): 16-byte accesses, two per thread and trip in flight
+#define BI_LOOP(k2) for (int64_t k2 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k2 < (n >> 1); k2 += (int64_t)gridDim.x * blockDim.x)
+__device__ __forceinline__ double2 ld2(const double* p, int64_t k2) { return reinterpret_cast<const double2*>(p)[k2]; }
+__device__ __forceinline__ void st2(double* p, int64_t k2, double a, double b) { reinterpret_cast<double2*>(p)[k2] = make_double2(a, b); }
+
 // (re)start, rules K1 / K5: relres = |r| / |b| decides converged / restart; rhat = r, rho' = (rhat, r) = |r|^2
 __global__ void __launch_bounds__(RED_THREADS) k_bi_start(GmresState* st, const double* __restrict__ r, double* __restrict__ rhat, int64_t n) {
     st += blockIdx.y; r += blockIdx.y * n; rhat += blockIdx.y * n;
@@ -72,7 +77,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bi_start(GmresState* st, const 
     const bool broke = st->status == 3;
     __syncthreads();
     if (!conv && !capped && !broke)
-        for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) rhat[k] = r[k];
+        BI_LOOP(k2) { const double2 a = ld2(r, k2); st2(rhat, k2, a.x, a.y); }
     if (last_block(st) && threadIdx.x == 0) {
         st->relres = relres;
         if (bn == 0.0) { st->status = 4; st->cycle_end = 1; }
@@ -94,8 +99,14 @@ __global__ void __launch_bounds__(RED_THREADS) k_bi_p(GmresState* st, const doub
     const bool first = st->b_first != 0;
     const double omega = st->b_omega;
     const double beta = (st->b_rho1 / st->b_rho) * (st->b_alpha / omega);
-    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x)
-        p[k] = first ? r[k] : r[k] + beta * (p[k] - omega * v[k]);
+    BI_LOOP(k2) {
+        const double2 rr = ld2(r, k2);
+        if (first) st2(p, k2, rr.x, rr.y);
+        else {
+            const double2 pp = ld2(p, k2), vv = ld2(v, k2);
+            st2(p, k2, rr.x + beta * (pp.x - omega * vv.x), rr.y + beta * (pp.y - omega * vv.y));
+        }
+    }
 }
 
 __global__ void __launch_bounds__(RED_THREADS) k_bi_alpha(GmresState* st, const double* __restrict__ rhat, const double* __restrict__ v, int64_t n,
@@ -103,7 +114,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_bi_alpha(GmresState* st, const 
     st += blockIdx.y; rhat += blockIdx.y * n; v += blockIdx.y * n; partial += blockIdx.y * PARTIAL_PLANE;
     if (st->cycle_end) return;
     double a = 0.0, b = 0.0;
-    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) a += rhat[k] * v[k];
+    BI_LOOP(k2) { const double2 x = ld2(rhat, k2), y = ld2(v, k2); a += x.x * y.x; a += x.y * y.y; }
     if (gsum2(st, partial, a, b)) {
         if (a == 0.0) { st->status = 3; st->cycle_end = 1; st->b_skip2 = 1; }      // breakdown: (rhat, v) = 0
         else st->b_alpha = st->b_rho1 / a;
@@ -116,10 +127,11 @@ __global__ void __launch_bounds__(RED_THREADS) k_bi_s(GmresState* st, const doub
     if (st->cycle_end) return;
     const double alpha = st->b_alpha;
     double a = 0.0, b = 0.0;
-    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
-        const double sk = r[k] - alpha * v[k];
-        s[k] = sk;
-        a += sk * sk;
+    BI_LOOP(k2) {
+        const double2 rr = ld2(r, k2), vv = ld2(v, k2);
+        const double s0 = rr.x - alpha * vv.x, s1 = rr.y - alpha * vv.y;
+        st2(s, k2, s0, s1);
+        a += s0 * s0; a += s1 * s1;
     }
     if (gsum2(st, partial, a, b)) {
         st->iters += 1;                                                           // first preconditioner application of the step
@@ -134,10 +146,10 @@ __global__ void __launch_bounds__(RED_THREADS) k_bi_omega(GmresState* st, const 
     st += blockIdx.y; t += blockIdx.y * n; s += blockIdx.y * n; partial += blockIdx.y * PARTIAL_PLANE;
     if (st->cycle_end || st->b_half) return;
     double a = 0.0, b = 0.0;
-    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
-        const double tk = t[k];
-        a += tk * s[k];
-        b += tk * tk;
+    BI_LOOP(k2) {
+        const double2 tt = ld2(t, k2), ss = ld2(s, k2);
+        a += tt.x * ss.x; a += tt.y * ss.y;
+        b += tt.x * tt.x; b += tt.y * tt.y;
     }
     if (gsum2(st, partial, a, b)) {
         if (b == 0.0) { st->status = 3; st->b_half = 1; }                          // breakdown: (t, t) = 0; x still takes alpha y
@@ -155,14 +167,15 @@ __global__ void __launch_bounds__(RED_THREADS) k_bi_update(GmresState* st, doubl
     const bool half = st->b_half != 0;
     double a = 0.0, b = 0.0;
     if (half) {
-        for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) x[k] += alpha * y[k];
+        BI_LOOP(k2) { const double2 xx = ld2(x, k2), yy = ld2(y, k2); st2(x, k2, xx.x + alpha * yy.x, xx.y + alpha * yy.y); }
     } else {
-        for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) {
-            x[k] += alpha * y[k] + omega * z[k];
-            const double rk = s[k] - omega * t[k];
-            r[k] = rk;
-            a += rhat[k] * rk;
-            b += rk * rk;
+        BI_LOOP(k2) {
+            const double2 xx = ld2(x, k2), yy = ld2(y, k2), zz = ld2(z, k2), ss = ld2(s, k2), tt = ld2(t, k2), hh = ld2(rhat, k2);
+            st2(x, k2, xx.x + (alpha * yy.x + omega * zz.x), xx.y + (alpha * yy.y + omega * zz.y));
+            const double r0 = ss.x - omega * tt.x, r1 = ss.y - omega * tt.y;
+            st2(r, k2, r0, r1);
+            a += hh.x * r0; a += hh.y * r1;
+            b += r0 * r0; b += r1 * r1;
         }
     }
     if (gsum2(st, partial, a, b)) {
